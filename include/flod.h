@@ -1,0 +1,175 @@
+/*
+ * flod.h -- C ABI of the B200-native forward rasterizer for multi-level 3D Gaussian sets (FLoD, arXiv 2408.12894).
+ *
+ * Citations: P:n = PAPER.md line n, S:n = SPEC.md line n, Rk = reading k in DESIGN.md §3.
+ *
+ * The library renders a multi-level Gaussian set {G^(l)} at a single level, at the maximum level, or selectively
+ * (Eq. 6-7): for l in [l_start, l_end] a level-l Gaussian is drawn iff
+ *     d_proj^(l) <= |mu - ref| < d_proj^(l-1),   d_proj^(l) = s_min^(l) * fx / gamma,
+ *     d_proj^(l_end) = 0,  d_proj^(l_start - 1) = +inf                                   (R1-R4).
+ * Selected Gaussians are projected (mu', Sigma' of P:110, +0.3 px^2 dilation, R8-R9), binned to 16x16 tiles by the
+ * box of their alpha = 1/255 contour (R13), ordered per tile by (depth, global id) (R15) and composited front
+ * to back with alpha = min(0.99, o exp(-1/2 d^T Sigma'^-1 d)) (Eq. 2), skipping alpha < 1/255 and stopping
+ * after the blend that takes the transmittance below 1e-4 (R11-R12).
+ *
+ * Ownership: ALL device memory is allocated and owned by the caller (scene arena, workspace, output image); the
+ * library never allocates device memory, never creates streams, and never synchronises inside flod_render.
+ * Pointers named *_dev are device pointers, everything else is a host pointer.  All arrays are fp32, C-contiguous.
+ * Every function returns 0 (FLOD_OK) or a negative FLOD_E_* code; flod_last_error() gives the message.
+ * One context = one scene on one device.  Calls on one context are not thread-safe; contexts are independent.
+ * There is no CPU fallback anywhere.
+ */
+#ifndef FLOD_H
+#define FLOD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define FLOD_API __attribute__((visibility("default")))
+#else
+#define FLOD_API
+#endif
+
+#define FLOD_ABI_VERSION 1
+#define FLOD_MAX_LEVELS 16
+#define FLOD_TILE 16                 /* tiles are 16x16 pixels */
+#define FLOD_N_STAGES 4              /* 0 preprocess (a1-a6), 1 sort (a7), 2 ranges (a8), 3 blend (a9) */
+
+enum {
+    FLOD_OK = 0,
+    FLOD_E_INVALID_ARG = -1,         /* null pointer, gamma <= 0 or non-finite, fx/fy <= 0, width/height < 1, z_near < 0 */
+    FLOD_E_LEVEL_RANGE = -2,         /* not first_level <= l_start <= l_end <= last_level */
+    FLOD_E_NOT_UPLOADED = -3,        /* render / workspace query before flod_upload_levels */
+    FLOD_E_ARENA_TOO_SMALL = -4,     /* scene arena or workspace smaller than flod_*_bytes() says */
+    FLOD_E_CAPACITY = -5,            /* previous frame needed more pairs than max_pairs (reported by flod_get_stats) */
+    FLOD_E_CUDA = -6,                /* CUDA runtime error; text in flod_last_error */
+    FLOD_E_NO_WORKSPACE = -7         /* flod_render before flod_set_workspace */
+};
+
+typedef struct flod_ctx flod_ctx;    /* opaque, host side */
+
+/* One level G^(l).  Host pointers, read-only, copied by flod_upload_levels. */
+typedef struct {
+    int64_t n;                       /* number of Gaussians (may be 0) */
+    int     level;                   /* level id l, 1-based; uploaded levels are consecutive and ascending (R23) */
+    float   s_min;                   /* Eq. 3 value s_min^(l) for this level; >= 0, strictly decreasing in l */
+    const float *mean;               /* [n][3] world units */
+    const float *log_scale;          /* [n][3] log of the EFFECTIVE scale s^(l) = exp(s_opt) + s_min (Eq. 4; Alg. 1; R6) */
+    const float *quat;               /* [n][4] w,x,y,z; any non-zero norm */
+    const float *opacity_logit;      /* [n]; o = sigmoid(logit) */
+    const float *sh;                 /* [n][K][3], K = (sh_degree+1)^2, real SH of R16 */
+} flod_level_desc;
+
+/* Pinhole camera.  x_cam = R x_world + t; camera axes +x right, +y down, +z forward.
+ * Pixel (i,j) covers [i,i+1)x[j,j+1) and is sampled at (i+.5, j+.5) (R14). */
+typedef struct {
+    float R[9];                      /* row-major */
+    float t[3];
+    float fx, fy, cx, cy;            /* pixels */
+    int   width, height;
+    float z_near;                    /* cull z_cam <= z_near; must be >= 0 (R10, R24) */
+    float bg[3];                     /* background colour */
+} flod_camera;
+
+/* Which levels to render, by level id, inclusive.  Single level l = {l,l}; maximum level = {L,L};
+ * selective rendering = {l_start < l_end} (Eq. 6).  gamma is ignored (but validated) when l_start == l_end. */
+typedef struct { int l_start, l_end; } flod_level_mode;
+
+typedef struct {
+    int64_t n_scan;                  /* Gaussians in levels l_start..l_end */
+    int64_t n_sel;                   /* pass Eq. 6 */
+    int64_t n_front;                 /* selected with z_cam > z_near */
+    int64_t n_vis;                   /* also alive, det > 0, non-empty tile rect */
+    int64_t n_pairs;                 /* (Gaussian, tile) pairs the frame REQUIRES (may exceed max_pairs) */
+    int64_t max_pairs;               /* capacity given to flod_set_workspace */
+    int     overflow;                /* 1 when n_pairs > max_pairs: out_rgb of that frame is undefined */
+    int64_t evals, blends;           /* E, B of DESIGN §6 when FLOD_OPT_COUNT is on, else 0 */
+    float   ms_stage[FLOD_N_STAGES]; /* device time per stage when FLOD_OPT_PROFILE is on, else 0 */
+    float   ms_total;
+} flod_stats;
+
+enum {                               /* flod_set_options bits */
+    FLOD_OPT_DEBUG   = 1,            /* also write the selection mask and per-Gaussian projection records */
+    FLOD_OPT_PROFILE = 2,            /* record CUDA events between stages (flod_get_stats reports ms) */
+    FLOD_OPT_COUNT   = 4             /* instrumented blend kernel counting evaluations and blends */
+};
+
+enum {                               /* flod_debug_copy selectors; host_dst sizes in bytes */
+    FLOD_DBG_MASK = 0,               /* uint8[n_total]: Eq. 6 membership, zero outside the range (needs FLOD_OPT_DEBUG) */
+    FLOD_DBG_TILE_COUNTS = 1,        /* uint32[TX*TY]: pairs per tile */
+    FLOD_DBG_PROJECTED = 2,          /* flod_dbg_projected[n_vis] in ascending gid (needs FLOD_OPT_DEBUG) */
+    FLOD_DBG_SORTED_PAIRS = 3,       /* flod_dbg_pair[min(n_pairs,max_pairs)] in final order */
+    FLOD_DBG_ACTIVATED = 4           /* float[n_total][8]: Sigma xx,xy,xz,yy,yz,zz, o, kappa (kappa = -1 when dead) */
+};
+
+typedef struct {
+    uint32_t gid; float mu2d[2]; float depth; float conic[3]; float opacity; float rgb[3];
+    int32_t rect[4];                 /* tx0, ty0, tx1, ty1 */
+} flod_dbg_projected;
+
+typedef struct { uint32_t tile; float depth; uint32_t gid; } flod_dbg_pair;
+
+/* Create / destroy a context bound to CUDA device `device`.  No device memory is allocated. */
+FLOD_API int flod_create(flod_ctx **out, int device);
+FLOD_API int flod_destroy(flod_ctx *ctx);
+
+/* Bytes of the scene arena needed for these levels (only n and sh_degree are read).  0 on invalid input. */
+FLOD_API size_t flod_scene_bytes(int n_levels, const flod_level_desc *levels, int sh_degree);
+
+/* Step a0 (Eq. 1): activate on the host in fp64 (s = exp(log_scale), Sigma = R S S^T R^T,
+ * o = sigmoid, kappa = 2 ln(255 o), dead = o < 1/255), lay out as SoA planes and copy into the caller's arena.
+ * The copy is enqueued on `stream` and the call returns after it completed; host arrays may then be freed.
+ * Validates: consecutive ascending level ids, s_min >= 0 strictly decreasing, finite attributes, |mean| <= 1e15,
+ * non-zero quaternions, 0 <= sh_degree <= 3, arena 256-byte aligned and large enough (R22, R23). */
+FLOD_API int flod_upload_levels(flod_ctx *ctx, int n_levels, const flod_level_desc *levels, int sh_degree,
+                       void *scene_arena_dev, size_t arena_bytes, void *stream);
+
+/* Workspace needed to render images up to width x height with at most max_pairs (Gaussian, tile) pairs
+ * (1 <= max_pairs < 2^30; width, height <= 16384).  0 on invalid input or before upload. */
+FLOD_API size_t flod_workspace_bytes(const flod_ctx *ctx, int width, int height, int64_t max_pairs);
+
+/* Hand the workspace to the context (256-byte aligned device pointer).  width/height/max_pairs are the same
+ * values given to flod_workspace_bytes; flod_render rejects larger cameras. */
+FLOD_API int flod_set_workspace(flod_ctx *ctx, void *workspace_dev, size_t bytes, int width, int height, int64_t max_pairs);
+
+/* R2: position d_G is measured from.  NULL (default) = the camera centre of each frame;
+ * a fixed position reproduces the paper's "average training camera" or "position at the last
+ * rebuild" policies. */
+FLOD_API int flod_set_selection_reference(flod_ctx *ctx, const float ref_pos[3]);
+
+FLOD_API int flod_set_options(flod_ctx *ctx, unsigned flags);
+
+/* Steps a1-a9 for one frame, asynchronous on `stream` (a cudaStream_t passed as void*).
+ * out_rgb_dev: [3][height][width] planar fp32.  Errors detected on the host are returned here; a capacity
+ * overflow is detected on the device: the frame is not silently truncated -- out_rgb is undefined, and
+ * flod_get_stats reports overflow = 1 and the required n_pairs so the caller can grow the workspace. */
+FLOD_API int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma,
+                float *out_rgb_dev, void *stream);
+
+/* Same, end to end with HOST buffers: renders into the workspace's image and copies it to out_rgb_host
+ * ([3][height][width] fp32, ideally pinned) on `stream`, then waits for the stream. */
+FLOD_API int flod_render_to_host(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma,
+                        float *out_rgb_host, void *stream);
+
+/* Waits for the last frame's stream, then reports its counters (and FLOD_E_CAPACITY if it overflowed). */
+FLOD_API int flod_get_stats(flod_ctx *ctx, flod_stats *out);
+
+/* Copies an intermediate of the LAST rendered frame to host memory (synchronous).  `bytes` must be at least the
+ * size implied by the selector; see the FLOD_DBG_* comments. */
+FLOD_API int flod_debug_copy(flod_ctx *ctx, int what, void *host_dst, size_t bytes);
+
+/* Number of kernel launches flod_render enqueues per frame with the current options. */
+FLOD_API int flod_launches_per_frame(const flod_ctx *ctx);
+
+FLOD_API const char *flod_last_error(const flod_ctx *ctx);
+FLOD_API int flod_abi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FLOD_H */

@@ -1,0 +1,484 @@
+// Host side of libflod: the C ABI of include/flod.h.  Argument checking, step a0 (upload + activation),
+// workspace carving, per-frame constants and kernel sequencing.  No device allocation, no stream creation,
+// no synchronisation inside flod_render.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <thread>
+#include <vector>
+
+#include "flod_internal.cuh"
+
+using namespace flod;
+
+struct flod_ctx : public flod::Context {};
+
+namespace {
+
+int fail(const flod_ctx *c, int code, const std::string &msg)
+{
+    if (c) const_cast<flod_ctx *>(c)->err = msg;
+    return code;
+}
+
+#define CUDA_TRY(ctx, expr)                                                                         \
+    do {                                                                                            \
+        cudaError_t e__ = (expr);                                                                   \
+        if (e__ != cudaSuccess)                                                                     \
+            return fail(ctx, FLOD_E_CUDA, std::string(#expr) + ": " + cudaGetErrorString(e__));     \
+    } while (0)
+
+size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+int sh_stride_for(int deg) { int k = (deg + 1) * (deg + 1); return (3 * k + 3) / 4 * 4; }
+
+constexpr int kScenePlanes = 3 + 6 + 3;   // mean xyz, cov x6, opacity, kappa, log2 o
+
+size_t scene_bytes_for(int64_t n, int sh_degree)
+{
+    size_t per_plane = align_up((size_t)std::max<int64_t>(n, 1) * sizeof(float));
+    return per_plane * kScenePlanes + align_up((size_t)std::max<int64_t>(n, 1) * sh_stride_for(sh_degree) * sizeof(float));
+}
+
+// Step a0 for one Gaussian (DESIGN §2 "O0"; Eq. 1).  fp64 from the fp32 inputs, rounded once.
+void activate_one(const float *ls, const float *q, float logit, float cov[6], float *o_out, float *kappa, float *l2o)
+{
+    const double s0 = exp((double)ls[0]), s1 = exp((double)ls[1]), s2 = exp((double)ls[2]);
+    double w = q[0], x = q[1], y = q[2], z = q[3];
+    const double nrm = sqrt(((w * w + x * x) + y * y) + z * z);
+    w /= nrm; x /= nrm; y /= nrm; z /= nrm;
+    const double r[3][3] = {
+        {1.0 - 2.0 * (y * y + z * z), 2.0 * (x * y - w * z), 2.0 * (x * z + w * y)},
+        {2.0 * (x * y + w * z), 1.0 - 2.0 * (x * x + z * z), 2.0 * (y * z - w * x)},
+        {2.0 * (x * z - w * y), 2.0 * (y * z + w * x), 1.0 - 2.0 * (x * x + y * y)}};
+    const double v0 = s0 * s0, v1 = s1 * s1, v2 = s2 * s2;
+    int k = 0;
+    for (int i = 0; i < 3; ++i)
+        for (int j = i; j < 3; ++j)
+            cov[k++] = (float)((r[i][0] * v0 * r[j][0] + r[i][1] * v1 * r[j][1]) + r[i][2] * v2 * r[j][2]);
+    const float o = (float)(1.0 / (1.0 + exp(-(double)logit)));
+    const bool dead = o < (float)(1.0 / 255.0);
+    *o_out = o;
+    *kappa = dead ? -1.0f : (float)(2.0 * log(255.0 * (double)o));
+    *l2o = dead ? -126.0f : (float)log2((double)o);
+}
+
+bool finite_all(const float *p, size_t n)
+{
+    for (size_t i = 0; i < n; ++i)
+        if (!isfinite(p[i])) return false;
+    return true;
+}
+
+template <class F>
+void parallel_for(int64_t n, F f)
+{
+    unsigned hw = std::max(1u, std::min(std::thread::hardware_concurrency(), 32u));
+    if (n < 4096 || hw == 1) { f(0, n); return; }
+    std::vector<std::thread> th;
+    int64_t chunk = (n + hw - 1) / hw;
+    for (unsigned t = 0; t < hw; ++t) {
+        int64_t b = t * chunk, e = std::min<int64_t>(n, b + chunk);
+        if (b >= e) break;
+        th.emplace_back([=] { f(b, e); });
+    }
+    for (auto &t : th) t.join();
+}
+
+struct WsLayout { WorkspaceDev ws; size_t bytes; size_t zero_bytes_fixed; };
+
+// Carve the workspace.  Order: [header | ranges | pre_status] (zeroed every frame, only the used prefix of
+// pre_status), then sort_status (zeroed once), then the per-Gaussian and per-pair arrays.
+WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_pairs)
+{
+    WsLayout L{};
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return (unsigned char *)((uintptr_t)base + o); };
+    const size_t tiles = (size_t)((w + kTile - 1) / kTile) * ((h + kTile - 1) / kTile);
+    const size_t nt = (size_t)std::max<int64_t>(n_total, 1);
+    const size_t pre_blocks = (nt + kPreBlock - 1) / kPreBlock;
+    const size_t sort_blocks = ((size_t)max_pairs + kSortTile - 1) / kSortTile;
+    L.ws.hdr = (FrameHeader *)take(sizeof(FrameHeader));
+    L.ws.ranges = (uint2 *)take(tiles * sizeof(uint2));
+    L.zero_bytes_fixed = off;
+    L.ws.pre_status = (unsigned long long *)take(pre_blocks * 8);
+    L.ws.sort_status = (unsigned long long *)take(sort_blocks * kRadix * 8);
+    L.ws.gA = (float4 *)take(nt * sizeof(float4));
+    L.ws.gB = (float4 *)take(nt * sizeof(float4));
+    L.ws.cB = (float *)take(nt * sizeof(float));
+    L.ws.cgid = (uint32_t *)take(nt * sizeof(uint32_t));
+    L.ws.dbg = (flod_dbg_projected *)take(nt * sizeof(flod_dbg_projected));
+    L.ws.mask = (uint8_t *)take(nt);
+    for (int b = 0; b < 2; ++b) {
+        L.ws.keys[b] = (unsigned long long *)take((size_t)max_pairs * 8);
+        L.ws.vals[b] = (uint32_t *)take((size_t)max_pairs * 4);
+    }
+    L.ws.image = (float *)take((size_t)3 * w * h * sizeof(float));
+    L.bytes = off;
+    return L;
+}
+
+int ceil_log2(unsigned v) { int b = 0; while ((1u << b) < v) ++b; return b; }
+
+}  // namespace
+
+extern "C" {
+
+int flod_abi_version(void) { return FLOD_ABI_VERSION; }
+
+const char *flod_last_error(const flod_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int flod_create(flod_ctx **out, int device)
+{
+    if (!out) return FLOD_E_INVALID_ARG;
+    *out = nullptr;
+    int count = 0;
+    cudaError_t e = cudaGetDeviceCount(&count);
+    if (e != cudaSuccess || device < 0 || device >= count) return FLOD_E_CUDA;
+    flod_ctx *c = new flod_ctx();
+    c->device = device;
+    if (cudaSetDevice(device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) {
+        delete c;
+        return FLOD_E_CUDA;
+    }
+    for (auto &ev : c->ev) cudaEventCreate(&ev);
+    *out = c;
+    return FLOD_OK;
+}
+
+int flod_destroy(flod_ctx *ctx)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    for (auto &ev : ctx->ev) if (ev) cudaEventDestroy(ev);
+    delete ctx;
+    return FLOD_OK;
+}
+
+size_t flod_scene_bytes(int n_levels, const flod_level_desc *levels, int sh_degree)
+{
+    if (n_levels < 1 || n_levels > FLOD_MAX_LEVELS || !levels || sh_degree < 0 || sh_degree > 3) return 0;
+    int64_t n = 0;
+    for (int l = 0; l < n_levels; ++l) { if (levels[l].n < 0) return 0; n += levels[l].n; }
+    return scene_bytes_for(n, sh_degree);
+}
+
+int flod_upload_levels(flod_ctx *ctx, int n_levels, const flod_level_desc *levels, int sh_degree,
+                       void *scene_arena_dev, size_t arena_bytes, void *stream)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    if (n_levels < 1 || n_levels > FLOD_MAX_LEVELS || !levels || sh_degree < 0 || sh_degree > 3 || !scene_arena_dev)
+        return fail(ctx, FLOD_E_INVALID_ARG, "upload: bad n_levels / sh_degree / null pointer");
+    if ((uintptr_t)scene_arena_dev % 256) return fail(ctx, FLOD_E_INVALID_ARG, "upload: arena must be 256-byte aligned");
+    int64_t n = 0;
+    const int K = (sh_degree + 1) * (sh_degree + 1);
+    for (int l = 0; l < n_levels; ++l) {
+        const flod_level_desc &d = levels[l];
+        if (d.n < 0) return fail(ctx, FLOD_E_INVALID_ARG, "upload: negative count");
+        if (d.n > 0 && (!d.mean || !d.log_scale || !d.quat || !d.opacity_logit || !d.sh))
+            return fail(ctx, FLOD_E_INVALID_ARG, "upload: null attribute array");
+        if (l > 0 && d.level != levels[l - 1].level + 1)
+            return fail(ctx, FLOD_E_INVALID_ARG, "upload: level ids must be consecutive and ascending");
+        if (d.level < 1) return fail(ctx, FLOD_E_INVALID_ARG, "upload: level ids are 1-based");
+        if (!(d.s_min >= 0.0f) || !isfinite(d.s_min)) return fail(ctx, FLOD_E_INVALID_ARG, "upload: s_min must be >= 0");
+        if (l > 0 && !(d.s_min < levels[l - 1].s_min))
+            return fail(ctx, FLOD_E_INVALID_ARG, "upload: s_min must strictly decrease with the level (Eq. 3)");
+        n += d.n;
+    }
+    if (n >= (1ll << 26)) return fail(ctx, FLOD_E_INVALID_ARG, "upload: at most 2^26 - 1 Gaussians per scene");
+    if (arena_bytes < scene_bytes_for(n, sh_degree)) return fail(ctx, FLOD_E_ARENA_TOO_SMALL, "upload: arena too small");
+
+    // validate values
+    for (int l = 0; l < n_levels; ++l) {
+        const flod_level_desc &d = levels[l];
+        const size_t m = (size_t)d.n;
+        if (!m) continue;
+        if (!finite_all(d.mean, 3 * m) || !finite_all(d.log_scale, 3 * m) || !finite_all(d.quat, 4 * m) ||
+            !finite_all(d.opacity_logit, m) || !finite_all(d.sh, 3 * (size_t)K * m))
+            return fail(ctx, FLOD_E_INVALID_ARG, "upload: non-finite attribute");
+        for (size_t i = 0; i < 3 * m; ++i)
+            if (fabsf(d.mean[i]) > 1e15f) return fail(ctx, FLOD_E_INVALID_ARG, "upload: |mean| > 1e15");
+        for (size_t i = 0; i < m; ++i) {
+            const float *q = d.quat + 4 * i;
+            if (q[0] == 0.0f && q[1] == 0.0f && q[2] == 0.0f && q[3] == 0.0f)
+                return fail(ctx, FLOD_E_INVALID_ARG, "upload: zero quaternion");
+        }
+    }
+
+    // activate into a host staging image of the arena, then one copy
+    const size_t nn = (size_t)std::max<int64_t>(n, 1);
+    const size_t plane = align_up(nn * sizeof(float));
+    const int stride = sh_stride_for(sh_degree);
+    const size_t total = scene_bytes_for(n, sh_degree);
+    std::vector<unsigned char> stage(total, 0);
+    float *pl[kScenePlanes];
+    for (int i = 0; i < kScenePlanes; ++i) pl[i] = (float *)(stage.data() + plane * i);
+    float *shp = (float *)(stage.data() + plane * kScenePlanes);
+    int64_t base = 0;
+    for (int l = 0; l < n_levels; ++l) {
+        const flod_level_desc d = levels[l];
+        parallel_for(d.n, [&, d, base](int64_t b, int64_t e) {
+            for (int64_t i = b; i < e; ++i) {
+                const int64_t g = base + i;
+                pl[0][g] = d.mean[3 * i]; pl[1][g] = d.mean[3 * i + 1]; pl[2][g] = d.mean[3 * i + 2];
+                float cov[6], o, kap, l2o;
+                activate_one(d.log_scale + 3 * i, d.quat + 4 * i, d.opacity_logit[i], cov, &o, &kap, &l2o);
+                for (int k = 0; k < 6; ++k) pl[3 + k][g] = cov[k];
+                pl[9][g] = o; pl[10][g] = kap; pl[11][g] = l2o;
+                memcpy(shp + (size_t)g * stride, d.sh + (size_t)i * 3 * K, sizeof(float) * 3 * K);
+            }
+        });
+        base += d.n;
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    CUDA_TRY(ctx, cudaMemcpyAsync(scene_arena_dev, stage.data(), total, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(ctx, cudaStreamSynchronize(s));
+
+    ctx->n_levels = n_levels; ctx->first_level = levels[0].level; ctx->sh_degree = sh_degree; ctx->n_total = n;
+    ctx->level_off[0] = 0;
+    for (int l = 0; l < n_levels; ++l) { ctx->level_off[l + 1] = ctx->level_off[l] + levels[l].n; ctx->s_min[l] = levels[l].s_min; }
+    const float *dev = (const float *)scene_arena_dev;
+    auto P = [&](int i) { return (const float *)((const unsigned char *)dev + plane * i); };
+    ctx->scene.mx = P(0); ctx->scene.my = P(1); ctx->scene.mz = P(2);
+    for (int k = 0; k < 6; ++k) ctx->scene.cov[k] = P(3 + k);
+    ctx->scene.opacity = P(9); ctx->scene.kappa = P(10); ctx->scene.l2o = P(11);
+    ctx->scene.sh = P(kScenePlanes);
+    ctx->scene.sh_stride = stride; ctx->scene.sh_degree = sh_degree;
+    ctx->arena = scene_arena_dev;
+    ctx->uploaded = true; ctx->has_ws = false; ctx->rendered = false;
+    return FLOD_OK;
+}
+
+size_t flod_workspace_bytes(const flod_ctx *ctx, int width, int height, int64_t max_pairs)
+{
+    if (!ctx || !ctx->uploaded || width < 1 || height < 1 || width > 16384 || height > 16384 || max_pairs < 1 ||
+        max_pairs >= (1ll << 30))
+        return 0;
+    return carve(nullptr, ctx->n_total, width, height, max_pairs).bytes;
+}
+
+int flod_set_workspace(flod_ctx *ctx, void *workspace_dev, size_t bytes, int width, int height, int64_t max_pairs)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    if (!ctx->uploaded) return fail(ctx, FLOD_E_NOT_UPLOADED, "set_workspace: no scene uploaded");
+    size_t need = flod_workspace_bytes(ctx, width, height, max_pairs);
+    if (!need || !workspace_dev || (uintptr_t)workspace_dev % 256)
+        return fail(ctx, FLOD_E_INVALID_ARG, "set_workspace: bad size / null or unaligned pointer / max_pairs out of [1, 2^30)");
+    if (bytes < need) return fail(ctx, FLOD_E_ARENA_TOO_SMALL, "set_workspace: workspace too small");
+    WsLayout L = carve((unsigned char *)workspace_dev, ctx->n_total, width, height, max_pairs);
+    ctx->ws = L.ws;
+    ctx->ws_w = width; ctx->ws_h = height; ctx->max_pairs = max_pairs;
+    ctx->sort_blocks_max = (int)(((size_t)max_pairs + kSortTile - 1) / kSortTile);
+    ctx->pre_blocks_max = (int)(((size_t)std::max<int64_t>(ctx->n_total, 1) + kPreBlock - 1) / kPreBlock);
+    // epoch-tagged look-back words must start from a state no epoch matches
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    CUDA_TRY(ctx, cudaMemset(ctx->ws.sort_status, 0, (size_t)ctx->sort_blocks_max * kRadix * 8));
+    ctx->epoch = 0;
+    ctx->has_ws = true; ctx->rendered = false;
+    return FLOD_OK;
+}
+
+int flod_set_selection_reference(flod_ctx *ctx, const float ref_pos[3])
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    if (!ref_pos) { ctx->has_ref = false; return FLOD_OK; }
+    for (int i = 0; i < 3; ++i)
+        if (!isfinite(ref_pos[i]) || fabsf(ref_pos[i]) > 1e15f) return fail(ctx, FLOD_E_INVALID_ARG, "reference must be finite, |x| <= 1e15");
+    ctx->has_ref = true;
+    memcpy(ctx->ref, ref_pos, sizeof(float) * 3);
+    return FLOD_OK;
+}
+
+int flod_set_options(flod_ctx *ctx, unsigned flags)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    ctx->flags = flags;
+    return FLOD_OK;
+}
+
+int flod_launches_per_frame(const flod_ctx *ctx)
+{
+    if (!ctx || !ctx->has_ws) return 0;
+    int tiles = ((ctx->ws_w + kTile - 1) / kTile) * ((ctx->ws_h + kTile - 1) / kTile);
+    return 1 + (1 + sort_passes_for(ceil_log2((unsigned)tiles))) + 1 + 1;
+}
+
+int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, float *out_rgb_dev, void *stream)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    if (!cam || !out_rgb_dev) return fail(ctx, FLOD_E_INVALID_ARG, "render: null pointer");
+    if (!ctx->uploaded) return fail(ctx, FLOD_E_NOT_UPLOADED, "render: no scene uploaded");
+    if (!ctx->has_ws) return fail(ctx, FLOD_E_NO_WORKSPACE, "render: no workspace set");
+    if (!(gamma > 0.0f) || !isfinite(gamma)) return fail(ctx, FLOD_E_INVALID_ARG, "render: gamma must be finite and > 0");
+    if (!(cam->fx > 0.0f) || !(cam->fy > 0.0f) || !isfinite(cam->fx) || !isfinite(cam->fy) || cam->width < 1 || cam->height < 1)
+        return fail(ctx, FLOD_E_INVALID_ARG, "render: fx, fy must be > 0 and width, height >= 1");
+    if (!(cam->z_near >= 0.0f) || !isfinite(cam->z_near)) return fail(ctx, FLOD_E_INVALID_ARG, "render: z_near must be >= 0");
+    if (cam->width > ctx->ws_w || cam->height > ctx->ws_h)
+        return fail(ctx, FLOD_E_INVALID_ARG, "render: camera larger than the workspace was sized for");
+    for (int i = 0; i < 9; ++i) if (!isfinite(cam->R[i])) return fail(ctx, FLOD_E_INVALID_ARG, "render: non-finite R");
+    for (int i = 0; i < 3; ++i) if (!isfinite(cam->t[i]) || !isfinite(cam->bg[i])) return fail(ctx, FLOD_E_INVALID_ARG, "render: non-finite t / bg");
+    if (!isfinite(cam->cx) || !isfinite(cam->cy)) return fail(ctx, FLOD_E_INVALID_ARG, "render: non-finite principal point");
+    const int last_level = ctx->first_level + ctx->n_levels - 1;
+    if (mode.l_start < ctx->first_level || mode.l_end > last_level || mode.l_start > mode.l_end)
+        return fail(ctx, FLOD_E_LEVEL_RANGE, "render: need first_level <= l_start <= l_end <= last_level");
+
+    FrameParams p{};
+    memcpy(p.R, cam->R, sizeof(p.R)); memcpy(p.t, cam->t, sizeof(p.t)); memcpy(p.bg, cam->bg, sizeof(p.bg));
+    p.fx = cam->fx; p.fy = cam->fy; p.cx = cam->cx; p.cy = cam->cy; p.z_near = cam->z_near;
+    p.W = cam->width; p.H = cam->height;
+    p.TX = (p.W + kTile - 1) / kTile; p.TY = (p.H + kTile - 1) / kTile;
+    // per-frame constants: fp64, rounded once
+    for (int i = 0; i < 3; ++i)
+        p.centre[i] = (float)(-(((double)cam->R[i] * (double)cam->t[0] + (double)cam->R[3 + i] * (double)cam->t[1]) +
+                                (double)cam->R[6 + i] * (double)cam->t[2]));
+    for (int i = 0; i < 3; ++i) p.ref[i] = ctx->has_ref ? ctx->ref[i] : p.centre[i];
+    p.limx = (float)(1.3 * (double)cam->width / (2.0 * (double)cam->fx));
+    p.limy = (float)(1.3 * (double)cam->height / (2.0 * (double)cam->fy));
+    const int i0 = mode.l_start - ctx->first_level, i1 = mode.l_end - ctx->first_level;   // level positions
+    p.n_levels = i1 - i0 + 1;
+    p.first_gid = ctx->level_off[i0];
+    const int64_t n_scan = ctx->level_off[i1 + 1] - ctx->level_off[i0];
+    p.n_scan = (int)n_scan;
+    for (int l = i0; l <= i1; ++l) {
+        const int k = l - i0;
+        p.level_end[k] = (int)(ctx->level_off[l + 1] - ctx->level_off[i0]);
+        if (l == i1) p.lo2[k] = 0.0f;                                   // d_proj^(L_end) = 0
+        else {
+            const double d = (double)ctx->s_min[l] * (double)cam->fx / (double)gamma;   // Eq. 7
+            p.lo2[k] = (float)(d * d);
+        }
+    }
+    for (int k = 0; k < p.n_levels; ++k) p.hi2[k] = (k == 0) ? INFINITY : p.lo2[k - 1];  // d_proj^(L_start-1) = inf
+    p.max_pairs = (unsigned int)ctx->max_pairs;
+    p.n_pre_blocks = (int)((n_scan + kPreBlock - 1) / kPreBlock);
+
+    cudaStream_t s = (cudaStream_t)stream;
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    const bool prof = ctx->flags & FLOD_OPT_PROFILE;
+    // zero header + ranges + the used prefix of the look-back words (contiguous)
+    const size_t zero_bytes = (size_t)((unsigned char *)ctx->ws.pre_status - (unsigned char *)ctx->ws.hdr) + (size_t)p.n_pre_blocks * 8;
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->ws.hdr, 0, zero_bytes, s));
+    if (prof) cudaEventRecord(ctx->ev[0], s);
+    launch_preprocess(*ctx, p, s);
+    if (prof) cudaEventRecord(ctx->ev[1], s);
+    int final_buf = 0;
+    launch_sort(*ctx, ceil_log2((unsigned)(p.TX * p.TY)), &final_buf, s);
+    if (prof) cudaEventRecord(ctx->ev[2], s);
+    launch_ranges(*ctx, final_buf, s);
+    if (prof) cudaEventRecord(ctx->ev[3], s);
+    launch_blend(*ctx, p, final_buf, out_rgb_dev, s);
+    if (prof) cudaEventRecord(ctx->ev[4], s);
+    CUDA_TRY(ctx, cudaGetLastError());
+    ctx->ev_valid = prof;
+    ctx->last_stream = s; ctx->rendered = true;
+    ctx->last_n_scan = n_scan;
+    ctx->last_w = p.W; ctx->last_h = p.H; ctx->last_tx = p.TX; ctx->last_ty = p.TY; ctx->last_final_buf = final_buf;
+    return FLOD_OK;
+}
+
+int flod_render_to_host(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, float *out_rgb_host, void *stream)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    if (!out_rgb_host) return fail(ctx, FLOD_E_INVALID_ARG, "render_to_host: null pointer");
+    if (!ctx->has_ws) return fail(ctx, FLOD_E_NO_WORKSPACE, "render_to_host: no workspace set");
+    int rc = flod_render(ctx, cam, mode, gamma, ctx->ws.image, stream);
+    if (rc != FLOD_OK) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    CUDA_TRY(ctx, cudaMemcpyAsync(out_rgb_host, ctx->ws.image, (size_t)3 * cam->width * cam->height * sizeof(float),
+                                  cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(ctx, cudaStreamSynchronize(s));
+    return FLOD_OK;
+}
+
+int flod_get_stats(flod_ctx *ctx, flod_stats *out)
+{
+    if (!ctx || !out) return FLOD_E_INVALID_ARG;
+    if (!ctx->rendered) return fail(ctx, FLOD_E_INVALID_ARG, "get_stats: nothing rendered yet");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->last_stream));
+    FrameHeader h;
+    CUDA_TRY(ctx, cudaMemcpy(&h, ctx->ws.hdr, sizeof(FrameHeader), cudaMemcpyDeviceToHost));
+    memset(out, 0, sizeof(*out));
+    out->n_sel = (int64_t)h.n_sel; out->n_front = (int64_t)h.n_front; out->n_vis = (int64_t)h.n_vis;
+    out->n_pairs = (int64_t)h.n_pairs; out->max_pairs = ctx->max_pairs; out->overflow = (int)h.overflow;
+    out->evals = (int64_t)h.evals; out->blends = (int64_t)h.blends;
+    out->n_scan = ctx->last_n_scan;
+    if (ctx->ev_valid) {
+        for (int i = 0; i < FLOD_N_STAGES; ++i) cudaEventElapsedTime(&out->ms_stage[i], ctx->ev[i], ctx->ev[i + 1]);
+        cudaEventElapsedTime(&out->ms_total, ctx->ev[0], ctx->ev[FLOD_N_STAGES]);
+    }
+    if (h.overflow) return fail(ctx, FLOD_E_CAPACITY, "frame needed more pairs than max_pairs; grow the workspace and re-render");
+    return FLOD_OK;
+}
+
+int flod_debug_copy(flod_ctx *ctx, int what, void *host_dst, size_t bytes)
+{
+    if (!ctx || !host_dst) return FLOD_E_INVALID_ARG;
+    if (what == FLOD_DBG_ACTIVATED) {
+        if (!ctx->uploaded) return fail(ctx, FLOD_E_NOT_UPLOADED, "debug_copy: no scene uploaded");
+        const size_t n = (size_t)ctx->n_total;
+        if (bytes < n * 8 * sizeof(float)) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: buffer too small");
+        std::vector<float> tmp(std::max<size_t>(n, 1));
+        float *dst = (float *)host_dst;
+        const float *planes[8] = {ctx->scene.cov[0], ctx->scene.cov[1], ctx->scene.cov[2], ctx->scene.cov[3],
+                                  ctx->scene.cov[4], ctx->scene.cov[5], ctx->scene.opacity, ctx->scene.kappa};
+        for (int k = 0; k < 8; ++k) {
+            CUDA_TRY(ctx, cudaMemcpy(tmp.data(), planes[k], n * sizeof(float), cudaMemcpyDeviceToHost));
+            for (size_t i = 0; i < n; ++i) dst[i * 8 + k] = tmp[i];
+        }
+        return FLOD_OK;
+    }
+    if (!ctx->rendered) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: nothing rendered yet");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->last_stream));
+    FrameHeader h;
+    CUDA_TRY(ctx, cudaMemcpy(&h, ctx->ws.hdr, sizeof(FrameHeader), cudaMemcpyDeviceToHost));
+    switch (what) {
+        case FLOD_DBG_MASK: {
+            if (!(ctx->flags & FLOD_OPT_DEBUG)) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: MASK needs FLOD_OPT_DEBUG");
+            if (bytes < (size_t)ctx->n_total) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: buffer too small");
+            CUDA_TRY(ctx, cudaMemcpy(host_dst, ctx->ws.mask, (size_t)ctx->n_total, cudaMemcpyDeviceToHost));
+            return FLOD_OK;
+        }
+        case FLOD_DBG_TILE_COUNTS: {
+            const size_t tiles = (size_t)ctx->last_tx * ctx->last_ty;
+            if (bytes < tiles * 4) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: buffer too small");
+            std::vector<uint2> r(tiles);
+            CUDA_TRY(ctx, cudaMemcpy(r.data(), ctx->ws.ranges, tiles * sizeof(uint2), cudaMemcpyDeviceToHost));
+            uint32_t *dst = (uint32_t *)host_dst;
+            for (size_t i = 0; i < tiles; ++i) dst[i] = r[i].y - r[i].x;
+            return FLOD_OK;
+        }
+        case FLOD_DBG_PROJECTED: {
+            if (!(ctx->flags & FLOD_OPT_DEBUG)) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: PROJECTED needs FLOD_OPT_DEBUG");
+            const size_t nv = (size_t)h.n_vis;
+            if (bytes < nv * sizeof(flod_dbg_projected)) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: buffer too small");
+            CUDA_TRY(ctx, cudaMemcpy(host_dst, ctx->ws.dbg, nv * sizeof(flod_dbg_projected), cudaMemcpyDeviceToHost));
+            return FLOD_OK;
+        }
+        case FLOD_DBG_SORTED_PAIRS: {
+            const size_t np = (size_t)h.n_pairs_clamped, nv = (size_t)h.n_vis;
+            if (bytes < np * sizeof(flod_dbg_pair)) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: buffer too small");
+            std::vector<unsigned long long> k(std::max<size_t>(np, 1));
+            std::vector<uint32_t> v(std::max<size_t>(np, 1)), cg(std::max<size_t>(nv, 1));
+            CUDA_TRY(ctx, cudaMemcpy(k.data(), ctx->ws.keys[ctx->last_final_buf], np * 8, cudaMemcpyDeviceToHost));
+            CUDA_TRY(ctx, cudaMemcpy(v.data(), ctx->ws.vals[ctx->last_final_buf], np * 4, cudaMemcpyDeviceToHost));
+            CUDA_TRY(ctx, cudaMemcpy(cg.data(), ctx->ws.cgid, nv * 4, cudaMemcpyDeviceToHost));
+            flod_dbg_pair *dst = (flod_dbg_pair *)host_dst;
+            for (size_t i = 0; i < np; ++i) {
+                dst[i].tile = (uint32_t)(k[i] >> 32);
+                uint32_t bits = (uint32_t)k[i];
+                memcpy(&dst[i].depth, &bits, 4);
+                dst[i].gid = v[i] < nv ? cg[v[i]] : 0xffffffffu;
+            }
+            return FLOD_OK;
+        }
+        default:
+            return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: unknown selector");
+    }
+}
+
+}  // extern "C"

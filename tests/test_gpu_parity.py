@@ -1,0 +1,333 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle on the same seeded inputs.
+
+Bit-exact: activation, selection masks, projected geometry (mu', depth, conic, rects), per-tile pair counts,
+the sorted (tile, depth, gid) sequence, frame counters.  Floating point: colours to 1e-5, images to max-abs 1e-3
+per channel (north_star) with the envelope rule of DESIGN §3 for the 1/255 skip.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import flod_synth as fs
+import oracle
+from helpers import camera, level
+from oracle import OracleScene, SKIP_THR
+
+pytestmark = pytest.mark.gpu
+
+DELTA = 2.0 ** -16
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    from paper_2408_12894_b200 import build
+    build.build()
+    import paper_2408_12894_b200 as p
+    return p
+
+
+def make_renderer(pkg, levels, sh_degree, width, height, max_pairs=1 << 20, flags=None):
+    r = pkg.Renderer(0)
+    r.upload_levels(levels, sh_degree)
+    r.set_workspace(width, height, max_pairs)
+    r.set_options(pkg.FLOD_OPT_DEBUG if flags is None else flags)
+    return r
+
+
+def check_image(gpu, fr, tol=1e-3):
+    """north_star tolerance with the envelope rule; returns (max abs diff, number of marginal pixels)."""
+    ref = fr.composite()
+    d = np.abs(gpu.astype(np.float64) - ref)
+    bad = d > tol
+    n_marginal = 0
+    if bad.any():
+        lo = fr.composite(skip_thr=SKIP_THR * (1 - DELTA))
+        hi = fr.composite(skip_thr=SKIP_THR * (1 + DELTA))
+        mn = np.minimum(np.minimum(ref, lo), hi) - tol
+        mx = np.maximum(np.maximum(ref, lo), hi) + tol
+        marginal = (np.abs(lo - ref) > 1e-5) | (np.abs(hi - ref) > 1e-5)
+        n_marginal = int(marginal.any(axis=0).sum())
+        still = bad & ~(marginal & (gpu >= mn) & (gpu <= mx))
+        assert not still.any(), f"{int(still.sum())} channel values off by more than {tol}: max {d[still].max():.3e}"
+    return float(d.max()), n_marginal
+
+
+def check_frame(r, osc, cam, l_start, l_end, gamma, ref_pos=None, image=True):
+    """Render one frame on the GPU and compare every checked intermediate with the oracle's frame."""
+    r.set_selection_reference(ref_pos)
+    img = r.render(cam, l_start, l_end, gamma).cpu().numpy()
+    st = r.get_stats()
+    fr = osc.frame(cam, l_start, l_end, gamma, ref_pos)
+    c = fr.counts
+    assert (st["n_scan"], st["n_sel"], st["n_front"], st["n_vis"], st["n_pairs"]) == (
+        c["n_scan"], c["n_sel"], c["n_front"], c["n_vis"], c["n_pairs"])
+    # level-selection mask: bit-exact
+    assert np.array_equal(r.debug_mask(), fr.mask)
+    # per-tile pair counts: bit-exact
+    assert np.array_equal(r.debug_tile_counts(fr.TX * fr.TY), fr.tile_counts)
+    # projected records in ascending gid
+    pr = r.debug_projected(st["n_vis"])
+    vis = np.nonzero(fr.state == oracle.ST_VISIBLE)[0]
+    assert np.array_equal(pr["gid"], vis.astype(np.uint32))
+    assert np.array_equal(pr["mu2d"], fr.mu2d[vis]) and np.array_equal(pr["depth"], fr.depth[vis])
+    assert np.array_equal(pr["conic"], fr.conic[vis]) and np.array_equal(pr["rect"], fr.rect[vis])
+    assert np.array_equal(pr["opacity"], osc.opacity[vis])
+    if len(vis):
+        assert np.abs(pr["rgb"].astype(np.float64) - fr.rgb[vis]).max() <= 1e-5
+    # the sorted (tile, depth, gid) sequence is unique, so it must be identical
+    sp = r.debug_sorted_pairs(st["n_pairs"])
+    tile, depth, gid = fr.sorted_pairs()
+    assert np.array_equal(sp["tile"], tile) and np.array_equal(sp["depth"], depth) and np.array_equal(sp["gid"], gid)
+    if image:
+        return check_image(img, fr), img, fr
+    return None, img, fr
+
+
+# ------------------------------------------------------------------------------------ config 0
+
+@pytest.fixture(scope="module")
+def config0(pkg):
+    sc = fs.make_scene(0)
+    cam = fs.make_poses(0)[0]
+    return sc, cam, OracleScene(sc.levels, sc.sh_degree), make_renderer(pkg, sc.levels, sc.sh_degree, cam.width, cam.height)
+
+
+def test_activation_bit_exact(config0):
+    """Step a0 (Eq. 1): the library's host activation equals the oracle's bit for bit."""
+    sc, cam, osc, r = config0
+    act = r.debug_activated()
+    assert np.array_equal(act[:, :6], osc.cov)
+    assert np.array_equal(act[:, 6], osc.opacity)
+    dead = osc.dead.astype(bool)
+    assert np.array_equal(act[~dead, 7], osc.kappa[~dead]) and (act[dead, 7] == -1.0).all()
+
+
+def test_config0_max_level(config0):
+    sc, cam, osc, r = config0
+    (dmax, nm), img, fr = check_frame(r, osc, cam, 2, 2, 1.0)
+    assert fr.counts["n_pairs"] > 10000 and dmax <= 1e-3 + 4e-3
+
+
+def test_config0_selective(config0):
+    """BASELINE.json config 0: selective render with levels {1,2}, gamma = 1 px."""
+    sc, cam, osc, r = config0
+    (dmax, nm), img, fr = check_frame(r, osc, cam, 1, 2, 1.0)
+    m = fr.mask
+    assert 0 < m[:1000].sum() < 1000 and 0 < m[1000:].sum() < 4000
+    for gamma in (0.5, 2.0, 4.0):
+        check_frame(r, osc, cam, 1, 2, gamma)
+    check_frame(r, osc, cam, 1, 2, 1.0, ref_pos=[0.3, -0.2, 0.1])
+
+
+def test_config0_single_level_equals_selective_single_range(config0):
+    """a single-level range renders bit-identically whatever gamma is."""
+    sc, cam, osc, r = config0
+    a = r.render(cam, 1, 1, 1.0).cpu().numpy()
+    b = r.render(cam, 1, 1, 7.0).cpu().numpy()
+    assert np.array_equal(a, b)
+    check_frame(r, osc, cam, 1, 1, 1.0)
+
+
+def test_determinism(config0):
+    sc, cam, osc, r = config0
+    a = r.render(cam, 1, 2, 1.0).cpu().numpy()
+    for _ in range(3):
+        assert np.array_equal(a, r.render(cam, 1, 2, 1.0).cpu().numpy())
+
+
+def test_brute_force_parity_on_tiny_input(config0):
+    """north_star: GPU image against per-pixel compositing over ALL depth-sorted Gaussians (no tiles)."""
+    sc, cam, osc, r = config0
+    img = r.render(cam, 1, 2, 1.0).cpu().numpy()
+    fr = osc.frame(cam, 1, 2, 1.0)
+    brute = fr.composite(brute=True)
+    d = np.abs(img - brute)
+    assert np.quantile(d, 0.999) <= 1e-3 and d.max() <= 5e-3
+
+
+# ------------------------------------------------------------------------- edge cases, small scenes
+
+def _rand_levels(rng, counts, s_min, extent=1.5, sh_degree=0, zrange=(0.3, 6.0), logs=(-4.0, -1.0)):
+    out = []
+    K = (sh_degree + 1) ** 2
+    for i, n in enumerate(counts):
+        pos = np.stack([rng.uniform(-extent, extent, n), rng.uniform(-extent, extent, n), rng.uniform(*zrange, n)], axis=1)
+        sh = rng.normal(0, 0.25, (n, K, 3)); sh[:, 0, :] += 0.8
+        lv = level(i + 1, s_min[i], pos.reshape(n, 3), np.exp(rng.uniform(*logs, (n, 3))), quat=rng.normal(size=(n, 4)) + 1e-3,
+                   logit=rng.normal(0, 2.0, n), sh=sh)
+        if n == 0:
+            lv.quat = np.zeros((0, 4), np.float32)
+        out.append(lv)
+    return out
+
+
+@pytest.mark.parametrize("seed,counts,wh,deg", [
+    (1, (300, 700), (100, 60), 0),          # ragged image (not a multiple of 16)
+    (2, (1, 1), (16, 16), 1),               # one tile, one Gaussian per level
+    (3, (0, 513), (33, 17), 2),             # empty level, ragged everything
+    (4, (257, 0), (64, 48), 3),             # empty top level, block-boundary count
+    (5, (5000, 9000, 14000), (250, 130), 3),  # several preprocess blocks / sort tiles, degree 3
+    (6, (255, 256, 257), (17, 200), 0),
+])
+def test_random_scenes(pkg, seed, counts, wh, deg):
+    rng = np.random.default_rng(seed)
+    s_min = np.sort(np.exp(rng.uniform(-4, -1, len(counts))))[::-1].copy()
+    s_min[-1] = 0.0
+    lv = _rand_levels(rng, counts, s_min, sh_degree=deg)
+    cam = camera(width=wh[0], height=wh[1], f=float(rng.uniform(40, 120)), bg=tuple(rng.uniform(0, 1, 3)))
+    osc = OracleScene(lv, deg)
+    r = make_renderer(pkg, lv, deg, wh[0], wh[1], max_pairs=1 << 21)
+    L = len(counts)
+    check_frame(r, osc, cam, L, L, 1.0)
+    check_frame(r, osc, cam, 1, L, 2.0)
+    check_frame(r, osc, cam, 1, 1, 1.0)
+    r.close()
+
+
+def test_empty_scene_and_all_culled(pkg):
+    """nothing to draw -> background; also everything behind the camera / dead."""
+    lv = level(1, 0.0, np.zeros((0, 3)), 0.1)
+    lv.quat = np.zeros((0, 4), np.float32)
+    cam = camera(width=40, height=24, bg=(0.25, 0.5, 0.75))
+    r = make_renderer(pkg, [lv], 0, 40, 24)
+    img = r.render(cam, 1, 1, 1.0).cpu().numpy()
+    assert (img[0] == 0.25).all() and (img[1] == 0.5).all() and (img[2] == 0.75).all()
+    st = r.get_stats()
+    assert st["n_pairs"] == 0 and st["n_vis"] == 0 and st["n_scan"] == 0
+    r.close()
+    lv = level(1, 0.0, [[0, 0, -1.0], [0, 0, 0.1], [0, 0, 2.0]], 0.1, logit=[0.0, 0.0, -9.0])
+    r = make_renderer(pkg, [lv], 0, 40, 24)
+    osc = OracleScene([lv], 0)
+    (dmax, _), img, fr = check_frame(r, osc, cam, 1, 1, 1.0)
+    assert fr.counts["n_vis"] == 0 and (img[1] == 0.5).all()
+    r.close()
+
+
+def test_screen_filling_and_degenerate_gaussians(pkg):
+    """Maximum footprints (every tile), a Gaussian beside the frustum (Jacobian clamp R8), exact depth ties."""
+    cam = camera(width=96, height=64, f=80.0)
+    pos = [[0, 0, 1.0], [0.05, 0.02, 1.0], [6.0, 0.1, 1.0], [0, 0, 1.0], [-0.3, 0.2, 0.5], [0.0, 0.0, 0.2000001]]
+    sc = [[3.0, 3.0, 3.0], [0.5, 0.001, 0.001], [0.4, 0.4, 0.4], [0.02, 0.02, 0.02], [1.0, 0.0005, 0.3], [0.01, 0.01, 0.01]]
+    lv = level(1, 0.0, pos, np.array(sc), quat=[[1, 0, 0, 0], [0.9, 0.1, 0.3, 0.2], [1, 0, 0, 0], [1, 0, 0, 0], [0.3, 0.5, 0.1, 0.8], [1, 0, 0, 0]],
+               opacity=[0.3, 0.9, 0.8, 0.99, 0.6, 0.5], rgb=[[1, 0, 0], [0, 1, 0], [0, 0, 1], [1, 1, 0], [0, 1, 1], [1, 0, 1]])
+    r = make_renderer(pkg, [lv], 0, 96, 64)
+    osc = OracleScene([lv], 0)
+    (dmax, _), img, fr = check_frame(r, osc, cam, 1, 1, 1.0)
+    assert fr.n_tiles.max() == fr.TX * fr.TY
+    r.close()
+
+
+def test_needle_gaussians_stay_within_tolerance(pkg):
+    """DESIGN R25: long thin footprints (short axis at the dilation floor) are where the textbook exponent loses
+    precision in fp32; the factorised form keeps the image within 1e-3."""
+    rng = np.random.default_rng(12)
+    n = 400
+    pos = np.stack([rng.uniform(-2, 2, n), rng.uniform(-1.5, 1.5, n), rng.uniform(3.0, 8.0, n)], axis=1)
+    scale = np.stack([np.exp(rng.uniform(-1.0, 1.0, n)), np.full(n, 1e-4), np.full(n, 1e-4)], axis=1)
+    lv = level(1, 0.0, pos, scale, quat=rng.normal(size=(n, 4)), opacity=rng.uniform(0.3, 0.95, n), rgb=rng.uniform(0, 1, (n, 3)))
+    cam = camera(width=640, height=400, f=600.0)
+    r = make_renderer(pkg, [lv], 0, 640, 400)
+    osc = OracleScene([lv], 0)
+    (dmax, nm), img, fr = check_frame(r, osc, cam, 1, 1, 1.0)
+    r.close()
+
+
+def test_paper_rho4_ladder(pkg):
+    """R7: the paper's tau = 0.2, rho = 4 ladder through Eq. 7, selective {1..5}."""
+    rng = np.random.default_rng(40)
+    s_min = [oracle.scale_constraint(l, 0.2, 4.0, 5) for l in range(1, 6)]
+    counts = (200, 400, 800, 1600, 3200)
+    lv = _rand_levels(rng, counts, s_min, extent=20.0, zrange=(0.5, 120.0), logs=(-3.0, 0.0))
+    cam = camera(width=200, height=120, f=170.0)
+    osc = OracleScene(lv, 0)
+    r = make_renderer(pkg, lv, 0, 200, 120, max_pairs=1 << 22)
+    for rng_l in ((1, 5), (3, 5), (2, 4)):
+        for gamma in (0.5, 1.0, 4.0):
+            _, _, fr = check_frame(r, osc, cam, rng_l[0], rng_l[1], gamma)
+    r.close()
+
+
+def test_errors_and_capacity(pkg):
+    """Error conventions of include/flod.h: level range, gamma, workspace too small for the camera, capacity."""
+    rng = np.random.default_rng(9)
+    lv = _rand_levels(rng, (500, 1500), (0.05, 0.0))
+    cam = camera(width=64, height=64, f=60.0)
+    r = make_renderer(pkg, lv, 0, 64, 64, max_pairs=256)
+    for args in ((0, 1, 1.0), (1, 3, 1.0), (2, 1, 1.0)):
+        with pytest.raises(pkg.FlodError) as e:
+            r.render(cam, *args)
+        assert e.value.code == -2
+    for gamma in (0.0, -1.0, float("nan"), float("inf")):
+        with pytest.raises(pkg.FlodError) as e:
+            r.render(cam, 1, 2, gamma)
+        assert e.value.code == -1
+    with pytest.raises(pkg.FlodError):
+        r.render(camera(width=65, height=64), 1, 2, 1.0)
+    # capacity: the frame needs more than 256 pairs -> flagged, required count reported, nothing out of bounds
+    r.render(cam, 2, 2, 1.0)
+    with pytest.raises(pkg.FlodError) as e:
+        r.get_stats()
+    assert e.value.code == -5
+    st = r.get_stats(raise_on_overflow=False)
+    need = OracleScene(lv, 0).frame(cam, 2, 2, 1.0).counts["n_pairs"]
+    assert st["overflow"] == 1 and st["n_pairs"] == need > 256
+    r.set_workspace(64, 64, need)            # grow to exactly what was reported and re-render
+    r.set_options(pkg.FLOD_OPT_DEBUG)
+    check_frame(r, OracleScene(lv, 0), cam, 2, 2, 1.0)
+    r.close()
+
+
+def test_upload_validation(pkg):
+    r = pkg.Renderer(0)
+    ok = level(1, 0.1, [[0, 0, 1.0]], 0.1)
+    bad_order = [level(2, 0.1, [[0, 0, 1.0]], 0.1), level(1, 0.0, [[0, 0, 1.0]], 0.1)]
+    bad_smin = [level(1, 0.1, [[0, 0, 1.0]], 0.1), level(2, 0.2, [[0, 0, 1.0]], 0.1)]
+    nan = level(1, 0.0, [[0, float("nan"), 1.0]], 0.1)
+    zq = level(1, 0.0, [[0, 0, 1.0]], 0.1, quat=[[0, 0, 0, 0]])
+    for lv in (bad_order, bad_smin, [nan], [zq]):
+        with pytest.raises(pkg.FlodError):
+            r.upload_levels(lv, 0)
+    with pytest.raises(pkg.FlodError):
+        r.render(camera(), 1, 1, 1.0)
+    r.upload_levels([ok], 0)
+    with pytest.raises(pkg.FlodError) as e:
+        r.render(camera(), 1, 1, 1.0)
+    assert e.value.code == -7
+    r.close()
+
+
+def test_levels_need_not_start_at_one(pkg):
+    """R23 / P:326-327: a small device may hold only some levels; ids are what the mode refers to."""
+    rng = np.random.default_rng(17)
+    lv = _rand_levels(rng, (300, 600, 900), (0.1, 0.03, 0.01))
+    for i, l in enumerate(lv):
+        l.level = i + 2                       # levels 2,3,4 of a 5-level ladder; the top uploaded s_min is not 0
+    cam = camera(width=80, height=48, f=70.0)
+    osc = OracleScene(lv, 0)
+    r = make_renderer(pkg, lv, 0, 80, 48)
+    check_frame(r, osc, cam, 2, 4, 1.5)
+    check_frame(r, osc, cam, 3, 4, 1.5)
+    with pytest.raises(pkg.FlodError):
+        r.render(cam, 1, 4, 1.0)
+    r.close()
+
+
+def test_render_to_host_matches_render(config0):
+    sc, cam, osc, r = config0
+    a = r.render(cam, 1, 2, 1.0).cpu().numpy()
+    b = r.render_to_host(cam, 1, 2, 1.0).numpy()
+    assert np.array_equal(a, b)
+
+
+def test_instrumented_counts_match_oracle(pkg, config0):
+    """E and B of the blend stage (used for the FP32 roofline) against the oracle's per-pixel counts."""
+    sc, cam, osc, _ = config0
+    r = make_renderer(pkg, sc.levels, sc.sh_degree, cam.width, cam.height, flags=pkg.FLOD_OPT_COUNT | pkg.FLOD_OPT_PROFILE)
+    r.render(cam, 2, 2, 1.0)
+    st = r.get_stats()
+    _, E, B, _ = osc.frame(cam, 2, 2, 1.0).composite(stats=True)
+    assert abs(st["blends"] - int(B.sum())) <= max(20, 1e-3 * B.sum())
+    assert abs(st["evals"] - int(E.sum())) <= max(20, 1e-3 * E.sum())
+    assert st["ms_total"] > 0 and all(m >= 0 for m in st["ms_stage"])
+    r.close()
