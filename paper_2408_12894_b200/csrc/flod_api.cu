@@ -361,6 +361,8 @@ int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, flo
     // zero header + ranges + the used prefix of the look-back words (contiguous)
     const size_t zero_bytes = (size_t)((unsigned char *)ctx->ws.pre_status - (unsigned char *)ctx->ws.hdr) + (size_t)p.n_pre_blocks * 8;
     CUDA_TRY(ctx, cudaMemsetAsync(ctx->ws.hdr, 0, zero_bytes, s));
+    if (ctx->flags & FLOD_OPT_DEBUG)   // the mask is zero outside the scanned levels
+        CUDA_TRY(ctx, cudaMemsetAsync(ctx->ws.mask, 0, (size_t)std::max<int64_t>(ctx->n_total, 1), s));
     if (prof) cudaEventRecord(ctx->ev[0], s);
     launch_preprocess(*ctx, p, s);
     if (prof) cudaEventRecord(ctx->ev[1], s);

@@ -50,7 +50,7 @@ struct FrameHeader {
 struct WorkspaceDev {
     FrameHeader *hdr;
     unsigned long long *pre_status;       // [pre_blocks_max] decoupled look-back of the fused preprocess scan
-    unsigned long long *sort_status;      // [passes][sort_blocks_max][kRadix] epoch-tagged look-back
+    unsigned long long *sort_status;      // [sort_blocks_max][kRadix] epoch-tagged look-back, shared by all passes
     float4 *gA, *gB;                      // [n_total]
     float *cB;                            // [n_total]
     uint32_t *cgid;                       // [n_total] compact index -> gid

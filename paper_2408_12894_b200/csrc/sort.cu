@@ -38,7 +38,7 @@ k_sort_hist(const WorkspaceDev ws, int passes)
 constexpr unsigned int kStAgg = 1u << 30, kStIncl = 2u << 30, kStFlagMask = 3u << 30, kStValMask = (1u << 30) - 1;
 
 __global__ void __launch_bounds__(kSortThreads)
-k_onesweep(const WorkspaceDev ws, int pass, int src, unsigned int epoch, int blocks_max)
+k_onesweep(const WorkspaceDev ws, int pass, int src, unsigned int epoch)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     unsigned long long *s_keys = reinterpret_cast<unsigned long long *>(smem_raw);                  // [kSortTile]
@@ -58,7 +58,7 @@ k_onesweep(const WorkspaceDev ws, int pass, int src, unsigned int epoch, int blo
     const uint32_t *__restrict__ vin = (src ? ws.vals[1] : ws.vals[0]);
     unsigned long long *__restrict__ kout = (src ? ws.keys[0] : ws.keys[1]);
     uint32_t *__restrict__ vout = (src ? ws.vals[0] : ws.vals[1]);
-    unsigned long long *status = ws.sort_status + (size_t)pass * blocks_max * kRadix;
+    unsigned long long *status = ws.sort_status;   // shared by all passes: words are tagged with the pass epoch
 
     while (true) {
         __syncthreads();
@@ -208,7 +208,7 @@ int launch_sort(Context &c, int tile_bits, int *final_buf, cudaStream_t s)
     for (int p = 0; p < passes; ++p) {
         c.epoch += 1;
         if (c.epoch == 0) c.epoch = 1;
-        k_onesweep<<<c.sm_count * 3, kSortThreads, smem, s>>>(c.ws, p, src, c.epoch, c.sort_blocks_max);
+        k_onesweep<<<c.sm_count * 3, kSortThreads, smem, s>>>(c.ws, p, src, c.epoch);
         src ^= 1;
     }
     *final_buf = src;
