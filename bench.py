@@ -1,0 +1,368 @@
+#!/usr/bin/env python
+"""bench.py -- frames/s of the FLoD forward rasterizer on BASELINE.json's headline workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1] [--mode max|sel345]
+
+A "step" is one pass of the whole hot path (a1-a9: select, project, scan, duplicate, sort, ranges, blend) for one
+camera pose of the synthetic config.  Default workload: BASELINE.json configs[1] -- 5-level
+outdoor-like scene, 5.35M Gaussians, SH degree 3, 1237x822, 200 poses on an ellipse, max-level (level 5) render.
+One JSON line is printed by rank 0 (see DESIGN.md §7 for every key).
+
+Multi-GPU: frames are independent, so ranks are replicas that shard the pose list; there is no
+collective in the data path -- torch.distributed is used for the barrier and the max-over-ranks time only.
+
+--impl reference times the CPU oracle (oracle/) on the host cores instead (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+FP32_LANES_PER_SM = 128          # 4 SMSPs x 32 FP32 lanes (guide: B300_MICROARCH "SMSPs per SM 4", 32-wide warps)
+SM_MAX_MHZ_FALLBACK = 1965.0
+HBM_FALLBACK_GBS = 6650.0        # B200_PROFILING.md fallback
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--mode", default=None, help="max | level<l> | sel<ls><le> e.g. sel345; default per config")
+    ap.add_argument("--gamma", type=float, default=1.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--count-scale", type=float, default=1.0, help="shrink the scene (debugging only; reported)")
+    return ap.parse_args()
+
+
+def mode_levels(args, n_levels):
+    mode = args.mode or {0: "max", 1: "max", 2: "sel345", 3: "max", 4: "sel345"}[args.config]
+    if mode == "max":
+        return mode, n_levels, n_levels
+    if mode.startswith("level"):
+        l = int(mode[5:])
+        return mode, l, l
+    if mode.startswith("sel"):
+        ls, le = int(mode[3]), int(mode[-1])
+        return mode, ls, le
+    raise SystemExit(f"bad --mode {mode}")
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK)), "measured"
+    return HBM_FALLBACK_GBS, SM_MAX_MHZ_FALLBACK, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons every 200 ms during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc = index, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.index)], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------------------- reference arm
+
+def oracle_frame_seconds(osc, cam, ls, le, gamma):
+    t0 = time.perf_counter()
+    fr = osc.frame(cam, ls, le, gamma)
+    img = fr.composite()
+    return time.perf_counter() - t0, fr, img
+
+
+def crop_camera(cam, frac):
+    """A centred window holding ~frac of the image's tiles (same pose and focal length): the bounded sample."""
+    import copy
+    c = copy.copy(cam)
+    s = max(frac, 1e-4) ** 0.5
+    w = max(16, int(cam.width * s) // 16 * 16)
+    h = max(16, int(cam.height * s) // 16 * 16)
+    x0, y0 = (cam.width - w) // 2, (cam.height - h) // 2
+    c.width, c.height = w, h
+    c.cx, c.cy = float(np.float32(cam.cx - x0)), float(np.float32(cam.cy - y0))
+    return c, (w * h) / float(cam.width * cam.height)
+
+
+def run_reference(args):
+    """The CPU oracle as it stands on the host cores.  Full frames when the run fits ~150 s; otherwise every step
+    renders a centred crop (a bounded sample) and the value is frame-equivalents per second."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import flod_synth as fs
+    import oracle
+    scene = fs.make_scene(args.config, count_scale=args.count_scale)
+    cams = fs.make_poses(args.config)
+    mode, ls, le = mode_levels(args, len(scene.levels))
+    K = args.steps if args.steps is not None else 5
+    W = args.warmup if args.warmup is not None else 1
+    osc = oracle.OracleScene(scene.levels, scene.sh_degree)
+    t_full, _, _ = oracle_frame_seconds(osc, cams[0], ls, le, args.gamma)      # un-timed probe of one full frame
+    budget = 150.0 / max(K + W, 1)
+    frac = 1.0 if t_full <= budget else max(1.0 / 64.0, budget / t_full)
+    use = []
+    for k in range(W + K):
+        cam = cams[k % len(cams)]
+        use.append(crop_camera(cam, frac) if frac < 1.0 else (cam, 1.0))
+    for k in range(W):
+        oracle_frame_seconds(osc, use[k][0], ls, le, args.gamma)
+    t0 = time.perf_counter()
+    done = 0.0
+    for k in range(W, W + K):
+        oracle_frame_seconds(osc, use[k][0], ls, le, args.gamma)
+        done += use[k][1]
+    dt = time.perf_counter() - t0
+    value = done / dt
+    sample = ("full frames" if frac >= 1.0 else
+              f"each step = full-scene geometry + a centred {use[W][0].width}x{use[W][0].height} crop "
+              f"({use[W][1]:.4f} of the frame's pixels); value = frame-equivalents/s")
+    line = {
+        "impl": "reference", "metric": "frames/sec", "value": value, "unit": "frames/s", "n_gpus": args.gpus,
+        "steps": K, "warmup": W, "ms_per_step": 1e3 * dt / K, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32 geometry + f64 compositing", "data": "synthetic",
+        "config": workload_config(args, scene, cams[0], mode, ls, le),
+        "cpu_baseline": {"value": value, "unit": "frames/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "frames/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(args, scene, cam, mode, ls, le):
+    return {
+        "workload": f"BASELINE.json configs[{args.config}]: {len(scene.levels)}-level synthetic scene, "
+                    f"{scene.n_total} Gaussians, SH degree {scene.sh_degree}, {cam.width}x{cam.height}, "
+                    f"{'max-level' if mode == 'max' else mode} render (levels {ls}..{le}"
+                    + (f", gamma {args.gamma} px" if ls != le else "") + ")",
+        "levels": [ls, le], "gamma": args.gamma, "n_gaussians": scene.n_total, "width": cam.width, "height": cam.height,
+        "count_scale": args.count_scale,
+        "l2": "inputs larger than L2 (scanned level planes + SH exceed 126 MB), no flush between frames",
+        "parallelism": f"replicas x{args.gpus} (poses sharded, no collective)",
+    }
+
+
+# ---------------------------------------------------------------------------------------------- our arm
+
+def run_ours(args):
+    import torch
+    import flod_synth as fs
+    from paper_2408_12894_b200 import build as flod_build
+    flod_build.build()
+    import paper_2408_12894_b200 as pkg
+    from paper_2408_12894_b200.binding import camera_struct
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    K = args.steps if args.steps is not None else 200
+    W = args.warmup if args.warmup is not None else 10
+    W = max(W, 3)
+    scene = fs.make_scene(args.config, count_scale=args.count_scale)
+    cams = fs.make_poses(args.config)
+    mode, ls, le = mode_levels(args, len(scene.levels))
+    cs = [camera_struct(c) for c in cams]
+    cam0 = cams[0]
+    r = pkg.Renderer(local_rank)
+    scene_bytes = r.upload_levels(scene.levels, scene.sh_degree)
+    max_pairs = 32 << 20
+    ws_bytes = r.set_workspace(cam0.width, cam0.height, max_pairs)
+    out = torch.empty((3, cam0.height, cam0.width), dtype=torch.float32, device=r.device)
+    host = torch.empty((3, cam0.height, cam0.width), dtype=torch.float32, pin_memory=True)
+    from paper_2408_12894_b200.shard import max_over_ranks, pose_index
+    my_pose = lambda k: cs[pose_index(k, rank, world, len(cs))]       # poses sharded over ranks
+
+    # ---- capacity check on every pose this rank will touch (un-timed)
+    r.set_options(0)
+    need = 0
+    for k in range(min(K, len(cs))):
+        r.render(my_pose(k), ls, le, args.gamma, out)
+        need = max(need, r.get_stats(raise_on_overflow=False)["n_pairs"])
+    if need > max_pairs:
+        max_pairs = int(need * 1.25)
+        ws_bytes = r.set_workspace(cam0.width, cam0.height, max_pairs)
+
+    # ---- timed region 1: device-resident output (value)
+    for k in range(W):
+        r.render(my_pose(k), ls, le, args.gamma, out)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for k in range(K):
+        r.render(my_pose(k), ls, le, args.gamma, out)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    # ---- timed region 2: end to end through flod_render_to_host (host camera in, pinned host image out)
+    for k in range(W):
+        r.render_to_host(my_pose(k), ls, le, args.gamma, host)
+    barrier()
+    t0 = time.perf_counter()
+    for k in range(K):
+        r.render_to_host(my_pose(k), ls, le, args.gamma, host)
+    torch.cuda.synchronize()
+    ms_e2e = 1e3 * (time.perf_counter() - t0)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms, ms_e2e = max_over_ranks([ms, ms_e2e], dist, r.device)
+
+    # ---- diagnostic passes (un-timed): ns per stage with events between kernels, then E/B counts
+    n_diag = min(K, len(cs), 50)
+    r.set_options(pkg.FLOD_OPT_PROFILE)
+    stage_ms = np.zeros(4)
+    agg = dict(n_scan=0, n_sel=0, n_front=0, n_vis=0, n_pairs=0)
+    for k in range(n_diag):
+        r.render(my_pose(k), ls, le, args.gamma, out)
+        st = r.get_stats()
+        stage_ms += np.array(st["ms_stage"])
+        for key in agg:
+            agg[key] += st[key]
+    stage_ms /= n_diag
+    for key in agg:
+        agg[key] /= n_diag
+    r.set_options(pkg.FLOD_OPT_COUNT)
+    E = B = 0
+    for k in range(n_diag):
+        r.render(my_pose(k), ls, le, args.gamma, out)
+        st = r.get_stats()
+        E += st["evals"]; B += st["blends"]
+    E /= n_diag; B /= n_diag
+    r.set_options(0)
+    launches = r.launches_per_frame()
+    peak_mem = torch.cuda.max_memory_allocated(r.device)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    hbm, sm_max_mhz, peak_src = peaks()
+    sm_count = torch.cuda.get_device_properties(r.device).multi_processor_count
+    fp32_peak = sm_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12          # TFLOP/s, non-tensor FMA
+    Kc = (scene.sh_degree + 1) ** 2
+    T_n = ((cam0.width + 15) // 16) * ((cam0.height + 15) // 16)
+    tile_bits = max(0, (T_n - 1).bit_length())
+    passes = (32 + tile_bits + 7) // 8
+    P = agg["n_pairs"]
+    alg = {   # algorithmic bytes / flops per frame, DESIGN §6
+        "preprocess": 12 * agg["n_scan"] + 28 * agg["n_front"] + (4 + 12 * Kc) * agg["n_vis"] + 52 * agg["n_vis"] + 12 * P,
+        "sort": (2 * 12 * passes + 8) * P,
+        "ranges": 8 * P + 8 * T_n,
+        "blend_flops": 14 * E + 10 * B,
+    }
+    stages = {}
+    for i, name in enumerate(["preprocess", "sort", "ranges"]):
+        gbs = alg[name] / (stage_ms[i] * 1e-3) / 1e9 if stage_ms[i] > 0 else 0.0
+        stages[name] = {"ns": stage_ms[i] * 1e6, "bound": "hbm", "achieved": gbs, "peak": hbm, "unit": "GB/s",
+                        "frac": gbs / hbm, "alg_bytes": alg[name]}
+    tfl = alg["blend_flops"] / (stage_ms[3] * 1e-3) / 1e12 if stage_ms[3] > 0 else 0.0
+    stages["blend"] = {"ns": stage_ms[3] * 1e6, "bound": "alu", "achieved": tfl, "peak": fp32_peak, "unit": "TFLOP/s",
+                       "frac": tfl / fp32_peak, "alg_flops": alg["blend_flops"], "evals": E, "blends": B}
+    dominant = max(stages, key=lambda n: stages[n]["ns"])
+    roof = {k: stages[dominant][k] for k in ("bound", "achieved", "peak", "unit", "frac")}
+    roof.update({"kernel": dominant, "traffic": None, "peak_source": f"{peak_src} MEASURED_PEAKS.json" if dominant != "blend"
+                 else f"{sm_count} SMs x 128 FP32 lanes x 2 x {sm_max_mhz:.0f} MHz (DESIGN §6.3)"})
+
+    fps = world * K / (ms * 1e-3)
+    fps_e2e = world * K / (ms_e2e * 1e-3)
+    line = {
+        "metric": "frames/sec", "value": fps, "unit": "frames/s", "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic", "config": workload_config(args, scene, cam0, mode, ls, le),
+        "blended_pairs_per_sec": B * fps, "tile_pairs_per_sec": P * fps,
+        "e2e": {"value": fps_e2e, "unit": "frames/s", "h2d_bytes_per_step": 88,
+                "d2h_bytes_per_step": 3 * cam0.width * cam0.height * 4, "ms_per_step": ms_e2e / K},
+        "gpu_launches": launches * K,
+        "roofline": roof, "stages": stages,
+        "frame": {k: v for k, v in agg.items()}, "clocks": clocks,
+        "peak_device_bytes": int(peak_mem), "scene_bytes": int(scene_bytes), "workspace_bytes": int(ws_bytes),
+        "target": {"fps": 300, "met": bool(fps >= 300)},
+    }
+    if not args.no_cpu_baseline and world == 1:
+        import oracle
+        osc = oracle.OracleScene(scene.levels, scene.sh_degree)
+        dt, fr, _ = oracle_frame_seconds(osc, cams[0], ls, le, args.gamma)
+        line["cpu_baseline"] = {"value": 1.0 / dt, "unit": "frames/s", "cores": oracle.num_threads(), "kind": "oracle",
+                                "sample": "1 full frame (pose 0): selection + projection + pair sort + tiled compositing"}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -227,6 +227,7 @@ typedef struct {
     orc_pair *pairs;             /* [n_pairs] sorted by (tile, depth, gid) */
     uint32_t *tile_start;        /* [T_n + 1] */
     uint32_t *bf_list;           /* [n_bf] all gaussians with state >= ST_EMPTY_RECT, (depth,gid) order */
+    int bf_sorted;               /* bf_list is ordered on first brute-force use */
 } orc_frame;
 
 /* Eq. 7 with the two boundary overrides, squared and rounded once to fp32.
@@ -407,8 +408,6 @@ orc_frame *orc_frame_create(const orc_scene *sc, const orc_camera *cam, int l_st
             }
     }
     qsort(fr->pairs, (size_t)n_pairs, sizeof(orc_pair), cmp_pair);
-    g_sort_frame = fr;
-    qsort(fr->bf_list, (size_t)n_bf, sizeof(uint32_t), cmp_bf);
     int T_n = fr->TX * fr->TY;
     fr->tile_start = (uint32_t *)calloc((size_t)T_n + 1, sizeof(uint32_t));
     for (int64_t i = 0; i < n_pairs; ++i) fr->tile_start[fr->pairs[i].tile + 1]++;
@@ -480,6 +479,12 @@ void orc_frame_composite(const orc_frame *fr, double skip_thr, double stop_thr, 
 {
     int W = fr->cam.width, H = fr->cam.height;
     int T_n = fr->TX * fr->TY;
+    if (brute && !fr->bf_sorted) {            /* global (depth, gid) order, built on first use */
+        orc_frame *mf = (orc_frame *)fr;
+        g_sort_frame = fr;
+        qsort(mf->bf_list, (size_t)mf->n_bf, sizeof(uint32_t), cmp_bf);
+        mf->bf_sorted = 1;
+    }
 #pragma omp parallel for schedule(dynamic, 1)
     for (int tile = 0; tile < T_n; ++tile) {
         int tx = tile % fr->TX, ty = tile / fr->TX;
