@@ -2,17 +2,22 @@
 // Eq. 2: alpha = o exp(-1/2 d^T Sigma'^-1 d); "alpha blending the projected Gaussians in depth
 // order"; clamp 0.99, skip below 1/255, stop after T < 1e-4 (R11, R12).
 //
-// One CTA of 256 threads owns one 16x16 tile (thread = pixel).  The tile's sorted list is consumed in batches
-// of 256: each thread fetches one compact index (coalesced), gathers that Gaussian's 36 B of blend features
-// (L2-resident: the compacted feature arrays of a frame are ~50 MB) into shared memory, then every pixel walks
-// the batch from shared memory (broadcast reads).  The exponent is evaluated in the factorised base-2 form of
-// DESIGN R25:   e = log2(o) - (a2 w^2 + d2 dy^2),  w = dx + k dy,  alpha = min(0.99, 2^min(e, log2 o)).
-// A warp whose 32 pixels have all terminated stops issuing math; the CTA stops when every warp has.
+// One CTA of 128 threads owns one 16x16 tile; a thread owns two vertically adjacent pixels, a warp a 16x4 strip.
+// The tile's sorted list is consumed in batches of 256: threads fetch compact indices (coalesced) and gather the
+// 36 B of blend features per Gaussian (L2-resident) into shared memory.  Each warp then FILTERS the batch against
+// its own strip -- a lane tests 8 Gaussians with the exact row-segment bound of the factorised exponent
+//     e(x, y) = log2(o) - a2 w^2 - d2 dy^2,   w = (mu'x - x) + k dy          (DESIGN R25)
+// (min over x in the strip of |w| is closed-form) and the survivors are ballot-compacted, in order, into a
+// per-warp index list.  Only those are evaluated per pixel.  A filtered-out Gaussian has alpha < 2^-0.001 / 255 on
+// every pixel of the strip, so the image is bit-identical to the unfiltered loop.  A warp whose 64 pixels have
+// all terminated skips filter and loop; the CTA stops when every warp has.
 #include "flod_internal.cuh"
 
 namespace flod {
 
-constexpr int kBlendThreads = 256;
+constexpr int kBlendThreads = 128;
+constexpr int kBatch = 256;
+constexpr int kBlendWarps = kBlendThreads / 32;
 
 // 2^x on the MUFU unit (x <= 0 here; results below 2^-126 flush to 0, far under the 1/255 skip threshold)
 __device__ __forceinline__ float ex2(float x)
@@ -27,17 +32,24 @@ __global__ void __launch_bounds__(kBlendThreads)
 k_blend(const WorkspaceDev ws, int buf, float *__restrict__ out, int W, int H, int TX, int n_tiles,
         float bg0, float bg1, float bg2)
 {
-    __shared__ float4 s_a[kBlendThreads];
-    __shared__ float4 s_b[kBlendThreads];
-    __shared__ float s_c[kBlendThreads];
+    __shared__ float4 s_a[kBatch];                      // mu'x, mu'y, k, -a2
+    __shared__ float4 s_b[kBatch];                      // -d2, log2 o, r, g
+    __shared__ float s_c[kBatch];                       // b
+    __shared__ unsigned char s_list[kBlendWarps][kBatch];
 
     const int tile = blockIdx.x;
     if (tile >= n_tiles) return;
     const int tx = tile % TX, ty = tile / TX;
-    const int tid = threadIdx.x;
-    const int px = tx * kTile + (tid & 15), py = ty * kTile + (tid >> 4);
-    const bool inside = px < W && py < H;
-    const float pxc = (float)px + 0.5f, pyc = (float)py + 0.5f;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // warp = rows 4w..4w+3 of the tile; lanes 0-15 rows (4w, 4w+1), lanes 16-31 rows (4w+2, 4w+3)
+    const int px = tx * kTile + (lane & 15);
+    const int py0 = ty * kTile + warp * 4 + (lane >> 4) * 2, py1 = py0 + 1;
+    const bool in0 = px < W && py0 < H, in1 = px < W && py1 < H;
+    const float pxc = (float)px + 0.5f, pyc0 = (float)py0 + 0.5f, pyc1 = (float)py1 + 0.5f;
+    // the warp's strip, for the filter: pixel centres x in [sx0, sx1], rows sy + {0,1,2,3}
+    const float sx0 = (float)(tx * kTile) + 0.5f, sx1 = sx0 + 15.0f;
+    const float sy = (float)(ty * kTile + warp * 4) + 0.5f;
+    const float kThr = -7.994353436858858f - 1.0e-3f;  // log2(1/255) minus a safety margin
 
     const uint2 rg = ws.ranges[tile];
     const uint32_t *__restrict__ vals = (buf ? ws.vals[1] : ws.vals[0]);
@@ -45,54 +57,109 @@ k_blend(const WorkspaceDev ws, int buf, float *__restrict__ out, int W, int H, i
     const float4 *__restrict__ gB = ws.gB;
     const float *__restrict__ cB = ws.cB;
 
-    float T = 1.0f, Cr = 0.0f, Cg = 0.0f, Cb = 0.0f;
-    bool done = !inside;
+    float T0 = 1.0f, r0 = 0.0f, g0 = 0.0f, b0 = 0.0f;
+    float T1 = 1.0f, r1 = 0.0f, g1 = 0.0f, b1 = 0.0f;
+    bool done0 = !in0, done1 = !in1;
     unsigned int n_eval = 0, n_blend = 0;
+    unsigned char *my_list = s_list[warp];
 
-    for (unsigned int base = rg.x; base < rg.y; base += kBlendThreads) {
-        if (__syncthreads_count(!done) == 0) break;
-        const unsigned int m = min((unsigned int)kBlendThreads, rg.y - base);
-        if ((unsigned int)tid < m) {
-            const uint32_t ci = vals[base + tid];
-            s_a[tid] = gA[ci];
-            s_b[tid] = gB[ci];
-            s_c[tid] = cB[ci];
+    for (unsigned int base = rg.x; base < rg.y; base += kBatch) {
+        const bool warp_done = __all_sync(0xffffffffu, done0 && done1);
+        if (__syncthreads_count(!warp_done) == 0) break;
+        const unsigned int m = min((unsigned int)kBatch, rg.y - base);
+#pragma unroll
+        for (int h = 0; h < kBatch / kBlendThreads; ++h) {
+            const unsigned int j = tid + h * kBlendThreads;
+            if (j < m) {
+                const uint32_t ci = vals[base + j];
+                s_a[j] = gA[ci];
+                s_b[j] = gB[ci];
+                s_c[j] = cB[ci];
+            }
         }
         __syncthreads();
-        if (!__all_sync(0xffffffffu, done)) {
-            for (unsigned int j = 0; j < m; ++j) {
+        if (warp_done) continue;
+
+        // ---- filter: which Gaussians of the batch can reach alpha >= 1/255 somewhere on this warp's strip
+        unsigned int cnt = 0;
+#pragma unroll
+        for (int i = 0; i < kBatch / 32; ++i) {
+            const unsigned int j = lane + 32 * i;
+            bool hit = false;
+            if (j < m) {
                 const float4 a = s_a[j];
                 const float4 b = s_b[j];
-                const float dx = a.x - pxc, dy = a.y - pyc;
-                const float w = fmaf(a.z, dy, dx);
-                float e = b.y - fmaf(a.w, w * w, b.x * (dy * dy));
-                e = fminf(e, b.y);                                   // q >= 0 (oracle clamps q at 0)
-                float alpha = fminf(ex2(e), 0.99f);
-                if (COUNT && !done) ++n_eval;
-                if (done || alpha < (1.0f / 255.0f)) continue;
-                const float wgt = T * alpha;
-                Cr = fmaf(wgt, b.z, Cr);
-                Cg = fmaf(wgt, b.w, Cg);
-                Cb = fmaf(wgt, s_c[j], Cb);
-                T = T - wgt;                                         // T (1 - alpha)
-                if (COUNT) ++n_blend;
-                if (T < 1e-4f) done = true;                          // blend, then stop (R12)
+                const float dxl = a.x - sx1, dxh = a.x - sx0;        // range of (mu'x - x) over the strip
+                float best = -INFINITY;
+#pragma unroll
+                for (int rr = 0; rr < 4; ++rr) {
+                    const float dy = a.y - (sy + (float)rr);
+                    const float kd = a.z * dy;
+                    const float wmin = fmaxf(fmaxf(dxl + kd, -(dxh + kd)), 0.0f);
+                    const float e = fmaf(a.w, wmin * wmin, fmaf(b.x, dy * dy, b.y));
+                    best = fmaxf(best, e);
+                }
+                hit = best >= kThr;
+            }
+            const unsigned int bal = __ballot_sync(0xffffffffu, hit);
+            if (hit) my_list[cnt + __popc(bal & ((1u << lane) - 1))] = (unsigned char)j;
+            cnt += __popc(bal);
+        }
+        __syncwarp();
+
+        // ---- evaluate the survivors, two pixels per thread
+        for (unsigned int t = 0; t < cnt; ++t) {
+            const unsigned int j = my_list[t];
+            const float4 a = s_a[j];
+            const float4 b = s_b[j];
+            const float dx = a.x - pxc;
+            const float dy0 = a.y - pyc0, dy1 = a.y - pyc1;
+            const float w0 = fmaf(a.z, dy0, dx), w1 = fmaf(a.z, dy1, dx);
+            float e0 = fmaf(a.w, w0 * w0, fmaf(b.x, dy0 * dy0, b.y));
+            float e1 = fmaf(a.w, w1 * w1, fmaf(b.x, dy1 * dy1, b.y));
+            e0 = fminf(e0, b.y);                                      // q >= 0 (the oracle clamps q at 0)
+            e1 = fminf(e1, b.y);
+            const float al0 = fminf(ex2(e0), 0.99f), al1 = fminf(ex2(e1), 0.99f);
+            const bool u0 = !done0 && al0 >= (1.0f / 255.0f);
+            const bool u1 = !done1 && al1 >= (1.0f / 255.0f);
+            if (u0 || u1) {
+                const float cb = s_c[j];
+                if (u0) {
+                    const float wgt = T0 * al0;
+                    r0 = fmaf(wgt, b.z, r0); g0 = fmaf(wgt, b.w, g0); b0 = fmaf(wgt, cb, b0);
+                    T0 -= wgt;                                        // T (1 - alpha)
+                    if (T0 < 1e-4f) { done0 = true; if (COUNT) n_eval += (base - rg.x) + j + 1; }   // blend, then stop (R12)
+                    if (COUNT) ++n_blend;
+                }
+                if (u1) {
+                    const float wgt = T1 * al1;
+                    r1 = fmaf(wgt, b.z, r1); g1 = fmaf(wgt, b.w, g1); b1 = fmaf(wgt, cb, b1);
+                    T1 -= wgt;
+                    if (T1 < 1e-4f) { done1 = true; if (COUNT) n_eval += (base - rg.x) + j + 1; }
+                    if (COUNT) ++n_blend;
+                }
             }
         }
     }
-    if (inside) {
-        const size_t o = (size_t)py * W + px, plane = (size_t)W * H;
-        out[o] = fmaf(T, bg0, Cr);
-        out[plane + o] = fmaf(T, bg1, Cg);
-        out[2 * plane + o] = fmaf(T, bg2, Cb);
+    const size_t plane = (size_t)W * H;
+    if (in0) {
+        const size_t o = (size_t)py0 * W + px;
+        out[o] = fmaf(T0, bg0, r0); out[plane + o] = fmaf(T0, bg1, g0); out[2 * plane + o] = fmaf(T0, bg2, b0);
+    }
+    if (in1) {
+        const size_t o = (size_t)py1 * W + px;
+        out[o] = fmaf(T1, bg0, r1); out[plane + o] = fmaf(T1, bg1, g1); out[2 * plane + o] = fmaf(T1, bg2, b1);
     }
     if (COUNT) {
+        // E as the oracle defines it: list entries visited before the pixel terminated (filtered ones included)
+        if (in0 && !done0) n_eval += rg.y - rg.x;
+        if (in1 && !done1) n_eval += rg.y - rg.x;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             n_eval += __shfl_xor_sync(0xffffffffu, n_eval, o);
             n_blend += __shfl_xor_sync(0xffffffffu, n_blend, o);
         }
-        if ((tid & 31) == 0) {
+        if (lane == 0) {
             atomicAdd(&ws.hdr->evals, (unsigned long long)n_eval);
             atomicAdd(&ws.hdr->blends, (unsigned long long)n_blend);
         }

@@ -46,7 +46,7 @@ struct FrameHeader {
 };
 
 // Blend features of one visible Gaussian (compact index): see DESIGN R25.
-//   gA = (mu'x, mu'y, k = B/A, a2 = A log2(e)/2)     gB = (d2 = (C - B^2/A) log2(e)/2, log2 o, r, g)    cB = b
+//   gA = (mu'x, mu'y, k = B/A, -A log2(e)/2)     gB = (-(C - B^2/A) log2(e)/2, log2 o, r, g)    cB = b
 struct WorkspaceDev {
     FrameHeader *hdr;
     unsigned long long *pre_status;       // [pre_blocks_max] decoupled look-back of the fused preprocess scan

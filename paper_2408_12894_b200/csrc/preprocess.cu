@@ -256,8 +256,8 @@ k_preprocess(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ F
         const double LOG2E = 1.4426950408889634;
         double dA = (double)cA, dB = (double)cB, dC = (double)cC;
         float kk = (float)(dB / dA);
-        float a2 = (float)(0.5 * LOG2E * dA);
-        float d2 = (float)(0.5 * LOG2E * (dC - dB * dB / dA));
+        float a2 = (float)(-0.5 * LOG2E * dA);                       // stored negated: e = log2 o + a2 w^2 + d2 dy^2
+        float d2 = (float)(-0.5 * LOG2E * (dC - dB * dB / dA));
         ws.gA[ci] = make_float4(mx2, my2, kk, a2);
         ws.gB[ci] = make_float4(d2, __ldg(sc.l2o + g), rgb[0], rgb[1]);
         ws.cB[ci] = rgb[2];
