@@ -87,10 +87,10 @@ void parallel_for(int64_t n, F f)
     for (auto &t : th) t.join();
 }
 
-struct WsLayout { WorkspaceDev ws; size_t bytes; size_t zero_bytes_fixed; };
+struct WsLayout { WorkspaceDev ws; size_t bytes; size_t sort_blocks; };
 
-// Carve the workspace.  Order: [header | ranges | pre_status] (zeroed every frame, only the used prefix of
-// pre_status), then sort_status (zeroed once), then the per-Gaussian and per-pair arrays.
+// Carve the workspace.  Order: [header | ranges | scan_status] (zeroed every frame, only the used prefix of
+// scan_status), then sort_status (zeroed once), then the per-Gaussian and per-pair arrays.
 WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_pairs)
 {
     WsLayout L{};
@@ -99,20 +99,27 @@ WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_p
     const size_t tiles = (size_t)((w + kTile - 1) / kTile) * ((h + kTile - 1) / kTile);
     const size_t nt = (size_t)std::max<int64_t>(n_total, 1);
     const size_t pre_blocks = (nt + kPreBlock - 1) / kPreBlock;
-    const size_t sort_blocks = ((size_t)max_pairs + kSortTile - 1) / kSortTile;
+    L.sort_blocks = std::max((nt + kDepthSortTile - 1) / kDepthSortTile, ((size_t)max_pairs + kTileSortTile - 1) / kTileSortTile);
+    const size_t tkey_bytes = tile_sort_plan((int)tiles).wide ? 4 : 2;
     L.ws.hdr = (FrameHeader *)take(sizeof(FrameHeader));
     L.ws.ranges = (uint2 *)take(tiles * sizeof(uint2));
-    L.zero_bytes_fixed = off;
-    L.ws.pre_status = (unsigned long long *)take(pre_blocks * 8);
-    L.ws.sort_status = (unsigned long long *)take(sort_blocks * kRadix * 8);
+    L.ws.scan_status = (unsigned long long *)take(pre_blocks * 16);
+    L.ws.sort_status = (unsigned long long *)take(L.sort_blocks * kRadix * 8);
     L.ws.gA = (float4 *)take(nt * sizeof(float4));
     L.ws.gB = (float4 *)take(nt * sizeof(float4));
     L.ws.cB = (float *)take(nt * sizeof(float));
+    L.ws.dirgid = (float4 *)take(nt * sizeof(float4));
+    L.ws.rect = (ushort4 *)take(nt * sizeof(ushort4));
     L.ws.cgid = (uint32_t *)take(nt * sizeof(uint32_t));
+    L.ws.depth = (uint32_t *)take(nt * sizeof(uint32_t));
+    for (int b = 0; b < 2; ++b) {
+        L.ws.dkeys[b] = (uint32_t *)take(nt * sizeof(uint32_t));
+        L.ws.dvals[b] = (uint32_t *)take(nt * sizeof(uint32_t));
+    }
     L.ws.dbg = (flod_dbg_projected *)take(nt * sizeof(flod_dbg_projected));
     L.ws.mask = (uint8_t *)take(nt);
     for (int b = 0; b < 2; ++b) {
-        L.ws.keys[b] = (unsigned long long *)take((size_t)max_pairs * 8);
+        L.ws.tkeys[b] = (void *)take((size_t)max_pairs * tkey_bytes);
         L.ws.vals[b] = (uint32_t *)take((size_t)max_pairs * 4);
     }
     L.ws.image = (float *)take((size_t)3 * w * h * sizeof(float));
@@ -120,7 +127,6 @@ WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_p
     return L;
 }
 
-int ceil_log2(unsigned v) { int b = 0; while ((1u << b) < v) ++b; return b; }
 
 }  // namespace
 
@@ -227,7 +233,18 @@ int flod_upload_levels(flod_ctx *ctx, int n_levels, const flod_level_desc *level
                 activate_one(d.log_scale + 3 * i, d.quat + 4 * i, d.opacity_logit[i], cov, &o, &kap, &l2o);
                 for (int k = 0; k < 6; ++k) pl[3 + k][g] = cov[k];
                 pl[9][g] = o; pl[10][g] = kap; pl[11][g] = l2o;
-                memcpy(shp + (size_t)g * stride, d.sh + (size_t)i * 3 * K, sizeof(float) * 3 * K);
+                float *dst = shp + (size_t)g * stride;
+                const float *src = d.sh + (size_t)i * 3 * K;
+                if (sh_degree == 3) {
+                    // 4-lane row layout of k_colour: lane j owns coefficients 4j..4j+3 = source floats [12j, 12j+12);
+                    // its floats [4i, 4i+4) are float4 number 4i + j of the row
+                    for (int f = 0; f < 48; ++f) {
+                        const int j = f / 12, within = f % 12;
+                        dst[((within / 4) * 4 + j) * 4 + (within % 4)] = src[f];
+                    }
+                } else {
+                    memcpy(dst, src, sizeof(float) * 3 * K);
+                }
             }
         });
         base += d.n;
@@ -271,7 +288,7 @@ int flod_set_workspace(flod_ctx *ctx, void *workspace_dev, size_t bytes, int wid
     WsLayout L = carve((unsigned char *)workspace_dev, ctx->n_total, width, height, max_pairs);
     ctx->ws = L.ws;
     ctx->ws_w = width; ctx->ws_h = height; ctx->max_pairs = max_pairs;
-    ctx->sort_blocks_max = (int)(((size_t)max_pairs + kSortTile - 1) / kSortTile);
+    ctx->sort_blocks_max = (int)L.sort_blocks;
     ctx->pre_blocks_max = (int)(((size_t)std::max<int64_t>(ctx->n_total, 1) + kPreBlock - 1) / kPreBlock);
     // epoch-tagged look-back words must start from a state no epoch matches
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
@@ -302,8 +319,10 @@ int flod_set_options(flod_ctx *ctx, unsigned flags)
 int flod_launches_per_frame(const flod_ctx *ctx)
 {
     if (!ctx || !ctx->has_ws) return 0;
-    int tiles = ((ctx->ws_w + kTile - 1) / kTile) * ((ctx->ws_h + kTile - 1) / kTile);
-    return 1 + (1 + sort_passes_for(ceil_log2((unsigned)tiles))) + 1 + 1;
+    const int tiles = ((ctx->ws_w + kTile - 1) / kTile) * ((ctx->ws_h + kTile - 1) / kTile);
+    const TileSortPlan pl = tile_sort_plan(tiles);
+    // geometry, colour, depth histogram + 4 passes, duplication, tile histogram + passes, ranges, blend
+    return 2 + (1 + kDepthPasses) + 1 + (pl.passes ? 1 + pl.passes : 0) + 1 + 1;
 }
 
 int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, float *out_rgb_dev, void *stream)
@@ -354,25 +373,27 @@ int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, flo
     for (int k = 0; k < p.n_levels; ++k) p.hi2[k] = (k == 0) ? INFINITY : p.lo2[k - 1];  // d_proj^(L_start-1) = inf
     p.max_pairs = (unsigned int)ctx->max_pairs;
     p.n_pre_blocks = (int)((n_scan + kPreBlock - 1) / kPreBlock);
+    p.n_tiles = p.TX * p.TY;
 
     cudaStream_t s = (cudaStream_t)stream;
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     const bool prof = ctx->flags & FLOD_OPT_PROFILE;
     // zero header + ranges + the used prefix of the look-back words (contiguous)
-    const size_t zero_bytes = (size_t)((unsigned char *)ctx->ws.pre_status - (unsigned char *)ctx->ws.hdr) + (size_t)p.n_pre_blocks * 8;
+    const size_t zero_bytes = (size_t)((unsigned char *)ctx->ws.scan_status - (unsigned char *)ctx->ws.hdr) + (size_t)p.n_pre_blocks * 16;
     CUDA_TRY(ctx, cudaMemsetAsync(ctx->ws.hdr, 0, zero_bytes, s));
     if (ctx->flags & FLOD_OPT_DEBUG)   // the mask is zero outside the scanned levels
         CUDA_TRY(ctx, cudaMemsetAsync(ctx->ws.mask, 0, (size_t)std::max<int64_t>(ctx->n_total, 1), s));
-    if (prof) cudaEventRecord(ctx->ev[0], s);
-    launch_preprocess(*ctx, p, s);
-    if (prof) cudaEventRecord(ctx->ev[1], s);
-    int final_buf = 0;
-    launch_sort(*ctx, ceil_log2((unsigned)(p.TX * p.TY)), &final_buf, s);
-    if (prof) cudaEventRecord(ctx->ev[2], s);
-    launch_ranges(*ctx, final_buf, s);
-    if (prof) cudaEventRecord(ctx->ev[3], s);
-    launch_blend(*ctx, p, final_buf, out_rgb_dev, s);
-    if (prof) cudaEventRecord(ctx->ev[4], s);
+    int stage = 0;
+    auto mark = [&]() { if (prof) cudaEventRecord(ctx->ev[stage], s); ++stage; };
+    int depth_buf = 0, final_buf = 0;
+    mark(); launch_geometry(*ctx, p, s);
+    mark(); launch_colour(*ctx, p, s);
+    mark(); if (p.n_pre_blocks > 0) launch_depth_sort(*ctx, &depth_buf, s);
+    mark(); launch_duplicate(*ctx, p, depth_buf, s);
+    mark(); if (p.n_pre_blocks > 0) launch_tile_sort(*ctx, p, &final_buf, s);
+    mark(); if (p.n_pre_blocks > 0) launch_ranges(*ctx, p, final_buf, s);
+    mark(); launch_blend(*ctx, p, final_buf, out_rgb_dev, s);
+    mark();
     CUDA_TRY(ctx, cudaGetLastError());
     ctx->ev_valid = prof;
     ctx->last_stream = s; ctx->rendered = true;
@@ -464,17 +485,20 @@ int flod_debug_copy(flod_ctx *ctx, int what, void *host_dst, size_t bytes)
         case FLOD_DBG_SORTED_PAIRS: {
             const size_t np = (size_t)h.n_pairs_clamped, nv = (size_t)h.n_vis;
             if (bytes < np * sizeof(flod_dbg_pair)) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: buffer too small");
-            std::vector<unsigned long long> k(std::max<size_t>(np, 1));
-            std::vector<uint32_t> v(std::max<size_t>(np, 1)), cg(std::max<size_t>(nv, 1));
-            CUDA_TRY(ctx, cudaMemcpy(k.data(), ctx->ws.keys[ctx->last_final_buf], np * 8, cudaMemcpyDeviceToHost));
+            const bool wide = tile_sort_plan(ctx->last_tx * ctx->last_ty).wide;
+            std::vector<unsigned char> k(std::max<size_t>(np, 1) * (wide ? 4 : 2));
+            std::vector<uint32_t> v(std::max<size_t>(np, 1)), cg(std::max<size_t>(nv, 1)), dz(std::max<size_t>(nv, 1));
+            CUDA_TRY(ctx, cudaMemcpy(k.data(), ctx->ws.tkeys[ctx->last_final_buf], np * (wide ? 4 : 2), cudaMemcpyDeviceToHost));
             CUDA_TRY(ctx, cudaMemcpy(v.data(), ctx->ws.vals[ctx->last_final_buf], np * 4, cudaMemcpyDeviceToHost));
             CUDA_TRY(ctx, cudaMemcpy(cg.data(), ctx->ws.cgid, nv * 4, cudaMemcpyDeviceToHost));
+            CUDA_TRY(ctx, cudaMemcpy(dz.data(), ctx->ws.depth, nv * 4, cudaMemcpyDeviceToHost));
             flod_dbg_pair *dst = (flod_dbg_pair *)host_dst;
             for (size_t i = 0; i < np; ++i) {
-                dst[i].tile = (uint32_t)(k[i] >> 32);
-                uint32_t bits = (uint32_t)k[i];
+                dst[i].tile = wide ? ((const uint32_t *)k.data())[i] : (uint32_t)((const uint16_t *)k.data())[i];
+                const uint32_t ci = v[i];
+                const uint32_t bits = ci < nv ? dz[ci] : 0u;
                 memcpy(&dst[i].depth, &bits, 4);
-                dst[i].gid = v[i] < nv ? cg[v[i]] : 0xffffffffu;
+                dst[i].gid = ci < nv ? cg[ci] : 0xffffffffu;
             }
             return FLOD_OK;
         }

@@ -1,10 +1,9 @@
-// Steps a1-a6 of the hot path in ONE kernel:
-//   a1 level selection (Eq. 6-7)         a2 cull + view transform
-//   a3 EWA projection, conic, tile rect     a4 SH -> RGB
-//   a5 exclusive scan of visible / tile counts      a6 (tile | depth) key duplication
-// One thread per scanned Gaussian; a decoupled look-back over blocks (ordered by an atomic ticket) gives every
-// block its compact-index base and pair base, so projected features are written compacted and pairs are emitted
-// in ascending gid, row-major tile order with a block-cooperative, perfectly coalesced expansion.
+// Steps a1-a4 of the hot path:
+//   k_geometry  a1 level selection (Eq. 6-7), a2 cull + view transform, a3 EWA projection, conic,
+//               tile rect, and the ordered compaction of the visible Gaussians (+ the frame's pair total);
+//   k_colour    a4 SH -> RGB over the compacted visible Gaussians.
+// k_geometry: one thread per scanned Gaussian; a decoupled look-back over blocks (ordered by an atomic ticket) gives
+// every block its compact-index base, so visible Gaussians get compact indices in ascending gid.
 //
 // The geometry (a1-a3 and the rect) is the canonical fp32 sequence of DESIGN §2: each operation is one IEEE
 // round-to-nearest binary32 operation (the *_rn intrinsics are never contracted into FMAs), in the written order.
@@ -29,67 +28,77 @@ __device__ __forceinline__ float fdiv(float a, float b) { return __fdiv_rn(a, b)
 #define SH_C3D 0.3731763325901154f    /* 1/4 sqrt(7/pi)        */
 #define SH_C3E 1.445305721320277f     /* 1/4 sqrt(105/pi)      */
 
+// The 16 real SH basis values of DESIGN R16 at the unit direction (x, y, z), up to degree DEG.
 template <int DEG>
-__device__ __forceinline__ void sh_to_rgb(const float *__restrict__ row, float dx, float dy, float dz, float rgb[3])
+__device__ __forceinline__ void sh_basis(float x, float y, float z, float *Y)
 {
-    constexpr int K = (DEG + 1) * (DEG + 1);
-    constexpr int NF = (3 * K + 3) / 4 * 4;
-    float f[NF];
-    const float4 *r4 = reinterpret_cast<const float4 *>(row);
-#pragma unroll
-    for (int i = 0; i < NF / 4; ++i) {
-        float4 v = __ldg(r4 + i);
-        f[4 * i] = v.x; f[4 * i + 1] = v.y; f[4 * i + 2] = v.z; f[4 * i + 3] = v.w;
-    }
-    float Y[K];
     Y[0] = SH_C0;
     if constexpr (DEG >= 1) {
-        float inv = 1.0f / sqrtf(dx * dx + dy * dy + dz * dz);
-        float x = dx * inv, y = dy * inv, z = dz * inv;
         Y[1] = -SH_C1 * y; Y[2] = SH_C1 * z; Y[3] = -SH_C1 * x;
-        if constexpr (DEG >= 2) {
-            float xx = x * x, yy = y * y, zz = z * z;
-            Y[4] = SH_C2A * x * y;
-            Y[5] = -SH_C2A * y * z;
-            Y[6] = SH_C2B * (2.0f * zz - xx - yy);
-            Y[7] = -SH_C2A * x * z;
-            Y[8] = SH_C2C * (xx - yy);
-            if constexpr (DEG >= 3) {
-                Y[9] = -SH_C3A * y * (3.0f * xx - yy);
-                Y[10] = SH_C3B * x * y * z;
-                Y[11] = -SH_C3C * y * (4.0f * zz - xx - yy);
-                Y[12] = SH_C3D * z * (2.0f * zz - 3.0f * xx - 3.0f * yy);
-                Y[13] = -SH_C3C * x * (4.0f * zz - xx - yy);
-                Y[14] = SH_C3E * z * (xx - yy);
-                Y[15] = -SH_C3A * x * (xx - 3.0f * yy);
-            }
+    }
+    if constexpr (DEG >= 2) {
+        const float xx = x * x, yy = y * y, zz = z * z;
+        Y[4] = SH_C2A * x * y;
+        Y[5] = -SH_C2A * y * z;
+        Y[6] = SH_C2B * (2.0f * zz - xx - yy);
+        Y[7] = -SH_C2A * x * z;
+        Y[8] = SH_C2C * (xx - yy);
+        if constexpr (DEG >= 3) {
+            Y[9] = -SH_C3A * y * (3.0f * xx - yy);
+            Y[10] = SH_C3B * x * y * z;
+            Y[11] = -SH_C3C * y * (4.0f * zz - xx - yy);
+            Y[12] = SH_C3D * z * (2.0f * zz - 3.0f * xx - 3.0f * yy);
+            Y[13] = -SH_C3C * x * (4.0f * zz - xx - yy);
+            Y[14] = SH_C3E * z * (xx - yy);
+            Y[15] = -SH_C3A * x * (xx - 3.0f * yy);
         }
     }
-    float r = 0.5f, g = 0.5f, b = 0.5f;
-#pragma unroll
-    for (int k = 0; k < K; ++k) {
-        r = fmaf(Y[k], f[3 * k], r);
-        g = fmaf(Y[k], f[3 * k + 1], g);
-        b = fmaf(Y[k], f[3 * k + 2], b);
-    }
-    rgb[0] = fmaxf(r, 0.0f); rgb[1] = fmaxf(g, 0.0f); rgb[2] = fmaxf(b, 0.0f);
 }
 
 constexpr unsigned long long kFlagAgg = 1ull << 62, kFlagIncl = 2ull << 62, kFlagMask = 3ull << 62;
 constexpr int kVisShift = 36;
 constexpr unsigned long long kPairMask = (1ull << kVisShift) - 1, kVisMask = (1ull << 26) - 1;
 
-template <int DEG, bool DEBUG>
+// Warp 0 of a block: publish this block's aggregate and sum the aggregates of all blocks before it (decoupled
+// look-back, 32 predecessors per step).  Returns the exclusive prefix in every lane of the warp.
+__device__ __forceinline__ unsigned long long lookback(unsigned long long *status, int stride, unsigned int vb,
+                                                       unsigned long long agg, int lane)
+{
+    unsigned long long excl = 0;
+    if (vb == 0) {
+        if (lane == 0) atomicExch(status, kFlagIncl | agg);
+        return 0;
+    }
+    if (lane == 0) atomicExch(status + (size_t)vb * stride, kFlagAgg | agg);
+    long long j = (long long)vb - 1;
+    while (true) {
+        const long long idx = j - lane;
+        unsigned long long st = kFlagIncl;                 // lanes before block 0 read "inclusive 0"
+        if (idx >= 0) {
+            volatile unsigned long long *ptr = status + (size_t)idx * stride;
+            do { st = *ptr; } while ((st & kFlagMask) == 0);
+        }
+        const unsigned int incl_mask = __ballot_sync(0xffffffffu, (st & kFlagMask) == kFlagIncl);
+        const unsigned long long val = st & ~kFlagMask;
+        const int first = incl_mask ? (__ffs(incl_mask) - 1) : 31;
+        unsigned long long contrib = (lane <= first) ? val : 0ull;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) contrib += __shfl_xor_sync(0xffffffffu, contrib, o);
+        excl += contrib;
+        if (incl_mask) break;
+        j -= 32;
+    }
+    if (lane == 0) atomicExch(status + (size_t)vb * stride, kFlagIncl | (excl + agg));
+    return excl;
+}
+
+template <bool DEBUG>
 __global__ void __launch_bounds__(kPreBlock)
-k_preprocess(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ FrameParams p)
+k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ FrameParams p)
 {
     __shared__ unsigned int s_vb;
     __shared__ unsigned long long s_warp_tot[kPreBlock / 32];
     __shared__ unsigned long long s_base;           // packed exclusive prefix of this block (status format)
-    __shared__ unsigned int s_incl[kPreBlock];      // inclusive pair scan by local visible rank
-    __shared__ unsigned int s_rect[kPreBlock];      // tx0 | ty0 << 16
-    __shared__ unsigned int s_wd[kPreBlock];        // rect width
-    __shared__ unsigned int s_depth[kPreBlock];     // depth bits
     __shared__ unsigned int s_cnt[2];               // n_sel, n_front of the block
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -173,7 +182,7 @@ k_preprocess(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ F
         }
     }
 
-    // ---- a5: block scan of (visible, n_tiles), packed vis << 40 | tiles
+    // ---- block scan of (visible, n_tiles), packed vis << 40 | tiles
     unsigned long long v = ((unsigned long long)(vis ? 1 : 0) << 40) | n_tiles;
     unsigned long long incl = v;
 #pragma unroll
@@ -198,44 +207,21 @@ k_preprocess(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ F
     const unsigned int block_vis = (unsigned int)(block_tot >> 40);
     const unsigned long long block_pairs = block_tot & ((1ull << 40) - 1);
     const unsigned int rank = (unsigned int)(incl >> 40) - (vis ? 1u : 0u);          // local visible rank
-    const unsigned int pair_incl = (unsigned int)(incl & ((1ull << 40) - 1));
 
     // ---- decoupled look-back over the blocks before this one (warp 0)
     if (warp == 0) {
         const unsigned long long agg = ((unsigned long long)block_vis << kVisShift) | block_pairs;
-        unsigned long long excl = 0;
-        if (vb == 0) {
-            if (lane == 0) atomicExch(ws.pre_status + 0, kFlagIncl | agg);
-        } else {
-            if (lane == 0) atomicExch(ws.pre_status + vb, kFlagAgg | agg);
-            long long j = (long long)vb - 1;
-            while (true) {
-                long long idx = j - lane;
-                unsigned long long st = kFlagIncl;                 // lanes before block 0 read "inclusive 0"
-                if (idx >= 0) {
-                    volatile unsigned long long *ptr = ws.pre_status + idx;
-                    do { st = *ptr; } while ((st & kFlagMask) == 0);
-                }
-                unsigned int incl_mask = __ballot_sync(0xffffffffu, (st & kFlagMask) == kFlagIncl);
-                unsigned long long val = st & ~kFlagMask;
-                int first = incl_mask ? (__ffs(incl_mask) - 1) : 31;
-                unsigned long long contrib = (lane <= first) ? val : 0ull;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) contrib += __shfl_xor_sync(0xffffffffu, contrib, o);
-                excl += contrib;
-                if (incl_mask) break;
-                j -= 32;
-            }
-            if (lane == 0) atomicExch(ws.pre_status + vb, kFlagIncl | (excl + agg));
-        }
+        const unsigned long long excl = lookback(ws.scan_status, 2, vb, agg, lane);
         if (lane == 0) {
             s_base = excl;
-            atomicAdd(&ws.hdr->n_sel, (unsigned long long)s_cnt[0]);
-            atomicAdd(&ws.hdr->n_front, (unsigned long long)s_cnt[1]);
+            if (s_cnt[0]) atomicAdd(&ws.hdr->n_sel, (unsigned long long)s_cnt[0]);
+            if (s_cnt[1]) atomicAdd(&ws.hdr->n_front, (unsigned long long)s_cnt[1]);
             if (vb == (unsigned int)p.n_pre_blocks - 1) {          // the last block knows the frame totals
-                unsigned long long tot = excl + agg;
-                unsigned long long np = tot & kPairMask;
-                ws.hdr->n_vis = (tot >> kVisShift) & kVisMask;
+                const unsigned long long tot = excl + agg;
+                const unsigned long long np = tot & kPairMask;
+                const unsigned long long nv = (tot >> kVisShift) & kVisMask;
+                ws.hdr->n_vis = nv;
+                ws.hdr->n_vis32 = (unsigned int)nv;
                 ws.hdr->n_pairs = np;
                 ws.hdr->n_pairs_clamped = (unsigned int)(np < p.max_pairs ? np : p.max_pairs);
                 ws.hdr->overflow = np > p.max_pairs ? 1u : 0u;
@@ -243,82 +229,124 @@ k_preprocess(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ F
         }
     }
     __syncthreads();
-    const unsigned long long base = s_base;
-    const unsigned int vis_base = (unsigned int)((base >> kVisShift) & kVisMask);
-    const unsigned long long pair_base = base & kPairMask;
+    if (!vis) return;
+    const unsigned int ci = (unsigned int)((s_base >> kVisShift) & kVisMask) + rank;
 
-    // ---- write the compacted blend features (+ a4 colour) of visible Gaussians
-    if (vis) {
-        const unsigned int ci = vis_base + rank;
-        float rgb[3];
-        sh_to_rgb<DEG>(sc.sh + (size_t)g * sc.sh_stride, wx - p.centre[0], wy - p.centre[1], wz - p.centre[2], rgb);
-        // DESIGN R25: factorised exponent from the ROUNDED conic, derived in fp64, rounded once
-        const double LOG2E = 1.4426950408889634;
-        double dA = (double)cA, dB = (double)cB, dC = (double)cC;
-        float kk = (float)(dB / dA);
-        float a2 = (float)(-0.5 * LOG2E * dA);                       // stored negated: e = log2 o + a2 w^2 + d2 dy^2
-        float d2 = (float)(-0.5 * LOG2E * (dC - dB * dB / dA));
-        ws.gA[ci] = make_float4(mx2, my2, kk, a2);
-        ws.gB[ci] = make_float4(d2, __ldg(sc.l2o + g), rgb[0], rgb[1]);
-        ws.cB[ci] = rgb[2];
-        ws.cgid[ci] = (uint32_t)g;
-        if (DEBUG) {
-            flod_dbg_projected d;
-            d.gid = (uint32_t)g; d.mu2d[0] = mx2; d.mu2d[1] = my2; d.depth = pz;
-            d.conic[0] = cA; d.conic[1] = cB; d.conic[2] = cC; d.opacity = __ldg(sc.opacity + g);
-            d.rgb[0] = rgb[0]; d.rgb[1] = rgb[1]; d.rgb[2] = rgb[2];
-            d.rect[0] = tx0; d.rect[1] = ty0; d.rect[2] = tx1; d.rect[3] = ty1;
-            ws.dbg[ci] = d;
-        }
-        s_incl[rank] = pair_incl;
-        s_rect[rank] = (unsigned int)tx0 | ((unsigned int)ty0 << 16);
-        s_wd[rank] = (unsigned int)(tx1 - tx0);
-        s_depth[rank] = __float_as_uint(pz);
-    }
-    __syncthreads();
-
-    // ---- a6: block-cooperative expansion, one pair per thread per step, coalesced stores
-    unsigned long long *__restrict__ keys = ws.keys[0];
-    uint32_t *__restrict__ vals = ws.vals[0];
-    for (unsigned long long q = tid; q < block_pairs; q += kPreBlock) {
-        const unsigned int qq = (unsigned int)q;
-        int lo = 0, hi = (int)block_vis - 1;           // first rank with s_incl[rank] > qq
-        while (lo < hi) {
-            int mid = (lo + hi) >> 1;
-            if (s_incl[mid] > qq) hi = mid; else lo = mid + 1;
-        }
-        const unsigned int r = (unsigned int)lo;
-        const unsigned int start = r ? s_incl[r - 1] : 0u;
-        const unsigned int k = qq - start;
-        const unsigned int w = s_wd[r];
-        const unsigned int ry = k / w, rx = k - ry * w;
-        const unsigned int rc = s_rect[r];
-        const unsigned int tile = ((rc >> 16) + ry) * (unsigned int)p.TX + ((rc & 0xffffu) + rx);
-        const unsigned long long dst = pair_base + q;
-        if (dst < p.max_pairs) {
-            keys[dst] = ((unsigned long long)tile << 32) | s_depth[r];
-            vals[dst] = vis_base + r;
-        }
+    // ---- per-visible records, compact index ci (ascending gid)
+    // DESIGN R25: factorised exponent from the ROUNDED conic, derived in fp64, rounded once
+    const double LOG2E = 1.4426950408889634;
+    const double dA = (double)cA, dB = (double)cB, dC = (double)cC;
+    const float kk = (float)(dB / dA);
+    const float a2 = (float)(-0.5 * LOG2E * dA);                       // stored negated: e = log2 o + a2 w^2 + d2 dy^2
+    const float d2 = (float)(-0.5 * LOG2E * (dC - dB * dB / dA));
+    ws.gA[ci] = make_float4(mx2, my2, kk, a2);
+    reinterpret_cast<float2 *>(ws.gB)[2 * (size_t)ci] = make_float2(d2, __ldg(sc.l2o + g));   // (r, g) by k_colour
+    ws.rect[ci] = make_ushort4((unsigned short)tx0, (unsigned short)ty0, (unsigned short)tx1, (unsigned short)ty1);
+    ws.depth[ci] = __float_as_uint(pz);
+    ws.dirgid[ci] = make_float4(wx - p.centre[0], wy - p.centre[1], wz - p.centre[2], __uint_as_float((unsigned int)g));
+    ws.cgid[ci] = (uint32_t)g;
+    if (DEBUG) {
+        flod_dbg_projected d;
+        d.gid = (uint32_t)g; d.mu2d[0] = mx2; d.mu2d[1] = my2; d.depth = pz;
+        d.conic[0] = cA; d.conic[1] = cB; d.conic[2] = cC; d.opacity = __ldg(sc.opacity + g);
+        d.rgb[0] = 0.0f; d.rgb[1] = 0.0f; d.rgb[2] = 0.0f;                                    // by k_colour
+        d.rect[0] = tx0; d.rect[1] = ty0; d.rect[2] = tx1; d.rect[3] = ty1;
+        ws.dbg[ci] = d;
     }
 }
 
-template <int DEG>
-static void launch_deg(const Context &c, const FrameParams &p, cudaStream_t s)
+// ---- a4: colour of every visible Gaussian.  rgb = max(0, 0.5 + sum_k Y_k(dir) sh_k)  (R16)
+// LANES threads share one Gaussian.  LANES = 4 needs the degree-3 row layout written by the upload: the row is 12
+// float4; float4 number (4 i + j), i = 0..2, holds floats [4 i, 4 i + 4) of the 12 floats (k, channel) of the
+// coefficients k = 4 j .. 4 j + 3, so one load instruction of the 4 lanes reads 64 contiguous bytes.
+template <int DEG, int LANES, bool DEBUG>
+__global__ void __launch_bounds__(256)
+k_colour(const SceneDev sc, const WorkspaceDev ws)
 {
-    if (c.flags & FLOD_OPT_DEBUG)
-        k_preprocess<DEG, true><<<p.n_pre_blocks, kPreBlock, 0, s>>>(c.scene, c.ws, p);
-    else
-        k_preprocess<DEG, false><<<p.n_pre_blocks, kPreBlock, 0, s>>>(c.scene, c.ws, p);
+    constexpr int K = (DEG + 1) * (DEG + 1);
+    const unsigned int n_vis = ws.hdr->n_vis32;
+    const unsigned int sub = threadIdx.x % LANES;
+    const unsigned int per_block = 256 / LANES;
+    for (unsigned int base = blockIdx.x * per_block; base < n_vis; base += gridDim.x * per_block) {
+        const unsigned int ci = base + threadIdx.x / LANES;
+        const bool ok = ci < n_vis;
+        float r = 0.0f, g = 0.0f, b = 0.0f;
+        if (ok) {
+            const float4 dg = ws.dirgid[ci];
+            const float *row = sc.sh + (size_t)__float_as_uint(dg.w) * sc.sh_stride;
+            float Y[K];
+            const float inv = DEG >= 1 ? 1.0f / sqrtf(dg.x * dg.x + dg.y * dg.y + dg.z * dg.z) : 0.0f;
+            if constexpr (LANES == 4) {
+                static_assert(DEG == 3 || LANES == 1, "4-lane layout is degree 3 only");
+                const float4 *r4 = reinterpret_cast<const float4 *>(row);
+                const float4 f0 = __ldg(r4 + sub), f1 = __ldg(r4 + 4 + sub), f2 = __ldg(r4 + 8 + sub);
+                sh_basis<DEG>(dg.x * inv, dg.y * inv, dg.z * inv, Y);
+                const float y0 = sub == 0 ? Y[0] : sub == 1 ? Y[4] : sub == 2 ? Y[8] : Y[12];
+                const float y1 = sub == 0 ? Y[1] : sub == 1 ? Y[5] : sub == 2 ? Y[9] : Y[13];
+                const float y2 = sub == 0 ? Y[2] : sub == 1 ? Y[6] : sub == 2 ? Y[10] : Y[14];
+                const float y3 = sub == 0 ? Y[3] : sub == 1 ? Y[7] : sub == 2 ? Y[11] : Y[15];
+                r = fmaf(y0, f0.x, fmaf(y1, f0.w, fmaf(y2, f1.z, y3 * f2.y)));
+                g = fmaf(y0, f0.y, fmaf(y1, f1.x, fmaf(y2, f1.w, y3 * f2.z)));
+                b = fmaf(y0, f0.z, fmaf(y1, f1.y, fmaf(y2, f2.x, y3 * f2.w)));
+            } else {
+                constexpr int NF = (3 * K + 3) / 4 * 4;
+                float f[NF];
+                const float4 *r4 = reinterpret_cast<const float4 *>(row);
+#pragma unroll
+                for (int q = 0; q < NF / 4; ++q) {
+                    const float4 t = __ldg(r4 + q);
+                    f[4 * q] = t.x; f[4 * q + 1] = t.y; f[4 * q + 2] = t.z; f[4 * q + 3] = t.w;
+                }
+                sh_basis<DEG>(dg.x * inv, dg.y * inv, dg.z * inv, Y);
+#pragma unroll
+                for (int k = 0; k < K; ++k) {
+                    r = fmaf(Y[k], f[3 * k], r);
+                    g = fmaf(Y[k], f[3 * k + 1], g);
+                    b = fmaf(Y[k], f[3 * k + 2], b);
+                }
+            }
+        }
+        if constexpr (LANES == 4) {
+#pragma unroll
+            for (int o = 1; o < 4; o <<= 1) {
+                r += __shfl_xor_sync(0xffffffffu, r, o);
+                g += __shfl_xor_sync(0xffffffffu, g, o);
+                b += __shfl_xor_sync(0xffffffffu, b, o);
+            }
+        }
+        if (ok && sub == 0) {
+            r = fmaxf(r + 0.5f, 0.0f); g = fmaxf(g + 0.5f, 0.0f); b = fmaxf(b + 0.5f, 0.0f);
+            reinterpret_cast<float2 *>(ws.gB)[2 * (size_t)ci + 1] = make_float2(r, g);
+            ws.cB[ci] = b;
+            if (DEBUG) { ws.dbg[ci].rgb[0] = r; ws.dbg[ci].rgb[1] = g; ws.dbg[ci].rgb[2] = b; }
+        }
+    }
 }
 
-int launch_preprocess(const Context &c, const FrameParams &p, cudaStream_t s)
+int launch_geometry(const Context &c, const FrameParams &p, cudaStream_t s)
 {
     if (p.n_pre_blocks <= 0) return 0;
+    if (c.flags & FLOD_OPT_DEBUG) k_geometry<true><<<p.n_pre_blocks, kPreBlock, 0, s>>>(c.scene, c.ws, p);
+    else k_geometry<false><<<p.n_pre_blocks, kPreBlock, 0, s>>>(c.scene, c.ws, p);
+    return 1;
+}
+
+template <int DEG, int LANES>
+static void launch_colour_t(const Context &c, int grid, cudaStream_t s)
+{
+    if (c.flags & FLOD_OPT_DEBUG) k_colour<DEG, LANES, true><<<grid, 256, 0, s>>>(c.scene, c.ws);
+    else k_colour<DEG, LANES, false><<<grid, 256, 0, s>>>(c.scene, c.ws);
+}
+
+int launch_colour(const Context &c, const FrameParams &p, cudaStream_t s)
+{
+    if (p.n_pre_blocks <= 0) return 0;
+    const int grid = c.sm_count * 8;
     switch (c.sh_degree) {
-        case 0: launch_deg<0>(c, p, s); break;
-        case 1: launch_deg<1>(c, p, s); break;
-        case 2: launch_deg<2>(c, p, s); break;
-        default: launch_deg<3>(c, p, s); break;
+        case 0: launch_colour_t<0, 1>(c, grid, s); break;
+        case 1: launch_colour_t<1, 1>(c, grid, s); break;
+        case 2: launch_colour_t<2, 1>(c, grid, s); break;
+        default: launch_colour_t<3, 4>(c, grid, s); break;
     }
     return 1;
 }
