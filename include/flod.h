@@ -38,8 +38,8 @@ extern "C" {
 #define FLOD_ABI_VERSION 2
 #define FLOD_MAX_LEVELS 16
 #define FLOD_TILE 16                 /* tiles are 16x16 pixels */
-#define FLOD_N_STAGES 7              /* 0 geometry (a1-a3), 1 colour (a4), 2 depth sort (a7, Gaussians), 3 duplication
-                                        (a5-a6), 4 tile sort (a7, pairs), 5 ranges (a8), 6 blend (a9) */
+#define FLOD_N_STAGES 6              /* 0 geometry (a1-a3), 1 tile scan (a5, a8), 2 colour (a4), 3 duplication (a6),
+                                        4 per-tile sort (a7), 5 blend (a9) */
 
 enum {
     FLOD_OK = 0,

@@ -18,8 +18,8 @@ HEADER = os.path.join(HERE, "..", "include", "flod.h")
 
 FLOD_OPT_DEBUG, FLOD_OPT_PROFILE, FLOD_OPT_COUNT = 1, 2, 4
 FLOD_DBG_MASK, FLOD_DBG_TILE_COUNTS, FLOD_DBG_PROJECTED, FLOD_DBG_SORTED_PAIRS, FLOD_DBG_ACTIVATED = range(5)
-FLOD_N_STAGES = 7
-STAGE_NAMES = ("geometry", "colour", "depth_sort", "duplicate", "tile_sort", "ranges", "blend")
+FLOD_N_STAGES = 6
+STAGE_NAMES = ("geometry", "tile_scan", "colour", "duplicate", "tile_sort", "blend")
 ERRORS = {-1: "FLOD_E_INVALID_ARG", -2: "FLOD_E_LEVEL_RANGE", -3: "FLOD_E_NOT_UPLOADED",
           -4: "FLOD_E_ARENA_TOO_SMALL", -5: "FLOD_E_CAPACITY", -6: "FLOD_E_CUDA", -7: "FLOD_E_NO_WORKSPACE"}
 

@@ -29,7 +29,7 @@ __device__ __forceinline__ float ex2(float x)
 
 template <bool COUNT>
 __global__ void __launch_bounds__(kBlendThreads)
-k_blend(const WorkspaceDev ws, int buf, float *__restrict__ out, int W, int H, int TX, int n_tiles,
+k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, int n_tiles,
         float bg0, float bg1, float bg2)
 {
     __shared__ float4 s_a[kBatch];                      // mu'x, mu'y, k, -a2
@@ -38,7 +38,7 @@ k_blend(const WorkspaceDev ws, int buf, float *__restrict__ out, int W, int H, i
     __shared__ unsigned char s_list[kBlendWarps][kBatch];
 
     const int tile = blockIdx.x;
-    if (tile >= n_tiles) return;
+    if (tile >= n_tiles || ws.hdr->overflow) return;   // an overflowed frame is undefined: its lists were not sorted
     const int tx = tile % TX, ty = tile / TX;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // warp = rows 4w..4w+3 of the tile; lanes 0-15 rows (4w, 4w+1), lanes 16-31 rows (4w+2, 4w+3)
@@ -52,7 +52,7 @@ k_blend(const WorkspaceDev ws, int buf, float *__restrict__ out, int W, int H, i
     const float kThr = -7.994353436858858f - 1.0e-3f;  // log2(1/255) minus a safety margin
 
     const uint2 rg = ws.ranges[tile];
-    const uint32_t *__restrict__ vals = (buf ? ws.vals[1] : ws.vals[0]);
+    const uint32_t *__restrict__ vals = ws.vals;
     const float4 *__restrict__ gA = ws.gA;
     const float4 *__restrict__ gB = ws.gB;
     const float *__restrict__ cB = ws.cB;
@@ -166,14 +166,14 @@ k_blend(const WorkspaceDev ws, int buf, float *__restrict__ out, int W, int H, i
     }
 }
 
-int launch_blend(const Context &c, const FrameParams &p, int final_buf, float *out_rgb, cudaStream_t s)
+int launch_blend(const Context &c, const FrameParams &p, float *out_rgb, cudaStream_t s)
 {
     const int n_tiles = p.TX * p.TY;
     if (c.flags & FLOD_OPT_COUNT)
-        k_blend<true><<<n_tiles, kBlendThreads, 0, s>>>(c.ws, final_buf, out_rgb, p.W, p.H, p.TX, n_tiles,
+        k_blend<true><<<n_tiles, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
                                                         p.bg[0], p.bg[1], p.bg[2]);
     else
-        k_blend<false><<<n_tiles, kBlendThreads, 0, s>>>(c.ws, final_buf, out_rgb, p.W, p.H, p.TX, n_tiles,
+        k_blend<false><<<n_tiles, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
                                                          p.bg[0], p.bg[1], p.bg[2]);
     return 1;
 }

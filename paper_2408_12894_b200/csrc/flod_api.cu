@@ -87,46 +87,36 @@ void parallel_for(int64_t n, F f)
     for (auto &t : th) t.join();
 }
 
-struct WsLayout { WorkspaceDev ws; size_t bytes; size_t sort_blocks; };
+struct WsLayout { WorkspaceDev ws; size_t bytes; };
 
-// Carve the workspace.  Order: [header | ranges | scan_status] (zeroed every frame, only the used prefix of
-// scan_status), then sort_status (zeroed once), then the per-Gaussian and per-pair arrays.
+// Carve the workspace.  [header | tile difference grid] come first and are zeroed together every frame.
 WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_pairs)
 {
     WsLayout L{};
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return (unsigned char *)((uintptr_t)base + o); };
-    const size_t tiles = (size_t)((w + kTile - 1) / kTile) * ((h + kTile - 1) / kTile);
+    const size_t tx = (size_t)(w + kTile - 1) / kTile, ty = (size_t)(h + kTile - 1) / kTile;
+    const size_t tiles = tx * ty;
     const size_t nt = (size_t)std::max<int64_t>(n_total, 1);
-    const size_t pre_blocks = (nt + kPreBlock - 1) / kPreBlock;
-    L.sort_blocks = std::max((nt + kDepthSortTile - 1) / kDepthSortTile, ((size_t)max_pairs + kTileSortTile - 1) / kTileSortTile);
-    const size_t tkey_bytes = tile_sort_plan((int)tiles).wide ? 4 : 2;
     L.ws.hdr = (FrameHeader *)take(sizeof(FrameHeader));
+    L.ws.tile_diff = (int *)take((tx + 1) * (ty + 1) * sizeof(int));
     L.ws.ranges = (uint2 *)take(tiles * sizeof(uint2));
-    L.ws.scan_status = (unsigned long long *)take(pre_blocks * 16);
-    L.ws.sort_status = (unsigned long long *)take(L.sort_blocks * kRadix * 8);
+    L.ws.cursor = (unsigned int *)take(tiles * sizeof(unsigned int));
     L.ws.gA = (float4 *)take(nt * sizeof(float4));
     L.ws.gB = (float4 *)take(nt * sizeof(float4));
     L.ws.cB = (float *)take(nt * sizeof(float));
     L.ws.dirgid = (float4 *)take(nt * sizeof(float4));
     L.ws.rect = (ushort4 *)take(nt * sizeof(ushort4));
-    L.ws.cgid = (uint32_t *)take(nt * sizeof(uint32_t));
     L.ws.depth = (uint32_t *)take(nt * sizeof(uint32_t));
-    for (int b = 0; b < 2; ++b) {
-        L.ws.dkeys[b] = (uint32_t *)take(nt * sizeof(uint32_t));
-        L.ws.dvals[b] = (uint32_t *)take(nt * sizeof(uint32_t));
-    }
+    L.ws.vis_list = (uint32_t *)take(nt * sizeof(uint32_t));
     L.ws.dbg = (flod_dbg_projected *)take(nt * sizeof(flod_dbg_projected));
     L.ws.mask = (uint8_t *)take(nt);
-    for (int b = 0; b < 2; ++b) {
-        L.ws.tkeys[b] = (void *)take((size_t)max_pairs * tkey_bytes);
-        L.ws.vals[b] = (uint32_t *)take((size_t)max_pairs * 4);
-    }
+    L.ws.pairs = (unsigned long long *)take((size_t)max_pairs * 8);
+    L.ws.vals = (uint32_t *)take((size_t)max_pairs * 4);
     L.ws.image = (float *)take((size_t)3 * w * h * sizeof(float));
     L.bytes = off;
     return L;
 }
-
 
 }  // namespace
 
@@ -288,12 +278,6 @@ int flod_set_workspace(flod_ctx *ctx, void *workspace_dev, size_t bytes, int wid
     WsLayout L = carve((unsigned char *)workspace_dev, ctx->n_total, width, height, max_pairs);
     ctx->ws = L.ws;
     ctx->ws_w = width; ctx->ws_h = height; ctx->max_pairs = max_pairs;
-    ctx->sort_blocks_max = (int)L.sort_blocks;
-    ctx->pre_blocks_max = (int)(((size_t)std::max<int64_t>(ctx->n_total, 1) + kPreBlock - 1) / kPreBlock);
-    // epoch-tagged look-back words must start from a state no epoch matches
-    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
-    CUDA_TRY(ctx, cudaMemset(ctx->ws.sort_status, 0, (size_t)ctx->sort_blocks_max * kRadix * 8));
-    ctx->epoch = 0;
     ctx->has_ws = true; ctx->rendered = false;
     return FLOD_OK;
 }
@@ -319,10 +303,7 @@ int flod_set_options(flod_ctx *ctx, unsigned flags)
 int flod_launches_per_frame(const flod_ctx *ctx)
 {
     if (!ctx || !ctx->has_ws) return 0;
-    const int tiles = ((ctx->ws_w + kTile - 1) / kTile) * ((ctx->ws_h + kTile - 1) / kTile);
-    const TileSortPlan pl = tile_sort_plan(tiles);
-    // geometry, colour, depth histogram + 4 passes, duplication, tile histogram + passes, ranges, blend
-    return 2 + (1 + kDepthPasses) + 1 + (pl.passes ? 1 + pl.passes : 0) + 1 + 1;
+    return 6;   // geometry, tile scan, colour, duplication, tile sort, blend
 }
 
 int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, float *out_rgb_dev, void *stream)
@@ -378,27 +359,26 @@ int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, flo
     cudaStream_t s = (cudaStream_t)stream;
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     const bool prof = ctx->flags & FLOD_OPT_PROFILE;
-    // zero header + ranges + the used prefix of the look-back words (contiguous)
-    const size_t zero_bytes = (size_t)((unsigned char *)ctx->ws.scan_status - (unsigned char *)ctx->ws.hdr) + (size_t)p.n_pre_blocks * 16;
+    // zero the header and the tile difference grid (contiguous)
+    const size_t zero_bytes = (size_t)((unsigned char *)ctx->ws.tile_diff - (unsigned char *)ctx->ws.hdr) +
+                              (size_t)(p.TX + 1) * (p.TY + 1) * sizeof(int);
     CUDA_TRY(ctx, cudaMemsetAsync(ctx->ws.hdr, 0, zero_bytes, s));
     if (ctx->flags & FLOD_OPT_DEBUG)   // the mask is zero outside the scanned levels
         CUDA_TRY(ctx, cudaMemsetAsync(ctx->ws.mask, 0, (size_t)std::max<int64_t>(ctx->n_total, 1), s));
     int stage = 0;
     auto mark = [&]() { if (prof) cudaEventRecord(ctx->ev[stage], s); ++stage; };
-    int depth_buf = 0, final_buf = 0;
     mark(); launch_geometry(*ctx, p, s);
+    mark(); launch_tile_scan(*ctx, p, s);
     mark(); launch_colour(*ctx, p, s);
-    mark(); if (p.n_pre_blocks > 0) launch_depth_sort(*ctx, &depth_buf, s);
-    mark(); launch_duplicate(*ctx, p, depth_buf, s);
-    mark(); if (p.n_pre_blocks > 0) launch_tile_sort(*ctx, p, &final_buf, s);
-    mark(); if (p.n_pre_blocks > 0) launch_ranges(*ctx, p, final_buf, s);
-    mark(); launch_blend(*ctx, p, final_buf, out_rgb_dev, s);
+    mark(); launch_duplicate(*ctx, p, s);
+    mark(); launch_tile_sort(*ctx, p, s);
+    mark(); launch_blend(*ctx, p, out_rgb_dev, s);
     mark();
     CUDA_TRY(ctx, cudaGetLastError());
     ctx->ev_valid = prof;
     ctx->last_stream = s; ctx->rendered = true;
     ctx->last_n_scan = n_scan;
-    ctx->last_w = p.W; ctx->last_h = p.H; ctx->last_tx = p.TX; ctx->last_ty = p.TY; ctx->last_final_buf = final_buf;
+    ctx->last_w = p.W; ctx->last_h = p.H; ctx->last_tx = p.TX; ctx->last_ty = p.TY; ctx->last_first_gid = p.first_gid;
     return FLOD_OK;
 }
 
@@ -425,7 +405,7 @@ int flod_get_stats(flod_ctx *ctx, flod_stats *out)
     FrameHeader h;
     CUDA_TRY(ctx, cudaMemcpy(&h, ctx->ws.hdr, sizeof(FrameHeader), cudaMemcpyDeviceToHost));
     memset(out, 0, sizeof(*out));
-    out->n_sel = (int64_t)h.n_sel; out->n_front = (int64_t)h.n_front; out->n_vis = (int64_t)h.n_vis;
+    out->n_sel = (int64_t)h.n_sel; out->n_front = (int64_t)h.n_front; out->n_vis = (int64_t)h.n_vis32;
     out->n_pairs = (int64_t)h.n_pairs; out->max_pairs = ctx->max_pairs; out->overflow = (int)h.overflow;
     out->evals = (int64_t)h.evals; out->blends = (int64_t)h.blends;
     out->n_scan = ctx->last_n_scan;
@@ -477,29 +457,34 @@ int flod_debug_copy(flod_ctx *ctx, int what, void *host_dst, size_t bytes)
         }
         case FLOD_DBG_PROJECTED: {
             if (!(ctx->flags & FLOD_OPT_DEBUG)) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: PROJECTED needs FLOD_OPT_DEBUG");
-            const size_t nv = (size_t)h.n_vis;
+            const size_t nv = (size_t)h.n_vis32, ns = (size_t)ctx->last_n_scan;
             if (bytes < nv * sizeof(flod_dbg_projected)) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: buffer too small");
-            CUDA_TRY(ctx, cudaMemcpy(host_dst, ctx->ws.dbg, nv * sizeof(flod_dbg_projected), cudaMemcpyDeviceToHost));
+            std::vector<flod_dbg_projected> all(std::max<size_t>(ns, 1));
+            CUDA_TRY(ctx, cudaMemcpy(all.data(), ctx->ws.dbg, ns * sizeof(flod_dbg_projected), cudaMemcpyDeviceToHost));
+            flod_dbg_projected *dst = (flod_dbg_projected *)host_dst;
+            size_t k = 0;
+            for (size_t i = 0; i < ns && k < nv; ++i)          // records sit at the scan index: compact in ascending gid
+                if (all[i].gid != 0xffffffffu) dst[k++] = all[i];
             return FLOD_OK;
         }
         case FLOD_DBG_SORTED_PAIRS: {
-            const size_t np = (size_t)h.n_pairs_clamped, nv = (size_t)h.n_vis;
+            const size_t np = (size_t)h.n_pairs_clamped, ns = (size_t)ctx->last_n_scan;
             if (bytes < np * sizeof(flod_dbg_pair)) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: buffer too small");
-            const bool wide = tile_sort_plan(ctx->last_tx * ctx->last_ty).wide;
-            std::vector<unsigned char> k(std::max<size_t>(np, 1) * (wide ? 4 : 2));
-            std::vector<uint32_t> v(std::max<size_t>(np, 1)), cg(std::max<size_t>(nv, 1)), dz(std::max<size_t>(nv, 1));
-            CUDA_TRY(ctx, cudaMemcpy(k.data(), ctx->ws.tkeys[ctx->last_final_buf], np * (wide ? 4 : 2), cudaMemcpyDeviceToHost));
-            CUDA_TRY(ctx, cudaMemcpy(v.data(), ctx->ws.vals[ctx->last_final_buf], np * 4, cudaMemcpyDeviceToHost));
-            CUDA_TRY(ctx, cudaMemcpy(cg.data(), ctx->ws.cgid, nv * 4, cudaMemcpyDeviceToHost));
-            CUDA_TRY(ctx, cudaMemcpy(dz.data(), ctx->ws.depth, nv * 4, cudaMemcpyDeviceToHost));
+            const size_t tiles = (size_t)ctx->last_tx * ctx->last_ty;
+            std::vector<uint2> r(std::max<size_t>(tiles, 1));
+            std::vector<uint32_t> v(std::max<size_t>(np, 1)), dz(std::max<size_t>(ns, 1));
+            CUDA_TRY(ctx, cudaMemcpy(r.data(), ctx->ws.ranges, tiles * sizeof(uint2), cudaMemcpyDeviceToHost));
+            CUDA_TRY(ctx, cudaMemcpy(v.data(), ctx->ws.vals, np * 4, cudaMemcpyDeviceToHost));
+            CUDA_TRY(ctx, cudaMemcpy(dz.data(), ctx->ws.depth, ns * 4, cudaMemcpyDeviceToHost));
             flod_dbg_pair *dst = (flod_dbg_pair *)host_dst;
-            for (size_t i = 0; i < np; ++i) {
-                dst[i].tile = wide ? ((const uint32_t *)k.data())[i] : (uint32_t)((const uint16_t *)k.data())[i];
-                const uint32_t ci = v[i];
-                const uint32_t bits = ci < nv ? dz[ci] : 0u;
-                memcpy(&dst[i].depth, &bits, 4);
-                dst[i].gid = ci < nv ? cg[ci] : 0xffffffffu;
-            }
+            for (size_t t = 0; t < tiles; ++t)
+                for (size_t i = r[t].x; i < r[t].y && i < np; ++i) {
+                    dst[i].tile = (uint32_t)t;
+                    const uint32_t si = v[i];
+                    const uint32_t bits = si < ns ? dz[si] : 0u;
+                    memcpy(&dst[i].depth, &bits, 4);
+                    dst[i].gid = si < ns ? (uint32_t)(ctx->last_first_gid + si) : 0xffffffffu;
+                }
             return FLOD_OK;
         }
         default:

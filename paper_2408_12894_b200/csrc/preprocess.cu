@@ -1,9 +1,9 @@
 // Steps a1-a4 of the hot path:
 //   k_geometry  a1 level selection (Eq. 6-7), a2 cull + view transform, a3 EWA projection, conic,
-//               tile rect, and the ordered compaction of the visible Gaussians (+ the frame's pair total);
-//   k_colour    a4 SH -> RGB over the compacted visible Gaussians.
-// k_geometry: one thread per scanned Gaussian; a decoupled look-back over blocks (ordered by an atomic ticket) gives
-// every block its compact-index base, so visible Gaussians get compact indices in ascending gid.
+//               tile rect; every visible Gaussian adds its rect to a 2-D difference grid of the tile counts
+//               (four integer atomics whatever the rect size) and appends its index to the unordered visible list;
+//   k_colour    a4 SH -> RGB over the visible list.
+// One thread per scanned Gaussian, no inter-block dependency: records are written in place at the scan index.
 //
 // The geometry (a1-a3 and the rect) is the canonical fp32 sequence of DESIGN §2: each operation is one IEEE
 // round-to-nearest binary32 operation (the *_rn intrinsics are never contracted into FMAs), in the written order.
@@ -55,57 +55,18 @@ __device__ __forceinline__ void sh_basis(float x, float y, float z, float *Y)
     }
 }
 
-constexpr unsigned long long kFlagAgg = 1ull << 62, kFlagIncl = 2ull << 62, kFlagMask = 3ull << 62;
-constexpr int kVisShift = 36;
-constexpr unsigned long long kPairMask = (1ull << kVisShift) - 1, kVisMask = (1ull << 26) - 1;
-
-// Warp 0 of a block: publish this block's aggregate and sum the aggregates of all blocks before it (decoupled
-// look-back, 32 predecessors per step).  Returns the exclusive prefix in every lane of the warp.
-__device__ __forceinline__ unsigned long long lookback(unsigned long long *status, int stride, unsigned int vb,
-                                                       unsigned long long agg, int lane)
-{
-    unsigned long long excl = 0;
-    if (vb == 0) {
-        if (lane == 0) atomicExch(status, kFlagIncl | agg);
-        return 0;
-    }
-    if (lane == 0) atomicExch(status + (size_t)vb * stride, kFlagAgg | agg);
-    long long j = (long long)vb - 1;
-    while (true) {
-        const long long idx = j - lane;
-        unsigned long long st = kFlagIncl;                 // lanes before block 0 read "inclusive 0"
-        if (idx >= 0) {
-            volatile unsigned long long *ptr = status + (size_t)idx * stride;
-            do { st = *ptr; } while ((st & kFlagMask) == 0);
-        }
-        const unsigned int incl_mask = __ballot_sync(0xffffffffu, (st & kFlagMask) == kFlagIncl);
-        const unsigned long long val = st & ~kFlagMask;
-        const int first = incl_mask ? (__ffs(incl_mask) - 1) : 31;
-        unsigned long long contrib = (lane <= first) ? val : 0ull;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) contrib += __shfl_xor_sync(0xffffffffu, contrib, o);
-        excl += contrib;
-        if (incl_mask) break;
-        j -= 32;
-    }
-    if (lane == 0) atomicExch(status + (size_t)vb * stride, kFlagIncl | (excl + agg));
-    return excl;
-}
-
 template <bool DEBUG>
 __global__ void __launch_bounds__(kPreBlock)
 k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ FrameParams p)
 {
-    __shared__ unsigned int s_vb;
-    __shared__ unsigned long long s_warp_tot[kPreBlock / 32];
-    __shared__ unsigned long long s_base;           // packed exclusive prefix of this block (status format)
+    __shared__ unsigned int s_warp_vis[kPreBlock / 32];
+    __shared__ unsigned int s_base;
     __shared__ unsigned int s_cnt[2];               // n_sel, n_front of the block
+    __shared__ unsigned long long s_pairs;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) { s_vb = atomicAdd(&ws.hdr->pre_ticket, 1u); s_cnt[0] = 0; s_cnt[1] = 0; }
-    __syncthreads();
-    const unsigned int vb = s_vb;
-    const int i = (int)(vb * kPreBlock) + tid;
+    if (tid == 0) { s_cnt[0] = 0; s_cnt[1] = 0; s_pairs = 0; }
+    const int i = (int)(blockIdx.x * kPreBlock) + tid;
 
     bool vis = false, sel = false, front = false;
     unsigned int n_tiles = 0;
@@ -182,77 +143,60 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
         }
     }
 
-    // ---- block scan of (visible, n_tiles), packed vis << 40 | tiles
-    unsigned long long v = ((unsigned long long)(vis ? 1 : 0) << 40) | n_tiles;
-    unsigned long long incl = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        unsigned long long n = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += n;
+    // ---- per-visible records, in place at the scan index i
+    if (vis) {
+        // DESIGN R25: factorised exponent from the ROUNDED conic, derived in fp64, rounded once
+        const double LOG2E = 1.4426950408889634;
+        const double dA = (double)cA, dB = (double)cB, dC = (double)cC;
+        const float kk = (float)(dB / dA);
+        const float a2 = (float)(-0.5 * LOG2E * dA);                   // stored negated: e = log2 o + a2 w^2 + d2 dy^2
+        const float d2 = (float)(-0.5 * LOG2E * (dC - dB * dB / dA));
+        ws.gA[i] = make_float4(mx2, my2, kk, a2);
+        reinterpret_cast<float2 *>(ws.gB)[2 * (size_t)i] = make_float2(d2, __ldg(sc.l2o + g));   // (r, g) by k_colour
+        ws.rect[i] = make_ushort4((unsigned short)tx0, (unsigned short)ty0, (unsigned short)tx1, (unsigned short)ty1);
+        ws.depth[i] = __float_as_uint(pz);
+        ws.dirgid[i] = make_float4(wx - p.centre[0], wy - p.centre[1], wz - p.centre[2], __uint_as_float((unsigned int)g));
+        // a5, first half: +1 over the rect in the 2-D difference grid of the per-tile pair counts
+        const int gw = p.TX + 1;
+        atomicAdd(ws.tile_diff + ty0 * gw + tx0, 1);
+        atomicAdd(ws.tile_diff + ty0 * gw + tx1, -1);
+        atomicAdd(ws.tile_diff + ty1 * gw + tx0, -1);
+        atomicAdd(ws.tile_diff + ty1 * gw + tx1, 1);
     }
-    if (lane == 31) s_warp_tot[warp] = incl;
-    {
-        unsigned int bs = __ballot_sync(0xffffffffu, sel), bf = __ballot_sync(0xffffffffu, front);
-        if (lane == 0) { atomicAdd(&s_cnt[0], __popc(bs)); atomicAdd(&s_cnt[1], __popc(bf)); }
-    }
-    __syncthreads();
-    unsigned long long warp_off = 0, block_tot = 0;
-#pragma unroll
-    for (int w = 0; w < kPreBlock / 32; ++w) {
-        unsigned long long t = s_warp_tot[w];
-        if (w < warp) warp_off += t;
-        block_tot += t;
-    }
-    incl += warp_off;
-    const unsigned int block_vis = (unsigned int)(block_tot >> 40);
-    const unsigned long long block_pairs = block_tot & ((1ull << 40) - 1);
-    const unsigned int rank = (unsigned int)(incl >> 40) - (vis ? 1u : 0u);          // local visible rank
-
-    // ---- decoupled look-back over the blocks before this one (warp 0)
-    if (warp == 0) {
-        const unsigned long long agg = ((unsigned long long)block_vis << kVisShift) | block_pairs;
-        const unsigned long long excl = lookback(ws.scan_status, 2, vb, agg, lane);
-        if (lane == 0) {
-            s_base = excl;
-            if (s_cnt[0]) atomicAdd(&ws.hdr->n_sel, (unsigned long long)s_cnt[0]);
-            if (s_cnt[1]) atomicAdd(&ws.hdr->n_front, (unsigned long long)s_cnt[1]);
-            if (vb == (unsigned int)p.n_pre_blocks - 1) {          // the last block knows the frame totals
-                const unsigned long long tot = excl + agg;
-                const unsigned long long np = tot & kPairMask;
-                const unsigned long long nv = (tot >> kVisShift) & kVisMask;
-                ws.hdr->n_vis = nv;
-                ws.hdr->n_vis32 = (unsigned int)nv;
-                ws.hdr->n_pairs = np;
-                ws.hdr->n_pairs_clamped = (unsigned int)(np < p.max_pairs ? np : p.max_pairs);
-                ws.hdr->overflow = np > p.max_pairs ? 1u : 0u;
-            }
-        }
-    }
-    __syncthreads();
-    if (!vis) return;
-    const unsigned int ci = (unsigned int)((s_base >> kVisShift) & kVisMask) + rank;
-
-    // ---- per-visible records, compact index ci (ascending gid)
-    // DESIGN R25: factorised exponent from the ROUNDED conic, derived in fp64, rounded once
-    const double LOG2E = 1.4426950408889634;
-    const double dA = (double)cA, dB = (double)cB, dC = (double)cC;
-    const float kk = (float)(dB / dA);
-    const float a2 = (float)(-0.5 * LOG2E * dA);                       // stored negated: e = log2 o + a2 w^2 + d2 dy^2
-    const float d2 = (float)(-0.5 * LOG2E * (dC - dB * dB / dA));
-    ws.gA[ci] = make_float4(mx2, my2, kk, a2);
-    reinterpret_cast<float2 *>(ws.gB)[2 * (size_t)ci] = make_float2(d2, __ldg(sc.l2o + g));   // (r, g) by k_colour
-    ws.rect[ci] = make_ushort4((unsigned short)tx0, (unsigned short)ty0, (unsigned short)tx1, (unsigned short)ty1);
-    ws.depth[ci] = __float_as_uint(pz);
-    ws.dirgid[ci] = make_float4(wx - p.centre[0], wy - p.centre[1], wz - p.centre[2], __uint_as_float((unsigned int)g));
-    ws.cgid[ci] = (uint32_t)g;
-    if (DEBUG) {
+    if (DEBUG && i < p.n_scan) {
         flod_dbg_projected d;
-        d.gid = (uint32_t)g; d.mu2d[0] = mx2; d.mu2d[1] = my2; d.depth = pz;
-        d.conic[0] = cA; d.conic[1] = cB; d.conic[2] = cC; d.opacity = __ldg(sc.opacity + g);
+        d.gid = vis ? (uint32_t)g : 0xffffffffu; d.mu2d[0] = mx2; d.mu2d[1] = my2; d.depth = pz;
+        d.conic[0] = cA; d.conic[1] = cB; d.conic[2] = cC; d.opacity = vis ? __ldg(sc.opacity + g) : 0.0f;
         d.rgb[0] = 0.0f; d.rgb[1] = 0.0f; d.rgb[2] = 0.0f;                                    // by k_colour
         d.rect[0] = tx0; d.rect[1] = ty0; d.rect[2] = tx1; d.rect[3] = ty1;
-        ws.dbg[ci] = d;
+        ws.dbg[i] = d;
     }
+
+    // ---- block-aggregated counters and the unordered visible list
+    const unsigned int bv = __ballot_sync(0xffffffffu, vis);
+    const unsigned int bs = __ballot_sync(0xffffffffu, sel), bf = __ballot_sync(0xffffffffu, front);
+    unsigned int wp = n_tiles;                       // warp sum of the tile counts (a rect has < 2^20 tiles)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) wp += __shfl_xor_sync(0xffffffffu, wp, o);
+    __syncthreads();                                 // s_cnt / s_pairs were zeroed by thread 0
+    if (lane == 0) {
+        s_warp_vis[warp] = __popc(bv);
+        if (bs) atomicAdd(&s_cnt[0], __popc(bs));
+        if (bf) atomicAdd(&s_cnt[1], __popc(bf));
+        if (wp) atomicAdd(&s_pairs, (unsigned long long)wp);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        unsigned int tot = 0;
+#pragma unroll
+        for (int w = 0; w < kPreBlock / 32; ++w) { const unsigned int t = s_warp_vis[w]; s_warp_vis[w] = tot; tot += t; }
+        s_base = tot ? atomicAdd(&ws.hdr->n_vis32, tot) : 0u;
+        if (s_cnt[0]) atomicAdd(&ws.hdr->n_sel, (unsigned long long)s_cnt[0]);
+        if (s_cnt[1]) atomicAdd(&ws.hdr->n_front, (unsigned long long)s_cnt[1]);
+        if (s_pairs) atomicAdd(&ws.hdr->n_pairs, s_pairs);
+    }
+    __syncthreads();
+    if (vis) ws.vis_list[s_base + s_warp_vis[warp] + __popc(bv & ((1u << lane) - 1))] = (uint32_t)i;
 }
 
 // ---- a4: colour of every visible Gaussian.  rgb = max(0, 0.5 + sum_k Y_k(dir) sh_k)  (R16)
@@ -268,10 +212,12 @@ k_colour(const SceneDev sc, const WorkspaceDev ws)
     const unsigned int sub = threadIdx.x % LANES;
     const unsigned int per_block = 256 / LANES;
     for (unsigned int base = blockIdx.x * per_block; base < n_vis; base += gridDim.x * per_block) {
-        const unsigned int ci = base + threadIdx.x / LANES;
-        const bool ok = ci < n_vis;
+        const unsigned int slot = base + threadIdx.x / LANES;
+        const bool ok = slot < n_vis;
         float r = 0.0f, g = 0.0f, b = 0.0f;
+        unsigned int ci = 0;
         if (ok) {
+            ci = ws.vis_list[slot];
             const float4 dg = ws.dirgid[ci];
             const float *row = sc.sh + (size_t)__float_as_uint(dg.w) * sc.sh_stride;
             float Y[K];
