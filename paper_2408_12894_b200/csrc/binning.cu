@@ -14,7 +14,7 @@
 namespace flod {
 
 // ------------------------------------------------------------------------------------------------ a5 / a8
-// One block.  grid = (TX+1) x (TY+1) ints, in shared memory when it fits, else in place in global memory.
+// One block.  grid = (TX+1) x (TY+1) ints, in shared memory when it fits, else in global memory (ws.tile_cnt).
 __global__ void __launch_bounds__(1024)
 k_tile_scan(const WorkspaceDev ws, int TX, int TY, unsigned int max_pairs, int use_smem)
 {
@@ -22,11 +22,9 @@ k_tile_scan(const WorkspaceDev ws, int TX, int TY, unsigned int max_pairs, int u
     __shared__ unsigned long long s_part[1024];
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int gw = TX + 1, gh = TY + 1, gn = gw * gh;
-    int *grid = use_smem ? s_grid : ws.tile_diff;
-    if (use_smem) {
-        for (int i = tid; i < gn; i += nthr) grid[i] = ws.tile_diff[i];
-        __syncthreads();
-    }
+    int *grid = use_smem ? s_grid : ws.tile_cnt;
+    for (int i = tid; i < gn; i += nthr) grid[i] = ws.tile_diff[(size_t)i * kCtrStride];
+    __syncthreads();
     for (int y = tid; y < gh; y += nthr) {           // prefix along x
         int run = 0;
         int *row = grid + y * gw;
@@ -58,7 +56,7 @@ k_tile_scan(const WorkspaceDev ws, int TX, int TY, unsigned int max_pairs, int u
         const unsigned int a = (unsigned int)min(run, (unsigned long long)max_pairs);
         const unsigned int b = (unsigned int)min(run + c, (unsigned long long)max_pairs);
         ws.ranges[t] = make_uint2(a, b);
-        ws.cursor[t] = a;
+        ws.cursor[(size_t)t * kCtrStride] = a;
         run += c;
     }
     if (tid == nthr - 1) {
@@ -139,7 +137,7 @@ k_duplicate(const WorkspaceDev ws, int TX, unsigned int max_pairs)
             const unsigned int ry = k / w, rx = k - ry * w;
             const unsigned int rc = s_rect[r];
             const unsigned int tile = ((rc >> 16) + ry) * (unsigned int)TX + ((rc & 0xffffu) + rx);
-            const unsigned int pos = atomicAdd(ws.cursor + tile, 1u);
+            const unsigned int pos = atomicAdd(ws.cursor + (size_t)tile * kCtrStride, 1u);
             if (pos < max_pairs) ws.pairs[pos] = ((unsigned long long)s_depth[r] << 32) | s_idx[r];
         }
         __syncthreads();
@@ -156,8 +154,25 @@ int launch_duplicate(const Context &c, const FrameParams &p, cudaStream_t s)
 
 // ------------------------------------------------------------------------------------------------ a7
 constexpr int kSortThreads = 256;
+constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kSortMaxBins = 512;
+constexpr int kSortRounds = kSortCap / kSortThreads;      // ranking rounds of a warp: its keys / 32
+static_assert(kSortCap % (kSortThreads * 1) == 0, "kSortCap must be a multiple of the block size");
 
-// Ascending bitonic sort of s[0, n_pad), n_pad a power of two >= 2, by the whole block.
+struct SortSmem {
+    unsigned long long keys[2][kSortCap];                 // ping-pong
+    unsigned int whist[kSortWarps][kSortMaxBins];         // per-warp digit counters -> exclusive offsets across warps
+    unsigned int binstart[kSortMaxBins];
+    unsigned int hist[256];                               // long lists: selection histogram
+    unsigned int wsum[kSortWarps];
+    unsigned int red[2][kSortWarps];
+    unsigned int count;
+    unsigned int flag;
+    unsigned long long bcast[2];
+    unsigned long long red64[kSortWarps];
+};
+
+// Ascending bitonic sort of s[0, n_pad), n_pad a power of two >= 2, by the whole block (fallback path).
 __device__ __forceinline__ void bitonic_sort(unsigned long long *s, unsigned int n_pad, int tid)
 {
     for (unsigned int k = 2; k <= n_pad; k <<= 1) {
@@ -179,14 +194,137 @@ __device__ __forceinline__ unsigned int next_pow2(unsigned int v)
     return v <= 2 ? 2u : 1u << (32 - __clz(v - 1));
 }
 
+// Block-wide min / max of the depth words; every thread gets the result.  Ends with a barrier.
+__device__ __forceinline__ void block_minmax(SortSmem &S, unsigned int &dmin, unsigned int &dmax, int lane, int warp)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        dmin = min(dmin, __shfl_xor_sync(0xffffffffu, dmin, o));
+        dmax = max(dmax, __shfl_xor_sync(0xffffffffu, dmax, o));
+    }
+    if (lane == 0) { S.red[0][warp] = dmin; S.red[1][warp] = dmax; }
+    __syncthreads();
+#pragma unroll
+    for (int w = 0; w < kSortWarps; ++w) { dmin = min(dmin, S.red[0][w]); dmax = max(dmax, S.red[1][w]); }
+    __syncthreads();
+}
+
+// Sorts the n <= kSortCap unique 64-bit keys (depth bits << 32 | index) held in S.keys[0][0, n) and returns the
+// sorted array.  Stable LSD radix passes over the bits in which the depth words differ (8 or 9 bits per pass; a warp
+// ranks a contiguous chunk with match_any, per-warp digit counters make it stable), then runs of equal depth, which
+// the passes leave in arrival order, are put in index order (insertion by the run's first thread; runs are short --
+// a list with a run longer than 32 falls back to a bitonic network on the whole 64-bit keys).
+__device__ unsigned long long *block_sort(SortSmem &S, unsigned int n, unsigned int dmin, unsigned int dmax, int tid)
+{
+    const int lane = tid & 31, warp = tid >> 5;
+    const int bits = 32 - __clz(dmax - dmin);                         // 0 when all depths are equal
+    const int dbits = (bits > 24 && bits <= 27) ? 9 : 8;
+    const int passes = (bits + dbits - 1) / dbits;
+    const unsigned int bins = 1u << dbits, dmask = bins - 1;
+    const int bpt = (int)(bins / kSortThreads);                       // bins per thread in the scan: 1 or 2
+    const unsigned int per_warp = (n + kSortThreads - 1) / kSortThreads * 32;   // keys per warp, a multiple of 32
+    int cur = 0;
+    for (int pass = 0; pass < passes; ++pass) {
+        const unsigned long long *src = S.keys[cur];
+        unsigned long long *dst = S.keys[cur ^ 1];
+        const int shift = pass * dbits;
+        for (unsigned int i = tid; i < kSortWarps * bins; i += kSortThreads) S.whist[i / bins][i % bins] = 0;
+        __syncthreads();
+        // ---- rank inside the warp's chunk, stable
+        unsigned long long key[kSortRounds];
+        unsigned short rnk[kSortRounds];
+        unsigned int *wh = S.whist[warp];
+#pragma unroll
+        for (int r = 0; r < kSortRounds; ++r) {
+            if ((unsigned int)r * 32 < per_warp) {
+                const unsigned int j = warp * per_warp + r * 32 + lane;
+                const bool ok = j < n;
+                const unsigned int vm = __ballot_sync(0xffffffffu, ok);
+                if (ok) {
+                    key[r] = src[j];
+                    const unsigned int d = (((unsigned int)(key[r] >> 32) - dmin) >> shift) & dmask;
+                    const unsigned int peers = __match_any_sync(vm, d);
+                    const unsigned int leader = __ffs(peers) - 1;
+                    unsigned int old = 0;
+                    if (lane == leader) { old = wh[d]; wh[d] = old + __popc(peers); }
+                    old = __shfl_sync(peers, old, leader);
+                    rnk[r] = (unsigned short)(old + __popc(peers & ((1u << lane) - 1)));
+                }
+                __syncwarp();
+            }
+        }
+        __syncthreads();
+        // ---- per bin: exclusive scan across warps; then exclusive scan across bins
+        {
+            unsigned int tot[2] = {0, 0};
+            for (int q = 0; q < bpt; ++q) {
+                const unsigned int b = tid * bpt + q;
+                unsigned int run = 0;
+#pragma unroll
+                for (int w = 0; w < kSortWarps; ++w) { const unsigned int t = S.whist[w][b]; S.whist[w][b] = run; run += t; }
+                tot[q] = run;
+            }
+            const unsigned int mine = tot[0] + tot[1];
+            unsigned int incl = mine;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const unsigned int t = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += t;
+            }
+            if (lane == 31) S.wsum[warp] = incl;
+            __syncthreads();
+            unsigned int excl = incl - mine;
+#pragma unroll
+            for (int w = 0; w < kSortWarps; ++w) if (w < warp) excl += S.wsum[w];
+            S.binstart[tid * bpt] = excl;
+            if (bpt == 2) S.binstart[tid * bpt + 1] = excl + tot[0];
+        }
+        __syncthreads();
+        // ---- scatter
+#pragma unroll
+        for (int r = 0; r < kSortRounds; ++r) {
+            if ((unsigned int)r * 32 < per_warp) {
+                const unsigned int j = warp * per_warp + r * 32 + lane;
+                if (j < n) {
+                    const unsigned int d = (((unsigned int)(key[r] >> 32) - dmin) >> shift) & dmask;
+                    dst[S.binstart[d] + wh[d] + rnk[r]] = key[r];
+                }
+            }
+        }
+        __syncthreads();
+        cur ^= 1;
+    }
+    // ---- equal-depth runs -> index order
+    unsigned long long *arr = S.keys[cur];
+    bool big = false;
+    for (unsigned int j = tid; j + 1 < n; j += kSortThreads) {
+        const unsigned int dj = (unsigned int)(arr[j] >> 32);
+        if (dj == (unsigned int)(arr[j + 1] >> 32) && (j == 0 || (unsigned int)(arr[j - 1] >> 32) != dj)) {
+            unsigned int e = j + 2;
+            while (e < n && (unsigned int)(arr[e] >> 32) == dj && e - j <= 32) ++e;
+            if (e - j > 32) { big = true; continue; }
+            for (unsigned int a = j + 1; a < e; ++a) {          // insertion sort of arr[j, e)
+                const unsigned long long k = arr[a];
+                unsigned int b = a;
+                while (b > j && arr[b - 1] > k) { arr[b] = arr[b - 1]; --b; }
+                arr[b] = k;
+            }
+        }
+    }
+    if (__syncthreads_or(big)) {
+        const unsigned int n_pad = next_pow2(n);
+        for (unsigned int j = n + tid; j < n_pad; j += kSortThreads) arr[j] = ~0ull;
+        __syncthreads();
+        bitonic_sort(arr, n_pad, tid);
+    }
+    return arr;
+}
+
 __global__ void __launch_bounds__(kSortThreads)
 k_tile_sort(const WorkspaceDev ws, int n_tiles)
 {
-    __shared__ unsigned long long s_keys[kSortCap];
-    __shared__ unsigned int s_hist[256];
-    __shared__ unsigned long long s_red[kSortThreads / 32];
-    __shared__ unsigned int s_count;
-    __shared__ unsigned long long s_bcast[2];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    SortSmem &S = *reinterpret_cast<SortSmem *>(smem_raw);
 
     const int tile = blockIdx.x;
     if (tile >= n_tiles) return;
@@ -198,11 +336,15 @@ k_tile_sort(const WorkspaceDev ws, int n_tiles)
     uint32_t *__restrict__ vals = ws.vals + rg.x;
 
     if (L <= kSortCap) {
-        const unsigned int n_pad = next_pow2(L);
-        for (unsigned int j = tid; j < n_pad; j += kSortThreads) s_keys[j] = j < L ? pairs[j] : ~0ull;
-        __syncthreads();
-        bitonic_sort(s_keys, n_pad, tid);
-        for (unsigned int j = tid; j < L; j += kSortThreads) vals[j] = (uint32_t)s_keys[j];
+        unsigned int dmin = 0xffffffffu, dmax = 0;
+        for (unsigned int j = tid; j < L; j += kSortThreads) {
+            const unsigned long long k = pairs[j];
+            S.keys[0][j] = k;
+            dmin = min(dmin, (unsigned int)(k >> 32)); dmax = max(dmax, (unsigned int)(k >> 32));
+        }
+        block_minmax(S, dmin, dmax, lane, warp);
+        const unsigned long long *arr = block_sort(S, L, dmin, dmax, tid);
+        for (unsigned int j = tid; j < L; j += kSortThreads) vals[j] = (uint32_t)arr[j];
         return;
     }
 
@@ -211,11 +353,11 @@ k_tile_sort(const WorkspaceDev ws, int n_tiles)
     for (unsigned int j = tid; j < L; j += kSortThreads) kmax = max(kmax, pairs[j]);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) kmax = max(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
-    if (lane == 0) s_red[warp] = kmax;
+    if (lane == 0) S.red64[warp] = kmax;
     __syncthreads();
     kmax = 0;
 #pragma unroll
-    for (int w = 0; w < kSortThreads / 32; ++w) kmax = max(kmax, s_red[w]);
+    for (int w = 0; w < kSortWarps; ++w) kmax = max(kmax, S.red64[w]);
 
     unsigned long long lo = 0;                         // every key < lo has been written out
     unsigned int out = 0;
@@ -230,20 +372,20 @@ k_tile_sort(const WorkspaceDev ws, int n_tiles)
                 const unsigned long long width = b - a;                  // b - a + 1 keys; both < 2^63
                 const int sh = max(0, 64 - __clzll(width) - 8);          // (b - a) >> sh < 256
                 __syncthreads();
-                s_hist[tid] = 0;
+                S.hist[tid] = 0;
                 __syncthreads();
                 for (unsigned int j = tid; j < L; j += kSortThreads) {
                     const unsigned long long k = pairs[j];
-                    if (k >= a && k <= b) atomicAdd(&s_hist[(unsigned int)((k - a) >> sh)], 1u);
+                    if (k >= a && k <= b) atomicAdd(&S.hist[(unsigned int)((k - a) >> sh)], 1u);
                 }
                 __syncthreads();
                 if (tid == 0) {
                     unsigned int cum = 0, m = 0;
-                    while (m < 256 && cum + s_hist[m] <= budget) { cum += s_hist[m]; ++m; }
-                    s_bcast[0] = m; s_bcast[1] = cum;
+                    while (m < 256 && cum + S.hist[m] <= budget) { cum += S.hist[m]; ++m; }
+                    S.bcast[0] = m; S.bcast[1] = cum;
                 }
                 __syncthreads();
-                const unsigned int m = (unsigned int)s_bcast[0], cum = (unsigned int)s_bcast[1];
+                const unsigned int m = (unsigned int)S.bcast[0], cum = (unsigned int)S.bcast[1];
                 if (m == 256) { hi = b; break; }
                 budget -= cum;
                 const unsigned long long edge = a + ((unsigned long long)m << sh);   // first key of the bin that overflows
@@ -254,26 +396,27 @@ k_tile_sort(const WorkspaceDev ws, int n_tiles)
         }
         // (hi >= lo always: with sh == 0 a bin holds at most one key, so the first bin of [a, b] fits the budget
         //  unless the budget is 0, which only happens after a round of refinement accepted keys below `edge`.)
-        if (tid == 0) s_count = 0;
+        if (tid == 0) S.count = 0;
         __syncthreads();
+        unsigned int dmin = 0xffffffffu, dmax = 0;
         for (unsigned int j0 = 0; j0 < L; j0 += kSortThreads) {
             const unsigned int j = j0 + tid;
             const unsigned long long k = j < L ? pairs[j] : 0ull;
             const bool take = j < L && k >= lo && k <= hi;
             const unsigned int bal = __ballot_sync(0xffffffffu, take);
             unsigned int wbase = 0;
-            if (lane == 0 && bal) wbase = atomicAdd(&s_count, __popc(bal));
+            if (lane == 0 && bal) wbase = atomicAdd(&S.count, __popc(bal));
             wbase = __shfl_sync(0xffffffffu, wbase, 0);
-            if (take) s_keys[wbase + __popc(bal & ((1u << lane) - 1))] = k;
+            if (take) {
+                S.keys[0][wbase + __popc(bal & ((1u << lane) - 1))] = k;
+                dmin = min(dmin, (unsigned int)(k >> 32)); dmax = max(dmax, (unsigned int)(k >> 32));
+            }
         }
-        __syncthreads();
-        const unsigned int n = s_count;
+        block_minmax(S, dmin, dmax, lane, warp);
+        const unsigned int n = S.count;
         if (n == 0) break;                             // cannot happen with unique keys; never spin
-        const unsigned int n_pad = next_pow2(n);
-        for (unsigned int j = n + tid; j < n_pad; j += kSortThreads) s_keys[j] = ~0ull;
-        __syncthreads();
-        bitonic_sort(s_keys, n_pad, tid);
-        for (unsigned int j = tid; j < n; j += kSortThreads) vals[out + j] = (uint32_t)s_keys[j];
+        const unsigned long long *arr = block_sort(S, n, dmin, dmax, tid);
+        for (unsigned int j = tid; j < n; j += kSortThreads) vals[out + j] = (uint32_t)arr[j];
         out += n;
         lo = hi + 1;
         __syncthreads();
@@ -283,7 +426,12 @@ k_tile_sort(const WorkspaceDev ws, int n_tiles)
 int launch_tile_sort(const Context &c, const FrameParams &p, cudaStream_t s)
 {
     if (p.n_pre_blocks <= 0) return 0;
-    k_tile_sort<<<p.n_tiles, kSortThreads, 0, s>>>(c.ws, p.n_tiles);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_tile_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
+        attr_set = true;
+    }
+    k_tile_sort<<<p.n_tiles, kSortThreads, sizeof(SortSmem), s>>>(c.ws, p.n_tiles);
     return 1;
 }
 

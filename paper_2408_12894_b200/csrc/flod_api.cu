@@ -99,9 +99,10 @@ WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_p
     const size_t tiles = tx * ty;
     const size_t nt = (size_t)std::max<int64_t>(n_total, 1);
     L.ws.hdr = (FrameHeader *)take(sizeof(FrameHeader));
-    L.ws.tile_diff = (int *)take((tx + 1) * (ty + 1) * sizeof(int));
+    L.ws.tile_diff = (int *)take((tx + 1) * (ty + 1) * kCtrStride * sizeof(int));
+    L.ws.tile_cnt = (int *)take((tx + 1) * (ty + 1) * sizeof(int));
     L.ws.ranges = (uint2 *)take(tiles * sizeof(uint2));
-    L.ws.cursor = (unsigned int *)take(tiles * sizeof(unsigned int));
+    L.ws.cursor = (unsigned int *)take(tiles * kCtrStride * sizeof(unsigned int));
     L.ws.gA = (float4 *)take(nt * sizeof(float4));
     L.ws.gB = (float4 *)take(nt * sizeof(float4));
     L.ws.cB = (float *)take(nt * sizeof(float));
@@ -361,7 +362,7 @@ int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, flo
     const bool prof = ctx->flags & FLOD_OPT_PROFILE;
     // zero the header and the tile difference grid (contiguous)
     const size_t zero_bytes = (size_t)((unsigned char *)ctx->ws.tile_diff - (unsigned char *)ctx->ws.hdr) +
-                              (size_t)(p.TX + 1) * (p.TY + 1) * sizeof(int);
+                              (size_t)(p.TX + 1) * (p.TY + 1) * kCtrStride * sizeof(int);
     CUDA_TRY(ctx, cudaMemsetAsync(ctx->ws.hdr, 0, zero_bytes, s));
     if (ctx->flags & FLOD_OPT_DEBUG)   // the mask is zero outside the scanned levels
         CUDA_TRY(ctx, cudaMemsetAsync(ctx->ws.mask, 0, (size_t)std::max<int64_t>(ctx->n_total, 1), s));

@@ -14,6 +14,8 @@ namespace flod {
 constexpr int kTile = FLOD_TILE;
 constexpr int kPreBlock = 256;            // geometry / duplication: Gaussians per block
 constexpr int kSortCap = 2048;            // per-tile sort: keys sorted in shared memory per round
+constexpr int kCtrStride = 64;            // ints between two per-tile atomic counters: one counter per 256 B, so that the
+                                          // L2 slices share the atomic traffic (a dense 16 KB grid sits on a few slices)
 
 // Scene planes in the caller's arena (SoA, one plane per attribute, gid order = levels concatenated).
 struct SceneDev {
@@ -42,9 +44,10 @@ struct FrameHeader {
 //   gA = (mu'x, mu'y, k = B/A, -A log2(e)/2)     gB = (-(C - B^2/A) log2(e)/2, log2 o, r, g)    cB = b
 struct WorkspaceDev {
     FrameHeader *hdr;
-    int *tile_diff;                       // [(TX+1)*(TY+1)] 2-D difference grid of the tile counts (zeroed per frame)
+    int *tile_diff;                       // [(TX+1)*(TY+1)][kCtrStride] 2-D difference grid of the tile counts (zeroed per frame)
+    int *tile_cnt;                        // [(TX+1)*(TY+1)] dense copy, used by the tile scan when the grid exceeds shared memory
     uint2 *ranges;                        // [T_n] (start, end) of every tile's pair list
-    unsigned int *cursor;                 // [T_n] next free slot of every tile's list during duplication
+    unsigned int *cursor;                 // [T_n][kCtrStride] next free slot of every tile's list during duplication
     float4 *gA, *gB;                      // [n_total]
     float *cB;                            // [n_total]
     float4 *dirgid;                       // [n_total] (mu - c_cam, gid bits): input of the colour kernel

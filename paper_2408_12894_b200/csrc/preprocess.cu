@@ -158,10 +158,10 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
         ws.dirgid[i] = make_float4(wx - p.centre[0], wy - p.centre[1], wz - p.centre[2], __uint_as_float((unsigned int)g));
         // a5, first half: +1 over the rect in the 2-D difference grid of the per-tile pair counts
         const int gw = p.TX + 1;
-        atomicAdd(ws.tile_diff + ty0 * gw + tx0, 1);
-        atomicAdd(ws.tile_diff + ty0 * gw + tx1, -1);
-        atomicAdd(ws.tile_diff + ty1 * gw + tx0, -1);
-        atomicAdd(ws.tile_diff + ty1 * gw + tx1, 1);
+        atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx0) * kCtrStride, 1);
+        atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx1) * kCtrStride, -1);
+        atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx0) * kCtrStride, -1);
+        atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx1) * kCtrStride, 1);
     }
     if (DEBUG && i < p.n_scan) {
         flod_dbg_projected d;
