@@ -113,6 +113,7 @@ WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_p
     L.ws.dbg = (flod_dbg_projected *)take(nt * sizeof(flod_dbg_projected));
     L.ws.mask = (uint8_t *)take(nt);
     L.ws.pairs = (unsigned long long *)take((size_t)max_pairs * 8);
+    L.ws.pairs_tmp = (unsigned long long *)take((size_t)max_pairs * 8);
     L.ws.vals = (uint32_t *)take((size_t)max_pairs * 4);
     L.ws.image = (float *)take((size_t)3 * w * h * sizeof(float));
     L.bytes = off;

@@ -13,7 +13,7 @@ namespace flod {
 
 constexpr int kTile = FLOD_TILE;
 constexpr int kPreBlock = 256;            // geometry / duplication: Gaussians per block
-constexpr int kSortCap = 2048;            // per-tile sort: keys sorted in shared memory per round
+constexpr int kSortCap = 4096;            // per-tile sort: lists up to this many keys are scattered into shared memory
 constexpr int kCtrStride = 64;            // ints between two per-tile atomic counters: one counter per 256 B, so that the
                                           // L2 slices share the atomic traffic (a dense 16 KB grid sits on a few slices)
 
@@ -57,6 +57,7 @@ struct WorkspaceDev {
     flod_dbg_projected *dbg;              // [n_total] (written only with FLOD_OPT_DEBUG; gid = ~0 when not visible)
     uint8_t *mask;                        // [n_total] (written only with FLOD_OPT_DEBUG)
     unsigned long long *pairs;            // [max_pairs] (depth bits << 32) | scan index, grouped by tile, unsorted
+    unsigned long long *pairs_tmp;        // [max_pairs] scatter target of the per-tile sort for lists longer than kSortCap
     uint32_t *vals;                       // [max_pairs] scan indices, grouped by tile, sorted by (depth, gid)
     float *image;                         // [3][H][W] for flod_render_to_host
 };

@@ -1,0 +1,200 @@
+// Step a7: every tile's pair list into (depth, gid) order ("in depth order"; R15).
+//
+// One CTA per tile.  The list holds unique 64-bit keys (depth bits << 32) | scan index, in the arbitrary order in
+// which k_duplicate's atomics were served.  It is sorted most-significant-digit first, without any stable ranking:
+//   bin pass   min / max of the keys -> bins of power-of-two width over [kmin, kmax] (at most 2048, about one key
+//              per bin) -> histogram with shared-memory atomics -> exclusive scan -> scatter with a second atomic.
+//              Bins are now in key order, keys inside a bin are not.
+//   rank pass  one thread per key counts the keys of its own bin that are smaller (a bin holds a few keys): that is
+//              its final position.  The 32-bit scan index is written to ws.vals.
+// A bin with more than kRankMax keys (a cluster of nearly equal depths) is binned once more over its own key range
+// (level 2, through global memory); what is still oversized after that is ranked by the whole block.
+// Lists of up to kSortCap keys are scattered into shared memory, longer ones into ws.pairs_tmp (global, L2).
+// Because the keys are unique the result is the unique sorted sequence whatever the atomics did.
+#include "flod_internal.cuh"
+
+namespace flod {
+
+constexpr int kSortThreads = 256;
+constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kSortBinsLog = 11;
+constexpr int kSortBins = 1 << kSortBinsLog;
+constexpr unsigned int kRankMax = 64;                     // bins up to this size are finished by per-key rank counting
+
+typedef unsigned long long u64;
+
+struct SortSmem {
+    u64 keys[kSortCap];                                   // level-1 scatter target of lists up to kSortCap keys
+    unsigned int ends[2][kSortBins];                      // per level: bin cursors; after the scatter, bin ends
+    u64 red_min[kSortWarps], red_max[kSortWarps];
+    unsigned int red_u[kSortWarps];
+    unsigned int wsum[kSortWarps];
+};
+
+struct BinMap { u64 kmin; int shift; unsigned int nb; };
+
+__device__ __forceinline__ unsigned int bin_of(const BinMap &m, u64 k) { return (unsigned int)((k - m.kmin) >> m.shift); }
+
+// Block-wide minimum of v (every thread gets it).  Two barriers.
+__device__ __forceinline__ unsigned int block_min_u32(SortSmem &S, unsigned int v, int tid)
+{
+    v = __reduce_min_sync(0xffffffffu, v);
+    if ((tid & 31) == 0) S.red_u[tid >> 5] = v;
+    __syncthreads();
+#pragma unroll
+    for (int w = 0; w < kSortWarps; ++w) v = min(v, S.red_u[w]);
+    __syncthreads();
+    return v;
+}
+
+// Distributes src[0, n) into dst[0, n) by bin (src and dst must not overlap).  On return ends[b] is the exclusive end
+// of bin b in dst (its start is ends[b-1], 0 for b = 0), and all writes are visible to the block.
+__device__ BinMap bin_pass(const u64 *src, u64 *dst, unsigned int n, unsigned int *ends, SortSmem &S, int tid)
+{
+    const int lane = tid & 31, warp = tid >> 5;
+    u64 kmin = ~0ull, kmax = 0ull;
+    for (unsigned int j = tid; j < n; j += kSortThreads) { const u64 k = src[j]; kmin = min(kmin, k); kmax = max(kmax, k); }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        kmin = min(kmin, __shfl_xor_sync(0xffffffffu, kmin, o));
+        kmax = max(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
+    }
+    if (lane == 0) { S.red_min[warp] = kmin; S.red_max[warp] = kmax; }
+    __syncthreads();
+#pragma unroll
+    for (int w = 0; w < kSortWarps; ++w) { kmin = min(kmin, S.red_min[w]); kmax = max(kmax, S.red_max[w]); }
+    BinMap m;
+    m.kmin = kmin;
+    const u64 range = kmax - kmin;
+    const int bits = range ? 64 - __clzll(range) : 0;
+    const int want = min(kSortBinsLog, max(8, 32 - __clz(max(n, 2u) - 1)));      // about one key per bin
+    m.shift = max(0, bits - want);
+    m.nb = (unsigned int)(range >> m.shift) + 1u;                                  // <= 2^want
+    for (unsigned int b = tid; b < m.nb; b += kSortThreads) ends[b] = 0;
+    __syncthreads();
+    for (unsigned int j = tid; j < n; j += kSortThreads) atomicAdd(&ends[bin_of(m, src[j])], 1u);
+    __syncthreads();
+    // exclusive scan of ends[0, nb): a thread owns ipt consecutive bins
+    {
+        const unsigned int ipt = (m.nb + kSortThreads - 1) / kSortThreads;
+        const unsigned int b0 = min(tid * ipt, m.nb), b1 = min(b0 + ipt, m.nb);
+        unsigned int sum = 0;
+        for (unsigned int b = b0; b < b1; ++b) sum += ends[b];
+        unsigned int incl = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        if (lane == 31) S.wsum[warp] = incl;
+        __syncthreads();
+        unsigned int run = incl - sum;
+#pragma unroll
+        for (int w = 0; w < kSortWarps; ++w) if (w < warp) run += S.wsum[w];
+        for (unsigned int b = b0; b < b1; ++b) { const unsigned int c = ends[b]; ends[b] = run; run += c; }
+    }
+    __syncthreads();
+    for (unsigned int j = tid; j < n; j += kSortThreads) {
+        const u64 k = src[j];
+        dst[atomicAdd(&ends[bin_of(m, k)], 1u)] = k;
+    }
+    __syncthreads();
+    return m;
+}
+
+// Final positions of the keys that sit in bins of at most kRankMax keys: position = bin start + number of smaller
+// keys in the bin.  buf[0, n) is the output of bin_pass; the scan indices go to out[0, n).
+__device__ __forceinline__ void rank_small(const u64 *buf, unsigned int n, const unsigned int *ends, const BinMap &m,
+                                           uint32_t *__restrict__ out, int tid)
+{
+    for (unsigned int p = tid; p < n; p += kSortThreads) {
+        const u64 k = buf[p];
+        const unsigned int b = bin_of(m, k);
+        const unsigned int lo = b ? ends[b - 1] : 0u, hi = ends[b];
+        if (hi - lo > kRankMax) continue;
+        unsigned int cnt = 0;
+        for (unsigned int q = lo; q < hi; ++q) cnt += buf[q] < k ? 1u : 0u;
+        out[lo + cnt] = (uint32_t)k;
+    }
+}
+
+// Smallest bin index >= from holding more than kRankMax keys, or ~0u.  Block-uniform result.
+__device__ __forceinline__ unsigned int next_big_bin(const unsigned int *ends, unsigned int nb, unsigned int from,
+                                                     SortSmem &S, int tid)
+{
+    unsigned int cand = 0xffffffffu;
+    for (unsigned int b = from + tid; b < nb; b += kSortThreads) {
+        const unsigned int lo = b ? ends[b - 1] : 0u;
+        if (ends[b] - lo > kRankMax) { cand = b; break; }
+    }
+    return block_min_u32(S, cand, tid);
+}
+
+// Sorts buf[0, n) (output of a level-1 bin pass with map m / ends) into out[0, n).  scratch[0, n) is global memory the
+// block may overwrite (level-2 scatter target).
+__device__ void finish_sort(const u64 *buf, unsigned int n, const BinMap &m, u64 *scratch, uint32_t *__restrict__ out,
+                            SortSmem &S, int tid)
+{
+    const unsigned int *ends = S.ends[0];
+    rank_small(buf, n, ends, m, out, tid);
+    unsigned int from = 0;
+    while (true) {
+        const unsigned int b = next_big_bin(ends, m.nb, from, S, tid);
+        if (b == 0xffffffffu) break;
+        from = b + 1;
+        const unsigned int lo = b ? ends[b - 1] : 0u, n2 = ends[b] - lo;
+        // ---- level 2: the bin over its own key range
+        u64 *buf2 = scratch + lo;
+        const BinMap m2 = bin_pass(buf + lo, buf2, n2, S.ends[1], S, tid);
+        const unsigned int *ends2 = S.ends[1];
+        rank_small(buf2, n2, ends2, m2, out + lo, tid);
+        unsigned int from2 = 0;
+        while (true) {
+            const unsigned int b2 = next_big_bin(ends2, m2.nb, from2, S, tid);
+            if (b2 == 0xffffffffu) break;
+            from2 = b2 + 1;
+            // ---- still oversized (nested clusters of nearly equal keys): rank counting by the whole block
+            const unsigned int lo2 = b2 ? ends2[b2 - 1] : 0u, hi2 = ends2[b2];
+            for (unsigned int p = lo2 + tid; p < hi2; p += kSortThreads) {
+                const u64 k = buf2[p];
+                unsigned int cnt = 0;
+                for (unsigned int q = lo2; q < hi2; ++q) cnt += buf2[q] < k ? 1u : 0u;
+                out[lo + lo2 + cnt] = (uint32_t)k;
+            }
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kSortThreads)
+k_tile_sort(const WorkspaceDev ws, int n_tiles)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    SortSmem &S = *reinterpret_cast<SortSmem *>(smem_raw);
+
+    const int tile = blockIdx.x;
+    if (tile >= n_tiles) return;
+    const int tid = threadIdx.x;
+    const uint2 rg = ws.ranges[tile];
+    const unsigned int L = rg.y - rg.x;
+    if (L == 0 || ws.hdr->overflow) return;            // an overflowed frame is undefined (and its keys need not be unique)
+    u64 *pairs = ws.pairs + rg.x;
+    uint32_t *vals = ws.vals + rg.x;
+    if (L == 1) { if (tid == 0) vals[0] = (uint32_t)pairs[0]; return; }
+    u64 *buf = L <= (unsigned int)kSortCap ? S.keys : ws.pairs_tmp + rg.x;
+    const BinMap m = bin_pass(pairs, buf, L, S.ends[0], S, tid);
+    finish_sort(buf, L, m, pairs, vals, S, tid);
+}
+
+int launch_tile_sort(const Context &c, const FrameParams &p, cudaStream_t s)
+{
+    if (p.n_pre_blocks <= 0) return 0;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_tile_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
+        attr_set = true;
+    }
+    k_tile_sort<<<p.n_tiles, kSortThreads, sizeof(SortSmem), s>>>(c.ws, p.n_tiles);
+    return 1;
+}
+
+}  // namespace flod

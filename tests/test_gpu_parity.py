@@ -218,6 +218,31 @@ def test_screen_filling_and_degenerate_gaussians(pkg):
     r.close()
 
 
+def test_sort_corner_cases_long_lists_and_depth_plateaus(pkg):
+    """Per-tile ordering (R15) where the per-tile sort leaves its common path: tile lists far longer than its
+    shared-memory capacity, thousands of exactly equal depths in one tile (planes facing the camera: the order is
+    decided by gid alone), and nested clusters of nearly equal depths inside a wide depth range."""
+    rng = np.random.default_rng(77)
+    n_plane, n_cl, n_far = 10000, 3000, 2000
+    # two planes of identical camera depth (identity pose: depth = z exactly), small footprints over 2x2 tiles
+    xy = rng.uniform(-0.06, 0.06, (2 * n_plane, 2))
+    z = np.repeat([2.0, 2.5], n_plane)
+    plane = np.column_stack([xy * z[:, None], z])
+    # nested clusters: depths 4 + k * 2^-20 (adjacent fp32 values around 4), and a wide-range background
+    cl = np.column_stack([rng.uniform(-0.3, 0.3, (n_cl, 2)), 4.0 + rng.integers(0, 40, n_cl) * 2.0 ** -20])
+    far = np.column_stack([rng.uniform(-2, 2, (n_far, 2)), rng.uniform(0.3, 400.0, n_far)])
+    pos = np.concatenate([plane, cl, far])
+    pos = pos[rng.permutation(len(pos))]
+    lv = level(1, 0.0, pos, 0.004 * pos[:, 2:3] * np.ones((1, 3)), opacity=rng.uniform(0.02, 0.2, len(pos)),
+               rgb=rng.uniform(0, 1, (len(pos), 3)))
+    cam = camera(width=64, height=48, f=100.0)
+    r = make_renderer(pkg, [lv], 0, 64, 48, max_pairs=1 << 20)
+    osc = OracleScene([lv], 0)
+    _, _, fr = check_frame(r, osc, cam, 1, 1, 1.0)
+    assert fr.tile_counts.max() > 2 * 4096          # beyond the shared-memory path of the sort
+    r.close()
+
+
 def test_needle_gaussians_stay_within_tolerance(pkg):
     """DESIGN R25: long thin footprints (short axis at the dilation floor) are where the textbook exponent loses
     precision in fp32; the factorised form keeps the image within 1e-3."""
