@@ -18,6 +18,7 @@ namespace flod {
 constexpr int kBlendThreads = 128;
 constexpr int kBatch = 256;
 constexpr int kBlendWarps = kBlendThreads / 32;
+constexpr float kTwo100 = 1.2676506002282294e30f;   // 2^100
 
 // 2^x on the MUFU unit (x <= 0 here; results below 2^-126 flush to 0, far under the 1/255 skip threshold)
 __device__ __forceinline__ float ex2(float x)
@@ -32,10 +33,9 @@ __global__ void __launch_bounds__(kBlendThreads)
 k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, int n_tiles,
         float bg0, float bg1, float bg2)
 {
-    __shared__ float4 s_a[kBatch];                      // mu'x, mu'y, k, -a2
-    __shared__ float4 s_b[kBatch];                      // -d2, log2 o, r, g
-    __shared__ float s_c[kBatch];                       // b
-    __shared__ unsigned char s_list[kBlendWarps][kBatch];
+    // one 48-byte record per Gaussian of the batch: (mu'x, mu'y, k, a2 | d2, log2 o, r, g | b, -, -, -)
+    __shared__ float4 s_rec[kBatch * 3];
+    __shared__ unsigned short s_list[kBlendWarps][kBatch];   // per warp: byte offsets of the surviving records
 
     const int tile = blockIdx.x;
     if (tile >= n_tiles || ws.hdr->overflow) return;   // an overflowed frame is undefined: its lists were not sorted
@@ -57,11 +57,16 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
     const float4 *__restrict__ gB = ws.gB;
     const float *__restrict__ cB = ws.cB;
 
-    float T0 = 1.0f, r0 = 0.0f, g0 = 0.0f, b0 = 0.0f;
-    float T1 = 1.0f, r1 = 0.0f, g1 = 0.0f, b1 = 0.0f;
+    // two pixels per thread, packed as float2 (.x = row py0, .y = row py1): the per-pixel arithmetic runs on the
+    // packed FP32 instructions of sm_100 (FADD2 / FMUL2 / FFMA2: one issue slot for both pixels)
+    float2 T = make_float2(1.0f, 1.0f), cr = make_float2(0.0f, 0.0f), cg = cr, cb2 = cr;
+    const float2 npyc = make_float2(-pyc0, -pyc1);
     bool done0 = !in0, done1 = !in1;
     unsigned int n_eval = 0, n_blend = 0;
-    unsigned char *my_list = s_list[warp];
+    unsigned short *my_list = s_list[warp];
+    const unsigned char *rec_bytes = reinterpret_cast<const unsigned char *>(s_rec);
+    // done pixels: thr = +huge, so that no alpha passes the skip test (live pixels: thr = 1/255)
+    float thr0 = in0 ? (1.0f / 255.0f) : 3.0e38f, thr1 = in1 ? (1.0f / 255.0f) : 3.0e38f;
 
     for (unsigned int base = rg.x; base < rg.y; base += kBatch) {
         const bool warp_done = __all_sync(0xffffffffu, done0 && done1);
@@ -72,9 +77,9 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
             const unsigned int j = tid + h * kBlendThreads;
             if (j < m) {
                 const uint32_t ci = vals[base + j];
-                s_a[j] = gA[ci];
-                s_b[j] = gB[ci];
-                s_c[j] = cB[ci];
+                s_rec[3 * j] = gA[ci];
+                s_rec[3 * j + 1] = gB[ci];
+                s_rec[3 * j + 2].x = cB[ci];
             }
         }
         __syncthreads();
@@ -87,8 +92,8 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
             const unsigned int j = lane + 32 * i;
             bool hit = false;
             if (j < m) {
-                const float4 a = s_a[j];
-                const float4 b = s_b[j];
+                const float4 a = s_rec[3 * j];
+                const float4 b = s_rec[3 * j + 1];
                 const float dxl = a.x - sx1, dxh = a.x - sx0;        // range of (mu'x - x) over the strip
                 float best = -INFINITY;
 #pragma unroll
@@ -102,45 +107,47 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
                 hit = best >= kThr;
             }
             const unsigned int bal = __ballot_sync(0xffffffffu, hit);
-            if (hit) my_list[cnt + __popc(bal & ((1u << lane) - 1))] = (unsigned char)j;
+            if (hit) my_list[cnt + __popc(bal & ((1u << lane) - 1))] = (unsigned short)(j * 48u);
             cnt += __popc(bal);
         }
         __syncwarp();
 
-        // ---- evaluate the survivors, two pixels per thread
+        // ---- evaluate the survivors.  a.w and b.x are <= 0 (k_geometry clamps them), so e <= log2 o: q >= 0 holds
+        // by construction and alpha needs the 0.99 clamp only.  A pixel that is done or below 1/255 blends alpha = 0.
+#pragma unroll 2
         for (unsigned int t = 0; t < cnt; ++t) {
-            const unsigned int j = my_list[t];
-            const float4 a = s_a[j];
-            const float4 b = s_b[j];
+            const unsigned int off = my_list[t];
+            const float4 a = *reinterpret_cast<const float4 *>(rec_bytes + off);
+            const float4 b = *reinterpret_cast<const float4 *>(rec_bytes + off + 16);
+            const float cbj = *reinterpret_cast<const float *>(rec_bytes + off + 32);
             const float dx = a.x - pxc;
-            const float dy0 = a.y - pyc0, dy1 = a.y - pyc1;
-            const float w0 = fmaf(a.z, dy0, dx), w1 = fmaf(a.z, dy1, dx);
-            float e0 = fmaf(a.w, w0 * w0, fmaf(b.x, dy0 * dy0, b.y));
-            float e1 = fmaf(a.w, w1 * w1, fmaf(b.x, dy1 * dy1, b.y));
-            e0 = fminf(e0, b.y);                                      // q >= 0 (the oracle clamps q at 0)
-            e1 = fminf(e1, b.y);
-            const float al0 = fminf(ex2(e0), 0.99f), al1 = fminf(ex2(e1), 0.99f);
-            const bool u0 = !done0 && al0 >= (1.0f / 255.0f);
-            const bool u1 = !done1 && al1 >= (1.0f / 255.0f);
-            if (u0 || u1) {
-                const float cb = s_c[j];
-                if (u0) {
-                    const float wgt = T0 * al0;
-                    r0 = fmaf(wgt, b.z, r0); g0 = fmaf(wgt, b.w, g0); b0 = fmaf(wgt, cb, b0);
-                    T0 -= wgt;                                        // T (1 - alpha)
-                    if (T0 < 1e-4f) { done0 = true; if (COUNT) n_eval += (base - rg.x) + j + 1; }   // blend, then stop (R12)
-                    if (COUNT) ++n_blend;
-                }
-                if (u1) {
-                    const float wgt = T1 * al1;
-                    r1 = fmaf(wgt, b.z, r1); g1 = fmaf(wgt, b.w, g1); b1 = fmaf(wgt, cb, b1);
-                    T1 -= wgt;
-                    if (T1 < 1e-4f) { done1 = true; if (COUNT) n_eval += (base - rg.x) + j + 1; }
-                    if (COUNT) ++n_blend;
-                }
+            const float2 dy = __fadd2_rn(make_float2(a.y, a.y), npyc);
+            const float2 w = __ffma2_rn(make_float2(a.z, a.z), dy, make_float2(dx, dx));
+            const float2 e = __ffma2_rn(make_float2(a.w, a.w), __fmul2_rn(w, w),
+                                        __ffma2_rn(make_float2(b.x, b.x), __fmul2_rn(dy, dy), make_float2(b.y, b.y)));
+            float al0 = fminf(ex2(e.x), 0.99f), al1 = fminf(ex2(e.y), 0.99f);
+            al0 = al0 >= thr0 ? al0 : 0.0f;
+            al1 = al1 >= thr1 ? al1 : 0.0f;
+            const float2 wgt = __fmul2_rn(T, make_float2(al0, al1));
+            cr = __ffma2_rn(wgt, make_float2(b.z, b.z), cr);
+            cg = __ffma2_rn(wgt, make_float2(b.w, b.w), cg);
+            cb2 = __ffma2_rn(wgt, make_float2(cbj, cbj), cb2);
+            T = __fadd2_rn(T, make_float2(-wgt.x, -wgt.y));           // T (1 - alpha)
+            if (COUNT) {
+                n_blend += (al0 > 0.0f ? 1u : 0u) + (al1 > 0.0f ? 1u : 0u);
+                if (thr0 < 1.0f && T.x < 1e-4f) n_eval += (base - rg.x) + off / 48u + 1;
+                if (thr1 < 1.0f && T.y < 1e-4f) n_eval += (base - rg.x) + off / 48u + 1;
             }
+            // blend, then stop (R12): (1e-4 - T) 2^100 is positive exactly when T < 1e-4 (the scaling by a power of
+            // two and the difference of the two products are exact up to one rounding that keeps the sign), and
+            // then at least 2^-37 2^100 > 0.99
+            const float2 stop = __ffma2_rn(T, make_float2(-kTwo100, -kTwo100), make_float2(1e-4f * kTwo100, 1e-4f * kTwo100));
+            thr0 = fmaxf(thr0, stop.x);
+            thr1 = fmaxf(thr1, stop.y);
         }
+        done0 = thr0 > 1.0f; done1 = thr1 > 1.0f;
     }
+    const float T0 = T.x, T1 = T.y, r0 = cr.x, r1 = cr.y, g0 = cg.x, g1 = cg.y, b0 = cb2.x, b1 = cb2.y;
     const size_t plane = (size_t)W * H;
     if (in0) {
         const size_t o = (size_t)py0 * W + px;

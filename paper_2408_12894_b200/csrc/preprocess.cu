@@ -150,7 +150,9 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
         const double dA = (double)cA, dB = (double)cB, dC = (double)cC;
         const float kk = (float)(dB / dA);
         const float a2 = (float)(-0.5 * LOG2E * dA);                   // stored negated: e = log2 o + a2 w^2 + d2 dy^2
-        const float d2 = (float)(-0.5 * LOG2E * (dC - dB * dB / dA));
+        // <= 0 so that q >= 0 holds by construction in k_blend (the oracle clamps q at 0; a conic left indefinite by
+        // rounding differs from its clamp by less than R25's evaluation error)
+        const float d2 = fminf((float)(-0.5 * LOG2E * (dC - dB * dB / dA)), 0.0f);
         ws.gA[i] = make_float4(mx2, my2, kk, a2);
         reinterpret_cast<float2 *>(ws.gB)[2 * (size_t)i] = make_float2(d2, __ldg(sc.l2o + g));   // (r, g) by k_colour
         ws.rect[i] = make_ushort4((unsigned short)tx0, (unsigned short)ty0, (unsigned short)tx1, (unsigned short)ty1);
