@@ -4,7 +4,7 @@
 //   k_tile_scan   a5/a8  2-D prefix sum of the difference grid written by k_geometry = pairs per tile; exclusive
 //                        scan over the tiles = [start, end) of every tile's list (the ranges of step a8);
 //   k_duplicate   a6     every (visible Gaussian, tile of its rect) pair takes the next free slot of ITS TILE's list
-//                        (one integer atomic) and stores the 64-bit key (depth bits << 32) | scan index;
+//                        (one integer atomic) and stores the 64-bit key (depth bits << 32) | position;
 //   k_tile_sort   a7     (tile_sort.cu) one CTA per tile sorts its list by that key.  The key is unique, so the
 //                        result does not depend on the order in which the atomics were served.
 #include "flod_internal.cuh"
@@ -78,75 +78,83 @@ int launch_tile_scan(const Context &c, const FrameParams &p, cudaStream_t s)
 }
 
 // ------------------------------------------------------------------------------------------------ a6
-// Persistent blocks over the visible list, kPreBlock Gaussians per step.  A block scan of the rect areas lets the
-// block expand its rects cooperatively, one pair per thread per step, whatever the individual rect sizes.
+// One block per segment of k_geometry (up to kGeoBlock visible Gaussians, four per thread).  A block scan of the rect
+// areas lets the block expand its rects cooperatively, one pair per thread per step, whatever the individual sizes.
+constexpr int kDupPer = kGeoBlock / kPreBlock;
+
 __global__ void __launch_bounds__(kPreBlock)
 k_duplicate(const WorkspaceDev ws, int TX, unsigned int max_pairs)
 {
     __shared__ unsigned int s_warp_tot[kPreBlock / 32];
-    __shared__ unsigned int s_incl[kPreBlock];      // inclusive pair scan of the step
-    __shared__ unsigned int s_rect[kPreBlock];      // tx0 | ty0 << 16
-    __shared__ unsigned int s_wd[kPreBlock];        // rect width
-    __shared__ unsigned int s_idx[kPreBlock];       // scan index
-    __shared__ unsigned int s_depth[kPreBlock];     // depth bits
+    __shared__ unsigned int s_incl[kGeoBlock];      // inclusive pair scan of the segment
+    __shared__ unsigned int s_rect[kGeoBlock];      // tx0 | ty0 << 16
+    __shared__ unsigned int s_wd[kGeoBlock];        // rect width
+    __shared__ unsigned int s_depth[kGeoBlock];     // depth bits
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const unsigned int n_vis = ws.hdr->n_vis32;
-    for (unsigned int base = blockIdx.x * kPreBlock; base < n_vis; base += gridDim.x * kPreBlock) {
-        const unsigned int s = base + tid;
-        unsigned int n_tiles = 0;
-        if (s < n_vis) {
-            const unsigned int i = ws.vis_list[s];
-            const ushort4 rc = ws.rect[i];
+    const unsigned int seg = blockIdx.x;
+    const unsigned int n_here = ws.seg_count[seg];
+    if (n_here == 0) return;
+    const unsigned int p0 = seg * kGeoBlock;
+    // thread t owns entries kDupPer t .. kDupPer t + kDupPer - 1 (consecutive, so that the scan is a plain block scan)
+    unsigned int nt[kDupPer], mine = 0;
+#pragma unroll
+    for (int k = 0; k < kDupPer; ++k) {
+        const unsigned int j = tid * kDupPer + k;
+        nt[k] = 0;
+        if (j < n_here) {
+            const ushort4 rc = ws.rect[p0 + j];
             const unsigned int w = (unsigned int)rc.z - rc.x;
-            n_tiles = w * ((unsigned int)rc.w - rc.y);
-            s_idx[tid] = i;
-            s_depth[tid] = ws.depth[i];
-            s_rect[tid] = (unsigned int)rc.x | ((unsigned int)rc.y << 16);
-            s_wd[tid] = w;
+            nt[k] = w * ((unsigned int)rc.w - rc.y);
+            s_depth[j] = ws.depth[p0 + j];
+            s_rect[j] = (unsigned int)rc.x | ((unsigned int)rc.y << 16);
+            s_wd[j] = w;
         }
-        unsigned int incl = n_tiles;
+        mine += nt[k];
+    }
+    unsigned int incl = mine;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const unsigned int n = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += n;
-        }
-        if (lane == 31) s_warp_tot[warp] = incl;
-        __syncthreads();
-        unsigned int warp_off = 0, block_pairs = 0;
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int n = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += n;
+    }
+    if (lane == 31) s_warp_tot[warp] = incl;
+    __syncthreads();
+    unsigned int run = incl - mine, block_pairs = 0;
 #pragma unroll
-        for (int w = 0; w < kPreBlock / 32; ++w) {
-            const unsigned int t = s_warp_tot[w];
-            if (w < warp) warp_off += t;
-            block_pairs += t;
+    for (int w = 0; w < kPreBlock / 32; ++w) {
+        const unsigned int t = s_warp_tot[w];
+        if (w < warp) run += t;
+        block_pairs += t;
+    }
+#pragma unroll
+    for (int k = 0; k < kDupPer; ++k) {
+        run += nt[k];
+        const unsigned int j = tid * kDupPer + k;
+        if (j < n_here) s_incl[j] = run;
+    }
+    __syncthreads();
+    for (unsigned int q = tid; q < block_pairs; q += kPreBlock) {
+        int lo = 0, hi = (int)n_here - 1;              // first entry with s_incl[entry] > q
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if (s_incl[mid] > q) hi = mid; else lo = mid + 1;
         }
-        s_incl[tid] = incl + warp_off;
-        __syncthreads();
-        const int n_here = (int)min((unsigned int)kPreBlock, n_vis - base);
-        for (unsigned int q = tid; q < block_pairs; q += kPreBlock) {
-            int lo = 0, hi = n_here - 1;               // first position with s_incl[pos] > q
-            while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if (s_incl[mid] > q) hi = mid; else lo = mid + 1;
-            }
-            const unsigned int r = (unsigned int)lo;
-            const unsigned int k = q - (r ? s_incl[r - 1] : 0u);
-            const unsigned int w = s_wd[r];
-            const unsigned int ry = k / w, rx = k - ry * w;
-            const unsigned int rc = s_rect[r];
-            const unsigned int tile = ((rc >> 16) + ry) * (unsigned int)TX + ((rc & 0xffffu) + rx);
-            const unsigned int pos = atomicAdd(ws.cursor + (size_t)tile * kCtrStride, 1u);
-            if (pos < max_pairs) ws.pairs[pos] = ((unsigned long long)s_depth[r] << 32) | s_idx[r];
-        }
-        __syncthreads();
+        const unsigned int r = (unsigned int)lo;
+        const unsigned int k = q - (r ? s_incl[r - 1] : 0u);
+        const unsigned int w = s_wd[r];
+        const unsigned int ry = k / w, rx = k - ry * w;
+        const unsigned int rc = s_rect[r];
+        const unsigned int tile = ((rc >> 16) + ry) * (unsigned int)TX + ((rc & 0xffffu) + rx);
+        const unsigned int pos = atomicAdd(ws.cursor + (size_t)tile * kCtrStride, 1u);
+        if (pos < max_pairs) ws.pairs[pos] = ((unsigned long long)s_depth[r] << 32) | (p0 + r);
     }
 }
 
 int launch_duplicate(const Context &c, const FrameParams &p, cudaStream_t s)
 {
     if (p.n_pre_blocks <= 0) return 0;
-    const int grid = min(p.n_pre_blocks, c.sm_count * 8);
-    k_duplicate<<<grid, kPreBlock, 0, s>>>(c.ws, p.TX, p.max_pairs);
+    k_duplicate<<<p.n_pre_blocks, kPreBlock, 0, s>>>(c.ws, p.TX, p.max_pairs);
     return 1;
 }
 

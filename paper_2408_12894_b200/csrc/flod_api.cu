@@ -97,9 +97,10 @@ WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_p
     auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return (unsigned char *)((uintptr_t)base + o); };
     const size_t tx = (size_t)(w + kTile - 1) / kTile, ty = (size_t)(h + kTile - 1) / kTile;
     const size_t tiles = tx * ty;
-    const size_t nt = (size_t)std::max<int64_t>(n_total, 1);
+    const size_t nt = (size_t)std::max<int64_t>(n_total, 1) + 2 * kGeoBlock;   // segment positions (see WorkspaceDev)
     L.ws.hdr = (FrameHeader *)take(sizeof(FrameHeader));
     L.ws.tile_diff = (int *)take((tx + 1) * (ty + 1) * kCtrStride * sizeof(int));
+    L.ws.seg_count = (unsigned int *)take((nt / kGeoBlock + 2) * sizeof(unsigned int));
     L.ws.tile_cnt = (int *)take((tx + 1) * (ty + 1) * sizeof(int));
     L.ws.ranges = (uint2 *)take(tiles * sizeof(uint2));
     L.ws.cursor = (unsigned int *)take(tiles * kCtrStride * sizeof(unsigned int));
@@ -109,7 +110,6 @@ WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_p
     L.ws.dirgid = (float4 *)take(nt * sizeof(float4));
     L.ws.rect = (ushort4 *)take(nt * sizeof(ushort4));
     L.ws.depth = (uint32_t *)take(nt * sizeof(uint32_t));
-    L.ws.vis_list = (uint32_t *)take(nt * sizeof(uint32_t));
     L.ws.dbg = (flod_dbg_projected *)take(nt * sizeof(flod_dbg_projected));
     L.ws.mask = (uint8_t *)take(nt);
     L.ws.pairs = (unsigned long long *)take((size_t)max_pairs * 8);
@@ -355,13 +355,14 @@ int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, flo
     }
     for (int k = 0; k < p.n_levels; ++k) p.hi2[k] = (k == 0) ? INFINITY : p.lo2[k - 1];  // d_proj^(L_start-1) = inf
     p.max_pairs = (unsigned int)ctx->max_pairs;
-    p.n_pre_blocks = (int)((n_scan + kPreBlock - 1) / kPreBlock);
+    p.quad_gid = p.first_gid & ~3ll;
+    p.n_pre_blocks = (int)((p.first_gid - p.quad_gid + n_scan + kGeoBlock - 1) / kGeoBlock);
     p.n_tiles = p.TX * p.TY;
 
     cudaStream_t s = (cudaStream_t)stream;
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     const bool prof = ctx->flags & FLOD_OPT_PROFILE;
-    // zero the header and the tile difference grid (contiguous)
+    // zero the header and the tile difference grid (contiguous in the workspace)
     const size_t zero_bytes = (size_t)((unsigned char *)ctx->ws.tile_diff - (unsigned char *)ctx->ws.hdr) +
                               (size_t)(p.TX + 1) * (p.TY + 1) * kCtrStride * sizeof(int);
     CUDA_TRY(ctx, cudaMemsetAsync(ctx->ws.hdr, 0, zero_bytes, s));
@@ -379,7 +380,7 @@ int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, flo
     CUDA_TRY(ctx, cudaGetLastError());
     ctx->ev_valid = prof;
     ctx->last_stream = s; ctx->rendered = true;
-    ctx->last_n_scan = n_scan;
+    ctx->last_n_scan = n_scan; ctx->last_n_segs = p.n_pre_blocks;
     ctx->last_w = p.W; ctx->last_h = p.H; ctx->last_tx = p.TX; ctx->last_ty = p.TY; ctx->last_first_gid = p.first_gid;
     return FLOD_OK;
 }
@@ -459,22 +460,28 @@ int flod_debug_copy(flod_ctx *ctx, int what, void *host_dst, size_t bytes)
         }
         case FLOD_DBG_PROJECTED: {
             if (!(ctx->flags & FLOD_OPT_DEBUG)) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: PROJECTED needs FLOD_OPT_DEBUG");
-            const size_t nv = (size_t)h.n_vis32, ns = (size_t)ctx->last_n_scan;
+            const size_t nv = (size_t)h.n_vis32, nseg = (size_t)ctx->last_n_segs;
             if (bytes < nv * sizeof(flod_dbg_projected)) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: buffer too small");
-            std::vector<flod_dbg_projected> all(std::max<size_t>(ns, 1));
-            CUDA_TRY(ctx, cudaMemcpy(all.data(), ctx->ws.dbg, ns * sizeof(flod_dbg_projected), cudaMemcpyDeviceToHost));
+            // segment s holds seg_count[s] records at positions s * kGeoBlock ..: concatenated they are in ascending gid
+            std::vector<unsigned int> cnt(std::max<size_t>(nseg, 1));
+            CUDA_TRY(ctx, cudaMemcpy(cnt.data(), ctx->ws.seg_count, nseg * 4, cudaMemcpyDeviceToHost));
             flod_dbg_projected *dst = (flod_dbg_projected *)host_dst;
             size_t k = 0;
-            for (size_t i = 0; i < ns && k < nv; ++i)          // records sit at the scan index: compact in ascending gid
-                if (all[i].gid != 0xffffffffu) dst[k++] = all[i];
+            for (size_t sgm = 0; sgm < nseg && k < nv; ++sgm) {
+                const size_t m = std::min<size_t>(cnt[sgm], nv - k);
+                if (m) CUDA_TRY(ctx, cudaMemcpy(dst + k, ctx->ws.dbg + sgm * kGeoBlock, m * sizeof(flod_dbg_projected), cudaMemcpyDeviceToHost));
+                k += m;
+            }
             return FLOD_OK;
         }
         case FLOD_DBG_SORTED_PAIRS: {
-            const size_t np = (size_t)h.n_pairs_clamped, ns = (size_t)ctx->last_n_scan;
+            const size_t np = (size_t)h.n_pairs_clamped, ns = (size_t)ctx->last_n_segs * kGeoBlock;
             if (bytes < np * sizeof(flod_dbg_pair)) return fail(ctx, FLOD_E_INVALID_ARG, "debug_copy: buffer too small");
             const size_t tiles = (size_t)ctx->last_tx * ctx->last_ty;
             std::vector<uint2> r(std::max<size_t>(tiles, 1));
             std::vector<uint32_t> v(std::max<size_t>(np, 1)), dz(std::max<size_t>(ns, 1));
+            std::vector<float4> dg(std::max<size_t>(ns, 1));
+            CUDA_TRY(ctx, cudaMemcpy(dg.data(), ctx->ws.dirgid, ns * sizeof(float4), cudaMemcpyDeviceToHost));
             CUDA_TRY(ctx, cudaMemcpy(r.data(), ctx->ws.ranges, tiles * sizeof(uint2), cudaMemcpyDeviceToHost));
             CUDA_TRY(ctx, cudaMemcpy(v.data(), ctx->ws.vals, np * 4, cudaMemcpyDeviceToHost));
             CUDA_TRY(ctx, cudaMemcpy(dz.data(), ctx->ws.depth, ns * 4, cudaMemcpyDeviceToHost));
@@ -485,7 +492,9 @@ int flod_debug_copy(flod_ctx *ctx, int what, void *host_dst, size_t bytes)
                     const uint32_t si = v[i];
                     const uint32_t bits = si < ns ? dz[si] : 0u;
                     memcpy(&dst[i].depth, &bits, 4);
-                    dst[i].gid = si < ns ? (uint32_t)(ctx->last_first_gid + si) : 0xffffffffu;
+                    uint32_t gid = 0xffffffffu;
+                    if (si < ns) memcpy(&gid, &dg[si].w, 4);
+                    dst[i].gid = gid;
                 }
             return FLOD_OK;
         }

@@ -12,7 +12,10 @@
 namespace flod {
 
 constexpr int kTile = FLOD_TILE;
-constexpr int kPreBlock = 256;            // geometry / duplication: Gaussians per block
+constexpr int kPreBlock = 256;            // duplication: visible Gaussians per block step
+constexpr int kGeoThreads = 256;          // geometry: threads per block, four consecutive Gaussians per thread
+constexpr int kGeoPer = 4;
+constexpr int kGeoBlock = kGeoThreads * kGeoPer;
 constexpr int kSortCap = 4096;            // per-tile sort: lists up to this many keys are scattered into shared memory
 constexpr int kCtrStride = 64;            // ints between two per-tile atomic counters: one counter per 256 B, so that the
                                           // L2 slices share the atomic traffic (a dense 16 KB grid sits on a few slices)
@@ -31,7 +34,7 @@ struct SceneDev {
 
 // Per-frame counters, zeroed (with the tile difference grid) by one memset at the start of every frame.
 struct FrameHeader {
-    unsigned int n_vis32;                 // visible Gaussians = length of vis_list
+    unsigned int n_vis32;                 // visible Gaussians = length of the compact per-frame arrays
     unsigned int overflow;
     unsigned int n_pairs_clamped;         // min(n_pairs, max_pairs)
     unsigned int pad;
@@ -39,26 +42,28 @@ struct FrameHeader {
     unsigned long long evals, blends;
 };
 
-// Everything per Gaussian is indexed by the SCAN INDEX i = gid - first_gid of the frame (no compaction: visible
-// Gaussians write their records in place, invisible ones write nothing).  Blend features (DESIGN R25):
-//   gA = (mu'x, mu'y, k = B/A, -A log2(e)/2)     gB = (-(C - B^2/A) log2(e)/2, log2 o, r, g)    cB = b
+// Everything per Gaussian is indexed by the POSITION p = segment * kGeoBlock + j: block `segment` of k_geometry
+// scans kGeoBlock consecutive gids and writes the records of its seg_count[segment] visible ones, in ascending gid
+// order, at the front of its segment (j < seg_count).  So p-order = gid-order, every segment is a dense run of full
+// sectors, and no inter-block scan is needed.  Blend features (DESIGN R25):
+//   gA = (mu'x, mu'y, k = B/A, -A log2(e)/2)     gB = (min(0, -(C - B^2/A) log2(e)/2), log2 o, r, g)    cB = b
 struct WorkspaceDev {
     FrameHeader *hdr;
     int *tile_diff;                       // [(TX+1)*(TY+1)][kCtrStride] 2-D difference grid of the tile counts (zeroed per frame)
+    unsigned int *seg_count;              // [geometry blocks] visible Gaussians of every segment
     int *tile_cnt;                        // [(TX+1)*(TY+1)] dense copy, used by the tile scan when the grid exceeds shared memory
     uint2 *ranges;                        // [T_n] (start, end) of every tile's pair list
     unsigned int *cursor;                 // [T_n][kCtrStride] next free slot of every tile's list during duplication
-    float4 *gA, *gB;                      // [n_total]
-    float *cB;                            // [n_total]
-    float4 *dirgid;                       // [n_total] (mu - c_cam, gid bits): input of the colour kernel
-    ushort4 *rect;                        // [n_total] tx0, ty0, tx1, ty1
-    uint32_t *depth;                      // [n_total] depth bits
-    uint32_t *vis_list;                   // [n_total] scan indices of the visible Gaussians, unordered
-    flod_dbg_projected *dbg;              // [n_total] (written only with FLOD_OPT_DEBUG; gid = ~0 when not visible)
-    uint8_t *mask;                        // [n_total] (written only with FLOD_OPT_DEBUG)
-    unsigned long long *pairs;            // [max_pairs] (depth bits << 32) | scan index, grouped by tile, unsorted
+    float4 *gA, *gB;                      // [n_total + 2 kGeoBlock]
+    float *cB;                            // [n_total + 2 kGeoBlock]
+    float4 *dirgid;                       // [n_total + 2 kGeoBlock] (mu - c_cam, gid bits): input of the colour kernel
+    ushort4 *rect;                        // [n_total + 2 kGeoBlock] tx0, ty0, tx1, ty1
+    uint32_t *depth;                      // [n_total + 2 kGeoBlock] depth bits (p_z > 0, so unsigned order = float order)
+    flod_dbg_projected *dbg;              // [n_total + 2 kGeoBlock] (written only with FLOD_OPT_DEBUG)
+    uint8_t *mask;                        // [n_total + 2 kGeoBlock] (written only with FLOD_OPT_DEBUG)
+    unsigned long long *pairs;            // [max_pairs] (depth bits << 32) | position, grouped by tile, unsorted
     unsigned long long *pairs_tmp;        // [max_pairs] scatter target of the per-tile sort for lists longer than kSortCap
-    uint32_t *vals;                       // [max_pairs] scan indices, grouped by tile, sorted by (depth, gid)
+    uint32_t *vals;                       // [max_pairs] positions, grouped by tile, sorted by (depth, gid)
     float *image;                         // [3][H][W] for flod_render_to_host
 };
 
@@ -71,12 +76,14 @@ struct FrameParams {
     float bg[3];
     int W, H, TX, TY;
     long long first_gid;                  // gid of the first scanned Gaussian
+    long long quad_gid;                   // first_gid rounded down to a multiple of 4: thread q of k_geometry owns
+                                          // gids quad_gid + 4 q .. + 3 (16-byte aligned in every plane)
     int n_scan;
     int n_levels;                         // levels in the range
     int level_end[FLOD_MAX_LEVELS];       // cumulative end (scan index) of each level in the range
     float lo2[FLOD_MAX_LEVELS], hi2[FLOD_MAX_LEVELS];
     unsigned int max_pairs;
-    int n_pre_blocks;
+    int n_pre_blocks;                     // blocks of k_geometry
     int n_tiles;                          // TX * TY
 };
 
@@ -106,6 +113,7 @@ struct Context {
     int last_w = 0, last_h = 0, last_tx = 0, last_ty = 0;
     int64_t last_first_gid = 0;
     int64_t last_n_scan = 0;
+    int last_n_segs = 0;
     cudaEvent_t ev[FLOD_N_STAGES + 1] = {nullptr};
     bool ev_valid = false;
 };

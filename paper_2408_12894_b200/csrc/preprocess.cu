@@ -1,9 +1,11 @@
 // Steps a1-a4 of the hot path:
 //   k_geometry  a1 level selection (Eq. 6-7), a2 cull + view transform, a3 EWA projection, conic,
-//               tile rect; every visible Gaussian adds its rect to a 2-D difference grid of the tile counts
-//               (four integer atomics whatever the rect size) and appends its index to the unordered visible list;
-//   k_colour    a4 SH -> RGB over the visible list.
-// One thread per scanned Gaussian, no inter-block dependency: records are written in place at the scan index.
+//               tile rect.  A thread owns four consecutive Gaussians (16-byte loads from every SoA plane, all
+//               loads of a phase in flight together); the block stages the records of its visible Gaussians in shared
+//               memory and copies them out, in gid order, dense and coalesced, at the front of its own segment of
+//               the per-frame arrays (no inter-block scan: see WorkspaceDev).  Every visible Gaussian also adds its rect to a 2-D
+//               difference grid of the tile counts (four integer atomics whatever the rect size);
+//   k_colour    a4 SH -> RGB, one block per segment.
 //
 // The geometry (a1-a3 and the rect) is the canonical fp32 sequence of DESIGN §2: each operation is one IEEE
 // round-to-nearest binary32 operation (the *_rn intrinsics are never contracted into FMAs), in the written order.
@@ -55,96 +57,145 @@ __device__ __forceinline__ void sh_basis(float x, float y, float z, float *Y)
     }
 }
 
+// Shared staging of one block's records, slot = k * kGeoThreads + tid for Gaussian k of thread tid (conflict-free).
 template <bool DEBUG>
-__global__ void __launch_bounds__(kPreBlock)
+struct GeoSmem {
+    float4 a[kGeoBlock];                              // mu'x, mu'y, k, a2
+    float4 dg[kGeoBlock];                             // mu - c_cam, gid bits
+    float2 b[kGeoBlock];                              // d2, log2 o
+    uint2 rect[kGeoBlock];                            // tx0 | ty0 << 16, tx1 | ty1 << 16
+    uint32_t depth[kGeoBlock];
+    float4 conic_o[DEBUG ? kGeoBlock : 1];            // A, B, C, o (debug records only)
+    unsigned short map[kGeoBlock];                    // block-local compact position -> slot
+    unsigned int warp_vis[kGeoThreads / 32];
+    unsigned int cnt[2];                              // n_sel, n_front of the block
+    unsigned long long pairs;
+};
+
+template <bool DEBUG>
+__global__ void __launch_bounds__(kGeoThreads, 3)
 k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ FrameParams p)
 {
-    __shared__ unsigned int s_warp_vis[kPreBlock / 32];
-    __shared__ unsigned int s_base;
-    __shared__ unsigned int s_cnt[2];               // n_sel, n_front of the block
-    __shared__ unsigned long long s_pairs;
+    extern __shared__ __align__(16) unsigned char geo_smem_raw[];
+    GeoSmem<DEBUG> &S = *reinterpret_cast<GeoSmem<DEBUG> *>(geo_smem_raw);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) { s_cnt[0] = 0; s_cnt[1] = 0; s_pairs = 0; }
-    const int i = (int)(blockIdx.x * kPreBlock) + tid;
+    if (tid == 0) { S.cnt[0] = 0; S.cnt[1] = 0; S.pairs = 0; }
+    const int bid = blockIdx.x;
+    const long long g0 = p.quad_gid + ((long long)bid * kGeoThreads + tid) * kGeoPer;   // multiple of 4
+    const long long g_end = p.first_gid + p.n_scan;
 
-    bool vis = false, sel = false, front = false;
-    unsigned int n_tiles = 0;
-    float mx2 = 0, my2 = 0, pz = 0, cA = 0, cB = 0, cC = 0;
-    int tx0 = 0, ty0 = 0, tx1 = 0, ty1 = 0;
-    float wx = 0, wy = 0, wz = 0;                   // world-space mean (for the view direction)
-    long long g = 0;
-
-    if (i < p.n_scan) {
-        g = p.first_gid + i;
-        int lv = 0;
+    // ---- phase 1 loads: mean and kappa of the quad (16-byte loads; the planes are padded to 256 B)
+    float wx[4], wy[4], wz[4], kap[4];
+    const bool quad_live = g0 < g_end && g0 + kGeoPer > p.first_gid;
+    if (quad_live) {
+        const float4 X = __ldg(reinterpret_cast<const float4 *>(sc.mx + g0));
+        const float4 Y = __ldg(reinterpret_cast<const float4 *>(sc.my + g0));
+        const float4 Z = __ldg(reinterpret_cast<const float4 *>(sc.mz + g0));
+        const float4 K = __ldg(reinterpret_cast<const float4 *>(sc.kappa + g0));
+        wx[0] = X.x; wx[1] = X.y; wx[2] = X.z; wx[3] = X.w;
+        wy[0] = Y.x; wy[1] = Y.y; wy[2] = Y.z; wy[3] = Y.w;
+        wz[0] = Z.x; wz[1] = Z.y; wz[2] = Z.z; wz[3] = Z.w;
+        kap[0] = K.x; kap[1] = K.y; kap[2] = K.z; kap[3] = K.w;
+    }
+    const float *R = p.R;
+    unsigned int m_sel = 0, m_front = 0, m_proj = 0;       // bit k: Gaussian k selected / in front / to be projected
+    float px[4], py[4], pz[4];
+    if (quad_live) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const long long g = g0 + k;
+            if (g < p.first_gid || g >= g_end) continue;
+            const int i = (int)(g - p.first_gid);
+            int lv = 0;
 #pragma unroll 1
-        while (lv < p.n_levels - 1 && i >= p.level_end[lv]) ++lv;
-        wx = __ldg(sc.mx + g); wy = __ldg(sc.my + g); wz = __ldg(sc.mz + g);
-        // ---- a1 (O1): Eq. 6 predicate on squared Euclidean distance to the reference
-        {
-            float dx = fsub(wx, p.ref[0]), dy = fsub(wy, p.ref[1]), dz = fsub(wz, p.ref[2]);
-            float d2 = fadd(fadd(fmul(dx, dx), fmul(dy, dy)), fmul(dz, dz));
-            sel = (d2 >= p.lo2[lv]) && (d2 < p.hi2[lv]);
-        }
-        if (DEBUG) ws.mask[g] = sel ? 1 : 0;
-        if (sel) {
+            while (lv < p.n_levels - 1 && i >= p.level_end[lv]) ++lv;
+            // ---- a1 (O1): Eq. 6 predicate on squared Euclidean distance to the reference
+            const float dx = fsub(wx[k], p.ref[0]), dy = fsub(wy[k], p.ref[1]), dz = fsub(wz[k], p.ref[2]);
+            const float d2 = fadd(fadd(fmul(dx, dx), fmul(dy, dy)), fmul(dz, dz));
+            const bool sel = (d2 >= p.lo2[lv]) && (d2 < p.hi2[lv]);
+            if (DEBUG) ws.mask[g] = sel ? 1 : 0;
+            if (!sel) continue;
+            m_sel |= 1u << k;
             // ---- a2 (O2): p = R mu + t
-            const float *R = p.R;
-            float px = fadd(fadd(fadd(fmul(R[0], wx), fmul(R[1], wy)), fmul(R[2], wz)), p.t[0]);
-            float py = fadd(fadd(fadd(fmul(R[3], wx), fmul(R[4], wy)), fmul(R[5], wz)), p.t[1]);
-            pz = fadd(fadd(fadd(fmul(R[6], wx), fmul(R[7], wy)), fmul(R[8], wz)), p.t[2]);
-            front = pz > p.z_near;
-            float kap = front ? __ldg(sc.kappa + g) : -1.0f;
-            if (front && kap >= 0.0f) {
-                float ix = fdiv(px, pz), iy = fdiv(py, pz);
-                mx2 = fadd(fmul(p.fx, ix), p.cx);
-                my2 = fadd(fmul(p.fy, iy), p.cy);
-                // ---- a3 (O3): J at the clamped point, M = J R, Sigma' = M Sigma M^T + 0.3 I
-                float u = fminf(fmaxf(ix, -p.limx), p.limx);
-                float v = fminf(fmaxf(iy, -p.limy), p.limy);
-                float j00 = fdiv(p.fx, pz);
-                float j02 = -fdiv(fmul(p.fx, u), pz);
-                float j11 = fdiv(p.fy, pz);
-                float j12 = -fdiv(fmul(p.fy, v), pz);
-                float m00 = fadd(fmul(j00, R[0]), fmul(j02, R[6]));
-                float m01 = fadd(fmul(j00, R[1]), fmul(j02, R[7]));
-                float m02 = fadd(fmul(j00, R[2]), fmul(j02, R[8]));
-                float m10 = fadd(fmul(j11, R[3]), fmul(j12, R[6]));
-                float m11 = fadd(fmul(j11, R[4]), fmul(j12, R[7]));
-                float m12 = fadd(fmul(j11, R[5]), fmul(j12, R[8]));
-                float Sxx = __ldg(sc.cov[0] + g), Sxy = __ldg(sc.cov[1] + g), Sxz = __ldg(sc.cov[2] + g);
-                float Syy = __ldg(sc.cov[3] + g), Syz = __ldg(sc.cov[4] + g), Szz = __ldg(sc.cov[5] + g);
-                float v0x = fadd(fadd(fmul(Sxx, m00), fmul(Sxy, m01)), fmul(Sxz, m02));
-                float v0y = fadd(fadd(fmul(Sxy, m00), fmul(Syy, m01)), fmul(Syz, m02));
-                float v0z = fadd(fadd(fmul(Sxz, m00), fmul(Syz, m01)), fmul(Szz, m02));
-                float v1x = fadd(fadd(fmul(Sxx, m10), fmul(Sxy, m11)), fmul(Sxz, m12));
-                float v1y = fadd(fadd(fmul(Sxy, m10), fmul(Syy, m11)), fmul(Syz, m12));
-                float v1z = fadd(fadd(fmul(Sxz, m10), fmul(Syz, m11)), fmul(Szz, m12));
-                float a = fadd(fadd(fadd(fmul(m00, v0x), fmul(m01, v0y)), fmul(m02, v0z)), 0.3f);
-                float b = fadd(fadd(fmul(m10, v0x), fmul(m11, v0y)), fmul(m12, v0z));
-                float c = fadd(fadd(fadd(fmul(m10, v1x), fmul(m11, v1y)), fmul(m12, v1z)), 0.3f);
-                float det = fsub(fmul(a, c), fmul(b, b));
-                if (det > 0.0f) {
-                    cA = fdiv(c, det); cB = -fdiv(b, det); cC = fdiv(a, det);
-                    // ---- O4: padded box of the alpha = 1/255 contour, in 16x16 tiles
-                    float hx = fadd(fmul(__fsqrt_rn(fmul(kap, a)), 1.0009765625f), 0.015625f);
-                    float hy = fadd(fmul(__fsqrt_rn(fmul(kap, c)), 1.0009765625f), 0.015625f);
-                    float fTX = (float)p.TX, fTY = (float)p.TY;
-                    float x0 = fminf(fmaxf(floorf(fmul(fsub(mx2, hx), 0.0625f)), 0.0f), fTX);
-                    float x1 = fminf(fmaxf(fadd(floorf(fmul(fadd(mx2, hx), 0.0625f)), 1.0f), 0.0f), fTX);
-                    float y0 = fminf(fmaxf(floorf(fmul(fsub(my2, hy), 0.0625f)), 0.0f), fTY);
-                    float y1 = fminf(fmaxf(fadd(floorf(fmul(fadd(my2, hy), 0.0625f)), 1.0f), 0.0f), fTY);
-                    tx0 = (int)x0; tx1 = (int)x1; ty0 = (int)y0; ty1 = (int)y1;
-                    n_tiles = (unsigned int)((tx1 - tx0) * (ty1 - ty0));
-                    vis = n_tiles > 0;
-                }
-            }
+            px[k] = fadd(fadd(fadd(fmul(R[0], wx[k]), fmul(R[1], wy[k])), fmul(R[2], wz[k])), p.t[0]);
+            py[k] = fadd(fadd(fadd(fmul(R[3], wx[k]), fmul(R[4], wy[k])), fmul(R[5], wz[k])), p.t[1]);
+            pz[k] = fadd(fadd(fadd(fmul(R[6], wx[k]), fmul(R[7], wy[k])), fmul(R[8], wz[k])), p.t[2]);
+            if (!(pz[k] > p.z_near)) continue;
+            m_front |= 1u << k;
+            if (kap[k] >= 0.0f) m_proj |= 1u << k;           // kappa = -1 marks a dead Gaussian (o < 1/255)
         }
     }
 
-    // ---- per-visible records, in place at the scan index i
-    if (vis) {
+    // ---- phase 2 loads: the six covariance planes, only for quads with something to project
+    float4 S0, S1, S2, S3, S4, S5;
+    if (m_proj) {
+        S0 = __ldg(reinterpret_cast<const float4 *>(sc.cov[0] + g0));
+        S1 = __ldg(reinterpret_cast<const float4 *>(sc.cov[1] + g0));
+        S2 = __ldg(reinterpret_cast<const float4 *>(sc.cov[2] + g0));
+        S3 = __ldg(reinterpret_cast<const float4 *>(sc.cov[3] + g0));
+        S4 = __ldg(reinterpret_cast<const float4 *>(sc.cov[4] + g0));
+        S5 = __ldg(reinterpret_cast<const float4 *>(sc.cov[5] + g0));
+    }
+    float4 L2O = make_float4(0.f, 0.f, 0.f, 0.f), OP = L2O;
+    if (m_proj) {
+        L2O = __ldg(reinterpret_cast<const float4 *>(sc.l2o + g0));
+        if (DEBUG) OP = __ldg(reinterpret_cast<const float4 *>(sc.opacity + g0));
+    }
+
+    unsigned int m_vis = 0, my_pairs = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        if (!((m_proj >> k) & 1u)) continue;
+        const float Sxx = k == 0 ? S0.x : k == 1 ? S0.y : k == 2 ? S0.z : S0.w;
+        const float Sxy = k == 0 ? S1.x : k == 1 ? S1.y : k == 2 ? S1.z : S1.w;
+        const float Sxz = k == 0 ? S2.x : k == 1 ? S2.y : k == 2 ? S2.z : S2.w;
+        const float Syy = k == 0 ? S3.x : k == 1 ? S3.y : k == 2 ? S3.z : S3.w;
+        const float Syz = k == 0 ? S4.x : k == 1 ? S4.y : k == 2 ? S4.z : S4.w;
+        const float Szz = k == 0 ? S5.x : k == 1 ? S5.y : k == 2 ? S5.z : S5.w;
+        const float l2o = k == 0 ? L2O.x : k == 1 ? L2O.y : k == 2 ? L2O.z : L2O.w;
+        const float z = pz[k];
+        const float ix = fdiv(px[k], z), iy = fdiv(py[k], z);
+        const float mx2 = fadd(fmul(p.fx, ix), p.cx);
+        const float my2 = fadd(fmul(p.fy, iy), p.cy);
+        // ---- a3 (O3): J at the clamped point, M = J R, Sigma' = M Sigma M^T + 0.3 I
+        const float u = fminf(fmaxf(ix, -p.limx), p.limx);
+        const float v = fminf(fmaxf(iy, -p.limy), p.limy);
+        const float j00 = fdiv(p.fx, z);
+        const float j02 = -fdiv(fmul(p.fx, u), z);
+        const float j11 = fdiv(p.fy, z);
+        const float j12 = -fdiv(fmul(p.fy, v), z);
+        const float m00 = fadd(fmul(j00, R[0]), fmul(j02, R[6]));
+        const float m01 = fadd(fmul(j00, R[1]), fmul(j02, R[7]));
+        const float m02 = fadd(fmul(j00, R[2]), fmul(j02, R[8]));
+        const float m10 = fadd(fmul(j11, R[3]), fmul(j12, R[6]));
+        const float m11 = fadd(fmul(j11, R[4]), fmul(j12, R[7]));
+        const float m12 = fadd(fmul(j11, R[5]), fmul(j12, R[8]));
+        const float v0x = fadd(fadd(fmul(Sxx, m00), fmul(Sxy, m01)), fmul(Sxz, m02));
+        const float v0y = fadd(fadd(fmul(Sxy, m00), fmul(Syy, m01)), fmul(Syz, m02));
+        const float v0z = fadd(fadd(fmul(Sxz, m00), fmul(Syz, m01)), fmul(Szz, m02));
+        const float v1x = fadd(fadd(fmul(Sxx, m10), fmul(Sxy, m11)), fmul(Sxz, m12));
+        const float v1y = fadd(fadd(fmul(Sxy, m10), fmul(Syy, m11)), fmul(Syz, m12));
+        const float v1z = fadd(fadd(fmul(Sxz, m10), fmul(Syz, m11)), fmul(Szz, m12));
+        const float a = fadd(fadd(fadd(fmul(m00, v0x), fmul(m01, v0y)), fmul(m02, v0z)), 0.3f);
+        const float b = fadd(fadd(fmul(m10, v0x), fmul(m11, v0y)), fmul(m12, v0z));
+        const float c = fadd(fadd(fadd(fmul(m10, v1x), fmul(m11, v1y)), fmul(m12, v1z)), 0.3f);
+        const float det = fsub(fmul(a, c), fmul(b, b));
+        if (!(det > 0.0f)) continue;
+        const float cA = fdiv(c, det), cB = -fdiv(b, det), cC = fdiv(a, det);
+        // ---- O4: padded box of the alpha = 1/255 contour, in 16x16 tiles
+        const float hx = fadd(fmul(__fsqrt_rn(fmul(kap[k], a)), 1.0009765625f), 0.015625f);
+        const float hy = fadd(fmul(__fsqrt_rn(fmul(kap[k], c)), 1.0009765625f), 0.015625f);
+        const float fTX = (float)p.TX, fTY = (float)p.TY;
+        const float x0 = fminf(fmaxf(floorf(fmul(fsub(mx2, hx), 0.0625f)), 0.0f), fTX);
+        const float x1 = fminf(fmaxf(fadd(floorf(fmul(fadd(mx2, hx), 0.0625f)), 1.0f), 0.0f), fTX);
+        const float y0 = fminf(fmaxf(floorf(fmul(fsub(my2, hy), 0.0625f)), 0.0f), fTY);
+        const float y1 = fminf(fmaxf(fadd(floorf(fmul(fadd(my2, hy), 0.0625f)), 1.0f), 0.0f), fTY);
+        const int tx0 = (int)x0, tx1 = (int)x1, ty0 = (int)y0, ty1 = (int)y1;
+        const unsigned int n_tiles = (unsigned int)((tx1 - tx0) * (ty1 - ty0));
+        if (n_tiles == 0) continue;
+        m_vis |= 1u << k;
+        my_pairs += n_tiles;
         // DESIGN R25: factorised exponent from the ROUNDED conic, derived in fp64, rounded once
         const double LOG2E = 1.4426950408889634;
         const double dA = (double)cA, dB = (double)cB, dC = (double)cC;
@@ -153,11 +204,14 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
         // <= 0 so that q >= 0 holds by construction in k_blend (the oracle clamps q at 0; a conic left indefinite by
         // rounding differs from its clamp by less than R25's evaluation error)
         const float d2 = fminf((float)(-0.5 * LOG2E * (dC - dB * dB / dA)), 0.0f);
-        ws.gA[i] = make_float4(mx2, my2, kk, a2);
-        reinterpret_cast<float2 *>(ws.gB)[2 * (size_t)i] = make_float2(d2, __ldg(sc.l2o + g));   // (r, g) by k_colour
-        ws.rect[i] = make_ushort4((unsigned short)tx0, (unsigned short)ty0, (unsigned short)tx1, (unsigned short)ty1);
-        ws.depth[i] = __float_as_uint(pz);
-        ws.dirgid[i] = make_float4(wx - p.centre[0], wy - p.centre[1], wz - p.centre[2], __uint_as_float((unsigned int)g));
+        const int slot = k * kGeoThreads + tid;
+        S.a[slot] = make_float4(mx2, my2, kk, a2);
+        S.b[slot] = make_float2(d2, l2o);
+        S.rect[slot] = make_uint2((unsigned int)tx0 | ((unsigned int)ty0 << 16), (unsigned int)tx1 | ((unsigned int)ty1 << 16));
+        S.depth[slot] = __float_as_uint(z);
+        S.dg[slot] = make_float4(wx[k] - p.centre[0], wy[k] - p.centre[1], wz[k] - p.centre[2],
+                                 __uint_as_float((unsigned int)(g0 + k)));
+        if (DEBUG) S.conic_o[slot] = make_float4(cA, cB, cC, k == 0 ? OP.x : k == 1 ? OP.y : k == 2 ? OP.z : OP.w);
         // a5, first half: +1 over the rect in the 2-D difference grid of the per-tile pair counts
         const int gw = p.TX + 1;
         atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx0) * kCtrStride, 1);
@@ -165,40 +219,71 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
         atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx0) * kCtrStride, -1);
         atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx1) * kCtrStride, 1);
     }
-    if (DEBUG && i < p.n_scan) {
-        flod_dbg_projected d;
-        d.gid = vis ? (uint32_t)g : 0xffffffffu; d.mu2d[0] = mx2; d.mu2d[1] = my2; d.depth = pz;
-        d.conic[0] = cA; d.conic[1] = cB; d.conic[2] = cC; d.opacity = vis ? __ldg(sc.opacity + g) : 0.0f;
-        d.rgb[0] = 0.0f; d.rgb[1] = 0.0f; d.rgb[2] = 0.0f;                                    // by k_colour
-        d.rect[0] = tx0; d.rect[1] = ty0; d.rect[2] = tx1; d.rect[3] = ty1;
-        ws.dbg[i] = d;
-    }
 
-    // ---- block-aggregated counters and the unordered visible list
-    const unsigned int bv = __ballot_sync(0xffffffffu, vis);
-    const unsigned int bs = __ballot_sync(0xffffffffu, sel), bf = __ballot_sync(0xffffffffu, front);
-    unsigned int wp = n_tiles;                       // warp sum of the tile counts (a rect has < 2^20 tiles)
+    // ---- block scan of the visible counts (gid order = thread order, then k), block totals of the statistics
+    const unsigned int nv = __popc(m_vis);
+    unsigned int incl = nv;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) wp += __shfl_xor_sync(0xffffffffu, wp, o);
-    __syncthreads();                                 // s_cnt / s_pairs were zeroed by thread 0
-    if (lane == 0) {
-        s_warp_vis[warp] = __popc(bv);
-        if (bs) atomicAdd(&s_cnt[0], __popc(bs));
-        if (bf) atomicAdd(&s_cnt[1], __popc(bf));
-        if (wp) atomicAdd(&s_pairs, (unsigned long long)wp);
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
     }
+    unsigned int ws_sel = __popc(m_sel), ws_front = __popc(m_front), ws_pairs = my_pairs;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        ws_sel += __shfl_xor_sync(0xffffffffu, ws_sel, o);
+        ws_front += __shfl_xor_sync(0xffffffffu, ws_front, o);
+        ws_pairs += __shfl_xor_sync(0xffffffffu, ws_pairs, o);
+    }
+    if (lane == 31) S.warp_vis[warp] = incl;
+    __syncthreads();                                     // S.cnt / S.pairs were zeroed by thread 0
+    if (lane == 0) {
+        if (ws_sel) atomicAdd(&S.cnt[0], ws_sel);
+        if (ws_front) atomicAdd(&S.cnt[1], ws_front);
+        if (ws_pairs) atomicAdd(&S.pairs, (unsigned long long)ws_pairs);
+    }
+    __syncthreads();
+    unsigned int local = incl - nv;                      // block-local compact position of the thread's first visible
+#pragma unroll
+    for (int w = 0; w < kGeoThreads / 32; ++w) if (w < warp) local += S.warp_vis[w];
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        if ((m_vis >> k) & 1u) S.map[local++] = (unsigned short)(k * kGeoThreads + tid);
+    unsigned int total = 0;
+#pragma unroll
+    for (int w = 0; w < kGeoThreads / 32; ++w) total += S.warp_vis[w];
     __syncthreads();
     if (tid == 0) {
-        unsigned int tot = 0;
-#pragma unroll
-        for (int w = 0; w < kPreBlock / 32; ++w) { const unsigned int t = s_warp_vis[w]; s_warp_vis[w] = tot; tot += t; }
-        s_base = tot ? atomicAdd(&ws.hdr->n_vis32, tot) : 0u;
-        if (s_cnt[0]) atomicAdd(&ws.hdr->n_sel, (unsigned long long)s_cnt[0]);
-        if (s_cnt[1]) atomicAdd(&ws.hdr->n_front, (unsigned long long)s_cnt[1]);
-        if (s_pairs) atomicAdd(&ws.hdr->n_pairs, s_pairs);
+        ws.seg_count[bid] = total;
+        if (total) atomicAdd(&ws.hdr->n_vis32, total);
+        if (S.cnt[0]) atomicAdd(&ws.hdr->n_sel, (unsigned long long)S.cnt[0]);
+        if (S.cnt[1]) atomicAdd(&ws.hdr->n_front, (unsigned long long)S.cnt[1]);
+        if (S.pairs) atomicAdd(&ws.hdr->n_pairs, S.pairs);
     }
-    __syncthreads();
-    if (vis) ws.vis_list[s_base + s_warp_vis[warp] + __popc(bv & ((1u << lane) - 1))] = (uint32_t)i;
+
+    // ---- copy-out: the block's visible records, dense and coalesced, at the front of the block's segment
+    const unsigned int base = (unsigned int)bid * kGeoBlock;
+    for (unsigned int j = tid; j < total; j += kGeoThreads) {
+        const int slot = S.map[j];
+        const size_t c = (size_t)base + j;
+        ws.gA[c] = S.a[slot];
+        reinterpret_cast<float2 *>(ws.gB)[2 * c] = S.b[slot];          // (r, g) by k_colour
+        const uint2 rc = S.rect[slot];
+        ws.rect[c] = make_ushort4((unsigned short)(rc.x & 0xffffu), (unsigned short)(rc.x >> 16),
+                                  (unsigned short)(rc.y & 0xffffu), (unsigned short)(rc.y >> 16));
+        ws.depth[c] = S.depth[slot];
+        ws.dirgid[c] = S.dg[slot];
+        if (DEBUG) {
+            const float4 a = S.a[slot], co = S.conic_o[slot];
+            flod_dbg_projected d;
+            d.gid = __float_as_uint(S.dg[slot].w); d.mu2d[0] = a.x; d.mu2d[1] = a.y; d.depth = __uint_as_float(S.depth[slot]);
+            d.conic[0] = co.x; d.conic[1] = co.y; d.conic[2] = co.z; d.opacity = co.w;
+            d.rgb[0] = 0.0f; d.rgb[1] = 0.0f; d.rgb[2] = 0.0f;                                // by k_colour
+            d.rect[0] = (int)(rc.x & 0xffffu); d.rect[1] = (int)(rc.x >> 16);
+            d.rect[2] = (int)(rc.y & 0xffffu); d.rect[3] = (int)(rc.y >> 16);
+            ws.dbg[c] = d;
+        }
+    }
 }
 
 // ---- a4: colour of every visible Gaussian.  rgb = max(0, 0.5 + sum_k Y_k(dir) sh_k)  (R16)
@@ -210,16 +295,18 @@ __global__ void __launch_bounds__(256)
 k_colour(const SceneDev sc, const WorkspaceDev ws)
 {
     constexpr int K = (DEG + 1) * (DEG + 1);
-    const unsigned int n_vis = ws.hdr->n_vis32;
     const unsigned int sub = threadIdx.x % LANES;
     const unsigned int per_block = 256 / LANES;
-    for (unsigned int base = blockIdx.x * per_block; base < n_vis; base += gridDim.x * per_block) {
-        const unsigned int slot = base + threadIdx.x / LANES;
-        const bool ok = slot < n_vis;
+    const unsigned int seg = blockIdx.x;                 // one block per segment of k_geometry
+    const unsigned int n_here = ws.seg_count[seg];
+    for (unsigned int j0 = 0; j0 < n_here; j0 += per_block) {
+        const unsigned int j = j0 + threadIdx.x / LANES;
+        const bool ok = j < n_here;
+        const unsigned int slot = seg * kGeoBlock + j;
         float r = 0.0f, g = 0.0f, b = 0.0f;
         unsigned int ci = 0;
         if (ok) {
-            ci = ws.vis_list[slot];
+            ci = slot;
             const float4 dg = ws.dirgid[ci];
             const float *row = sc.sh + (size_t)__float_as_uint(dg.w) * sc.sh_stride;
             float Y[K];
@@ -274,8 +361,14 @@ k_colour(const SceneDev sc, const WorkspaceDev ws)
 int launch_geometry(const Context &c, const FrameParams &p, cudaStream_t s)
 {
     if (p.n_pre_blocks <= 0) return 0;
-    if (c.flags & FLOD_OPT_DEBUG) k_geometry<true><<<p.n_pre_blocks, kPreBlock, 0, s>>>(c.scene, c.ws, p);
-    else k_geometry<false><<<p.n_pre_blocks, kPreBlock, 0, s>>>(c.scene, c.ws, p);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_geometry<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GeoSmem<true>));
+        cudaFuncSetAttribute(k_geometry<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GeoSmem<false>));
+        attr_set = true;
+    }
+    if (c.flags & FLOD_OPT_DEBUG) k_geometry<true><<<p.n_pre_blocks, kGeoThreads, sizeof(GeoSmem<true>), s>>>(c.scene, c.ws, p);
+    else k_geometry<false><<<p.n_pre_blocks, kGeoThreads, sizeof(GeoSmem<false>), s>>>(c.scene, c.ws, p);
     return 1;
 }
 
@@ -289,7 +382,7 @@ static void launch_colour_t(const Context &c, int grid, cudaStream_t s)
 int launch_colour(const Context &c, const FrameParams &p, cudaStream_t s)
 {
     if (p.n_pre_blocks <= 0) return 0;
-    const int grid = c.sm_count * 8;
+    const int grid = p.n_pre_blocks;
     switch (c.sh_degree) {
         case 0: launch_colour_t<0, 1>(c, grid, s); break;
         case 1: launch_colour_t<1, 1>(c, grid, s); break;

@@ -1,12 +1,12 @@
 // Step a7: every tile's pair list into (depth, gid) order ("in depth order"; R15).
 //
-// One CTA per tile.  The list holds unique 64-bit keys (depth bits << 32) | scan index, in the arbitrary order in
+// One CTA per tile.  The list holds unique 64-bit keys (depth bits << 32) | compact index, in the arbitrary order in
 // which k_duplicate's atomics were served.  It is sorted most-significant-digit first, without any stable ranking:
 //   bin pass   min / max of the keys -> bins of power-of-two width over [kmin, kmax] (at most 2048, about one key
 //              per bin) -> histogram with shared-memory atomics -> exclusive scan -> scatter with a second atomic.
 //              Bins are now in key order, keys inside a bin are not.
 //   rank pass  one thread per key counts the keys of its own bin that are smaller (a bin holds a few keys): that is
-//              its final position.  The 32-bit scan index is written to ws.vals.
+//              its final position.  The 32-bit compact index is written to ws.vals.
 // A bin with more than kRankMax keys (a cluster of nearly equal depths) is binned once more over its own key range
 // (level 2, through global memory); what is still oversized after that is ranked by the whole block.
 // Lists of up to kSortCap keys are scattered into shared memory, longer ones into ws.pairs_tmp (global, L2).
@@ -103,7 +103,7 @@ __device__ BinMap bin_pass(const u64 *src, u64 *dst, unsigned int n, unsigned in
 }
 
 // Final positions of the keys that sit in bins of at most kRankMax keys: position = bin start + number of smaller
-// keys in the bin.  buf[0, n) is the output of bin_pass; the scan indices go to out[0, n).
+// keys in the bin.  buf[0, n) is the output of bin_pass; the compact indices go to out[0, n).
 __device__ __forceinline__ void rank_small(const u64 *buf, unsigned int n, const unsigned int *ends, const BinMap &m,
                                            uint32_t *__restrict__ out, int tid)
 {
