@@ -35,11 +35,11 @@ extern "C" {
 #define FLOD_API
 #endif
 
-#define FLOD_ABI_VERSION 2
+#define FLOD_ABI_VERSION 3
 #define FLOD_MAX_LEVELS 16
 #define FLOD_TILE 16                 /* tiles are 16x16 pixels */
-#define FLOD_N_STAGES 6              /* 0 geometry (a1-a3), 1 tile scan (a5, a8), 2 colour (a4), 3 duplication (a6),
-                                        4 per-tile sort (a7), 5 blend (a9) */
+#define FLOD_N_STAGES 5              /* 0 geometry (a1-a3), 1 colour (a4) with the tile scan (a5, a8) in one of its blocks,
+                                        2 duplication (a6), 3 per-tile sort (a7), 4 blend (a9) */
 
 enum {
     FLOD_OK = 0,
@@ -152,10 +152,21 @@ FLOD_API int flod_set_options(flod_ctx *ctx, unsigned flags);
 FLOD_API int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma,
                 float *out_rgb_dev, void *stream);
 
-/* Same, end to end with HOST buffers: renders into the workspace's image and copies it to out_rgb_host
- * ([3][height][width] fp32, ideally pinned) on `stream`, then waits for the stream. */
+/* Same, end to end with HOST buffers: renders into an image of the workspace and copies it to out_rgb_host
+ * ([3][height][width] fp32, ideally pinned) on `stream`, then waits for the copy. */
 FLOD_API int flod_render_to_host(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma,
                         float *out_rgb_host, void *stream);
+
+/* Pipelined form of flod_render_to_host for frame sequences.  The kernels run on `stream`, the device-to-host copy
+ * on `copy_stream` (both caller-owned cudaStream_t; pass two different streams to overlap the copy of frame k with
+ * the kernels of frame k+1 -- the workspace holds two images and the library orders the two streams with its own
+ * events).  Returns without waiting: out_rgb_host (pinned) must stay valid and must not be read before
+ * flod_wait_host returns; give consecutive frames different host buffers if every frame is to be kept. */
+FLOD_API int flod_render_to_host_async(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma,
+                              float *out_rgb_host, void *stream, void *copy_stream);
+
+/* Blocks the calling host thread until every copy issued by flod_render_to_host_async has landed. */
+FLOD_API int flod_wait_host(flod_ctx *ctx);
 
 /* Waits for the last frame's stream, then reports its counters (and FLOD_E_CAPACITY if it overflowed). */
 FLOD_API int flod_get_stats(flod_ctx *ctx, flod_stats *out);

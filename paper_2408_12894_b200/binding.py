@@ -18,8 +18,8 @@ HEADER = os.path.join(HERE, "..", "include", "flod.h")
 
 FLOD_OPT_DEBUG, FLOD_OPT_PROFILE, FLOD_OPT_COUNT = 1, 2, 4
 FLOD_DBG_MASK, FLOD_DBG_TILE_COUNTS, FLOD_DBG_PROJECTED, FLOD_DBG_SORTED_PAIRS, FLOD_DBG_ACTIVATED = range(5)
-FLOD_N_STAGES = 6
-STAGE_NAMES = ("geometry", "tile_scan", "colour", "duplicate", "tile_sort", "blend")
+FLOD_N_STAGES = 5
+STAGE_NAMES = ("geometry", "colour", "duplicate", "tile_sort", "blend")
 ERRORS = {-1: "FLOD_E_INVALID_ARG", -2: "FLOD_E_LEVEL_RANGE", -3: "FLOD_E_NOT_UPLOADED",
           -4: "FLOD_E_ARENA_TOO_SMALL", -5: "FLOD_E_CAPACITY", -6: "FLOD_E_CUDA", -7: "FLOD_E_NO_WORKSPACE"}
 
@@ -90,6 +90,8 @@ def load_library():
     L.flod_set_options.argtypes = [vp, C.c_uint]
     L.flod_render.argtypes = [vp, C.POINTER(CameraStruct), LevelMode, C.c_float, vp, vp]
     L.flod_render_to_host.argtypes = [vp, C.POINTER(CameraStruct), LevelMode, C.c_float, vp, vp]
+    L.flod_render_to_host_async.argtypes = [vp, C.POINTER(CameraStruct), LevelMode, C.c_float, vp, vp, vp]
+    L.flod_wait_host.argtypes = [vp]
     L.flod_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.flod_debug_copy.argtypes = [vp, C.c_int, vp, sz]
     L.flod_launches_per_frame.argtypes = [vp]
@@ -210,6 +212,17 @@ class Renderer:
         self._check(self.lib.flod_render_to_host(self._h, C.byref(cs), LevelMode(l_start, l_end), float(gamma),
                                                  C.c_void_p(out_host.data_ptr()), self._stream()))
         return out_host
+
+    # ---- flod_render_to_host_async / flod_wait_host: kernels on the current stream, copy on `copy_stream`
+    def render_to_host_async(self, cam, l_start: int, l_end: int, gamma: float, out_host, copy_stream):
+        cs = cam if isinstance(cam, CameraStruct) else camera_struct(cam)
+        self._check(self.lib.flod_render_to_host_async(self._h, C.byref(cs), LevelMode(l_start, l_end), float(gamma),
+                                                       C.c_void_p(out_host.data_ptr()), self._stream(),
+                                                       C.c_void_p(copy_stream.cuda_stream)))
+        return out_host
+
+    def wait_host(self):
+        self._check(self.lib.flod_wait_host(self._h))
 
     def launches_per_frame(self) -> int:
         return self.lib.flod_launches_per_frame(self._h)

@@ -103,7 +103,7 @@ WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_p
     L.ws.seg_count = (unsigned int *)take((nt / kGeoBlock + 2) * sizeof(unsigned int));
     L.ws.tile_cnt = (int *)take((tx + 1) * (ty + 1) * sizeof(int));
     L.ws.ranges = (uint2 *)take(tiles * sizeof(uint2));
-    L.ws.cursor = (unsigned int *)take(tiles * kCtrStride * sizeof(unsigned int));
+    L.ws.cursor4 = (float *)take(((tx + 1) / 2) * ((ty + 1) / 2) * kCtrStride * sizeof(float));
     L.ws.gA = (float4 *)take(nt * sizeof(float4));
     L.ws.gB = (float4 *)take(nt * sizeof(float4));
     L.ws.cB = (float *)take(nt * sizeof(float));
@@ -115,7 +115,8 @@ WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_p
     L.ws.pairs = (unsigned long long *)take((size_t)max_pairs * 8);
     L.ws.pairs_tmp = (unsigned long long *)take((size_t)max_pairs * 8);
     L.ws.vals = (uint32_t *)take((size_t)max_pairs * 4);
-    L.ws.image = (float *)take((size_t)3 * w * h * sizeof(float));
+    L.ws.image[0] = (float *)take((size_t)3 * w * h * sizeof(float));
+    L.ws.image[1] = (float *)take((size_t)3 * w * h * sizeof(float));
     L.bytes = off;
     return L;
 }
@@ -143,6 +144,10 @@ int flod_create(flod_ctx **out, int device)
         return FLOD_E_CUDA;
     }
     for (auto &ev : c->ev) cudaEventCreate(&ev);
+    for (int i = 0; i < 2; ++i) {
+        cudaEventCreateWithFlags(&c->ev_rendered[i], cudaEventDisableTiming);
+        cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming);
+    }
     *out = c;
     return FLOD_OK;
 }
@@ -151,6 +156,10 @@ int flod_destroy(flod_ctx *ctx)
 {
     if (!ctx) return FLOD_E_INVALID_ARG;
     for (auto &ev : ctx->ev) if (ev) cudaEventDestroy(ev);
+    for (int i = 0; i < 2; ++i) {
+        if (ctx->ev_rendered[i]) cudaEventDestroy(ctx->ev_rendered[i]);
+        if (ctx->ev_copied[i]) cudaEventDestroy(ctx->ev_copied[i]);
+    }
     delete ctx;
     return FLOD_OK;
 }
@@ -280,6 +289,9 @@ int flod_set_workspace(flod_ctx *ctx, void *workspace_dev, size_t bytes, int wid
     WsLayout L = carve((unsigned char *)workspace_dev, ctx->n_total, width, height, max_pairs);
     ctx->ws = L.ws;
     ctx->ws_w = width; ctx->ws_h = height; ctx->max_pairs = max_pairs;
+    for (int i = 0; i < 2; ++i)
+        if (ctx->copy_pending[i]) { cudaEventSynchronize(ctx->ev_copied[i]); ctx->copy_pending[i] = false; }
+    ctx->img_turn = 0;
     ctx->has_ws = true; ctx->rendered = false;
     return FLOD_OK;
 }
@@ -305,7 +317,7 @@ int flod_set_options(flod_ctx *ctx, unsigned flags)
 int flod_launches_per_frame(const flod_ctx *ctx)
 {
     if (!ctx || !ctx->has_ws) return 0;
-    return 6;   // geometry, tile scan, colour, duplication, tile sort, blend
+    return 5;   // geometry, colour (+ tile scan in its block 0), duplication, tile sort, blend
 }
 
 int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, float *out_rgb_dev, void *stream)
@@ -371,7 +383,6 @@ int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, flo
     int stage = 0;
     auto mark = [&]() { if (prof) cudaEventRecord(ctx->ev[stage], s); ++stage; };
     mark(); launch_geometry(*ctx, p, s);
-    mark(); launch_tile_scan(*ctx, p, s);
     mark(); launch_colour(*ctx, p, s);
     mark(); launch_duplicate(*ctx, p, s);
     mark(); launch_tile_sort(*ctx, p, s);
@@ -385,18 +396,43 @@ int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, flo
     return FLOD_OK;
 }
 
-int flod_render_to_host(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, float *out_rgb_host, void *stream)
+int flod_render_to_host_async(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, float *out_rgb_host,
+                              void *stream, void *copy_stream)
 {
     if (!ctx) return FLOD_E_INVALID_ARG;
     if (!out_rgb_host) return fail(ctx, FLOD_E_INVALID_ARG, "render_to_host: null pointer");
     if (!ctx->has_ws) return fail(ctx, FLOD_E_NO_WORKSPACE, "render_to_host: no workspace set");
-    int rc = flod_render(ctx, cam, mode, gamma, ctx->ws.image, stream);
+    cudaStream_t s = (cudaStream_t)stream, cs = (cudaStream_t)copy_stream;
+    const int i = ctx->img_turn;
+    // image[i] may still be on its way out (frame k - 2): the kernels of this frame wait for that copy only
+    if (ctx->copy_pending[i]) CUDA_TRY(ctx, cudaStreamWaitEvent(s, ctx->ev_copied[i], 0));
+    int rc = flod_render(ctx, cam, mode, gamma, ctx->ws.image[i], stream);
     if (rc != FLOD_OK) return rc;
-    cudaStream_t s = (cudaStream_t)stream;
-    CUDA_TRY(ctx, cudaMemcpyAsync(out_rgb_host, ctx->ws.image, (size_t)3 * cam->width * cam->height * sizeof(float),
-                                  cudaMemcpyDeviceToHost, s));
-    CUDA_TRY(ctx, cudaStreamSynchronize(s));
+    CUDA_TRY(ctx, cudaEventRecord(ctx->ev_rendered[i], s));
+    CUDA_TRY(ctx, cudaStreamWaitEvent(cs, ctx->ev_rendered[i], 0));
+    CUDA_TRY(ctx, cudaMemcpyAsync(out_rgb_host, ctx->ws.image[i], (size_t)3 * cam->width * cam->height * sizeof(float),
+                                  cudaMemcpyDeviceToHost, cs));
+    CUDA_TRY(ctx, cudaEventRecord(ctx->ev_copied[i], cs));
+    ctx->copy_pending[i] = true;
+    ctx->last_copy_stream = cs;
+    ctx->img_turn = i ^ 1;
     return FLOD_OK;
+}
+
+int flod_wait_host(flod_ctx *ctx)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    for (int i = 0; i < 2; ++i)
+        if (ctx->copy_pending[i]) { CUDA_TRY(ctx, cudaEventSynchronize(ctx->ev_copied[i])); ctx->copy_pending[i] = false; }
+    return FLOD_OK;
+}
+
+int flod_render_to_host(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, float *out_rgb_host, void *stream)
+{
+    int rc = flod_render_to_host_async(ctx, cam, mode, gamma, out_rgb_host, stream, stream);
+    if (rc != FLOD_OK) return rc;
+    return flod_wait_host(ctx);
 }
 
 int flod_get_stats(flod_ctx *ctx, flod_stats *out)

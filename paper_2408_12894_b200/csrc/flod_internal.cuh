@@ -17,7 +17,10 @@ constexpr int kGeoThreads = 256;          // geometry: threads per block, four c
 constexpr int kGeoPer = 4;
 constexpr int kGeoBlock = kGeoThreads * kGeoPer;
 constexpr int kSortCap = 4096;            // per-tile sort: lists up to this many keys are scattered into shared memory
-constexpr int kCtrStride = 64;            // ints between two per-tile atomic counters: one counter per 256 B, so that the
+#ifndef FLOD_CTR_STRIDE
+#define FLOD_CTR_STRIDE 64
+#endif
+constexpr int kCtrStride = FLOD_CTR_STRIDE;            // ints between two per-tile atomic counters: one counter per 256 B, so that the
                                           // L2 slices share the atomic traffic (a dense 16 KB grid sits on a few slices)
 
 // Scene planes in the caller's arena (SoA, one plane per attribute, gid order = levels concatenated).
@@ -53,7 +56,8 @@ struct WorkspaceDev {
     unsigned int *seg_count;              // [geometry blocks] visible Gaussians of every segment
     int *tile_cnt;                        // [(TX+1)*(TY+1)] dense copy, used by the tile scan when the grid exceeds shared memory
     uint2 *ranges;                        // [T_n] (start, end) of every tile's pair list
-    unsigned int *cursor;                 // [T_n][kCtrStride] next free slot of every tile's list during duplication
+    float *cursor4;                       // [ceil(TX/2) * ceil(TY/2)][kCtrStride] first 4 floats: entries appended so far to the
+                                          // lists of the 2x2 tile group (x, y), (x+1, y), (x, y+1), (x+1, y+1); zeroed by the tile scan
     float4 *gA, *gB;                      // [n_total + 2 kGeoBlock]
     float *cB;                            // [n_total + 2 kGeoBlock]
     float4 *dirgid;                       // [n_total + 2 kGeoBlock] (mu - c_cam, gid bits): input of the colour kernel
@@ -64,7 +68,8 @@ struct WorkspaceDev {
     unsigned long long *pairs;            // [max_pairs] (depth bits << 32) | position, grouped by tile, unsorted
     unsigned long long *pairs_tmp;        // [max_pairs] scatter target of the per-tile sort for lists longer than kSortCap
     uint32_t *vals;                       // [max_pairs] positions, grouped by tile, sorted by (depth, gid)
-    float *image;                         // [3][H][W] for flod_render_to_host
+    float *image[2];                      // 2 x [3][H][W] for flod_render_to_host(_async): double-buffered so that the copy
+                                          // of frame k overlaps the kernels of frame k + 1
 };
 
 struct FrameParams {
@@ -115,13 +120,17 @@ struct Context {
     int64_t last_n_scan = 0;
     int last_n_segs = 0;
     cudaEvent_t ev[FLOD_N_STAGES + 1] = {nullptr};
+    cudaEvent_t ev_rendered[2] = {nullptr, nullptr};   // image[i] complete on the render stream
+    cudaEvent_t ev_copied[2] = {nullptr, nullptr};     // image[i] copied out on the copy stream (free to overwrite)
+    bool copy_pending[2] = {false, false};
+    int img_turn = 0;
+    cudaStream_t last_copy_stream = nullptr;
     bool ev_valid = false;
 };
 
 // kernel launchers (each enqueues on `s` and returns the number of kernels launched)
 int launch_geometry(const Context &c, const FrameParams &p, cudaStream_t s);    // a1-a3 + tile-count grid + visible list
-int launch_tile_scan(const Context &c, const FrameParams &p, cudaStream_t s);   // a5 (+ a8: ranges fall out of the scan)
-int launch_colour(const Context &c, const FrameParams &p, cudaStream_t s);      // a4
+int launch_colour(const Context &c, const FrameParams &p, cudaStream_t s);      // a4, and a5 + a8 (tile scan) in block 0
 int launch_duplicate(const Context &c, const FrameParams &p, cudaStream_t s);   // a6
 int launch_tile_sort(const Context &c, const FrameParams &p, cudaStream_t s);   // a7
 int launch_blend(const Context &c, const FrameParams &p, float *out_rgb, cudaStream_t s);   // a9

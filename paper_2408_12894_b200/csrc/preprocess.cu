@@ -5,11 +5,12 @@
 //               memory and copies them out, in gid order, dense and coalesced, at the front of its own segment of
 //               the per-frame arrays (no inter-block scan: see WorkspaceDev).  Every visible Gaussian also adds its rect to a 2-D
 //               difference grid of the tile counts (four integer atomics whatever the rect size);
-//   k_colour    a4 SH -> RGB, one block per segment.
+//   k_colour    a4 SH -> RGB, one block per segment; its block 0 runs the tile scan (a5 + a8, tile_scan.cuh).
 //
 // The geometry (a1-a3 and the rect) is the canonical fp32 sequence of DESIGN §2: each operation is one IEEE
 // round-to-nearest binary32 operation (the *_rn intrinsics are never contracted into FMAs), in the written order.
 #include "flod_internal.cuh"
+#include "tile_scan.cuh"
 
 namespace flod {
 
@@ -213,11 +214,13 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
                                  __uint_as_float((unsigned int)(g0 + k)));
         if (DEBUG) S.conic_o[slot] = make_float4(cA, cB, cC, k == 0 ? OP.x : k == 1 ? OP.y : k == 2 ? OP.z : OP.w);
         // a5, first half: +1 over the rect in the 2-D difference grid of the per-tile pair counts
+#ifndef FLOD_X_NO_GEO_ATOMICS
         const int gw = p.TX + 1;
         atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx0) * kCtrStride, 1);
         atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx1) * kCtrStride, -1);
         atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx0) * kCtrStride, -1);
         atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx1) * kCtrStride, 1);
+#endif
     }
 
     // ---- block scan of the visible counts (gid order = thread order, then k), block totals of the statistics
@@ -292,12 +295,13 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
 // coefficients k = 4 j .. 4 j + 3, so one load instruction of the 4 lanes reads 64 contiguous bytes.
 template <int DEG, int LANES, bool DEBUG>
 __global__ void __launch_bounds__(256)
-k_colour(const SceneDev sc, const WorkspaceDev ws)
+k_colour(const SceneDev sc, const WorkspaceDev ws, int TX, int TY, unsigned int max_pairs)
 {
     constexpr int K = (DEG + 1) * (DEG + 1);
+    if (blockIdx.x == 0) { tile_scan_block(ws, TX, TY, max_pairs); return; }
     const unsigned int sub = threadIdx.x % LANES;
     const unsigned int per_block = 256 / LANES;
-    const unsigned int seg = blockIdx.x;                 // one block per segment of k_geometry
+    const unsigned int seg = blockIdx.x - 1;             // one block per segment of k_geometry
     const unsigned int n_here = ws.seg_count[seg];
     for (unsigned int j0 = 0; j0 < n_here; j0 += per_block) {
         const unsigned int j = j0 + threadIdx.x / LANES;
@@ -373,21 +377,20 @@ int launch_geometry(const Context &c, const FrameParams &p, cudaStream_t s)
 }
 
 template <int DEG, int LANES>
-static void launch_colour_t(const Context &c, int grid, cudaStream_t s)
+static void launch_colour_t(const Context &c, const FrameParams &p, int grid, cudaStream_t s)
 {
-    if (c.flags & FLOD_OPT_DEBUG) k_colour<DEG, LANES, true><<<grid, 256, 0, s>>>(c.scene, c.ws);
-    else k_colour<DEG, LANES, false><<<grid, 256, 0, s>>>(c.scene, c.ws);
+    if (c.flags & FLOD_OPT_DEBUG) k_colour<DEG, LANES, true><<<grid, 256, 0, s>>>(c.scene, c.ws, p.TX, p.TY, p.max_pairs);
+    else k_colour<DEG, LANES, false><<<grid, 256, 0, s>>>(c.scene, c.ws, p.TX, p.TY, p.max_pairs);
 }
 
 int launch_colour(const Context &c, const FrameParams &p, cudaStream_t s)
 {
-    if (p.n_pre_blocks <= 0) return 0;
-    const int grid = p.n_pre_blocks;
+    const int grid = max(p.n_pre_blocks, 0) + 1;        // block 0 = tile scan: runs even when nothing is scanned
     switch (c.sh_degree) {
-        case 0: launch_colour_t<0, 1>(c, grid, s); break;
-        case 1: launch_colour_t<1, 1>(c, grid, s); break;
-        case 2: launch_colour_t<2, 1>(c, grid, s); break;
-        default: launch_colour_t<3, 4>(c, grid, s); break;
+        case 0: launch_colour_t<0, 1>(c, p, grid, s); break;
+        case 1: launch_colour_t<1, 1>(c, p, grid, s); break;
+        case 2: launch_colour_t<2, 1>(c, p, grid, s); break;
+        default: launch_colour_t<3, 4>(c, p, grid, s); break;
     }
     return 1;
 }

@@ -1,0 +1,93 @@
+// Steps a5 + a8: the 2-D prefix sum of the difference grid written by k_geometry = pairs per tile; the
+// exclusive scan over the tiles in row-major order = [start, end) of every tile's list (the ranges of step a8, known
+// before any pair exists) (the append counters of k_duplicate are zeroed here too).
+//
+// Run by ONE block of k_colour (block 0, so that it starts first): 65 KB of traffic and a few microseconds of pure
+// latency, hidden under the HBM-bound colour blocks instead of sitting on the critical path as a kernel of its own.
+// Works in place on ws.tile_cnt (global memory, L2-resident), any grid size, any block size that is a multiple of 32.
+#pragma once
+#include "flod_internal.cuh"
+
+namespace flod {
+
+__device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, int TY, unsigned int max_pairs)
+{
+    __shared__ unsigned long long s_wtot[32];
+    const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
+    const int gw = TX + 1, gh = TY + 1;
+    const int *__restrict__ diff = ws.tile_diff;
+    int *cnt = ws.tile_cnt;
+
+    // ---- prefix along x: a warp owns a row, 32 cells per step, carry in a register
+    for (int y = warp; y < gh; y += nwarp) {
+        int carry = 0;
+        for (int x0 = 0; x0 < gw; x0 += 32) {
+            const int x = x0 + lane;
+            int v = x < gw ? diff[(size_t)(y * gw + x) * kCtrStride] : 0;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, v, o);
+                if (lane >= o) v += t;
+            }
+            v += carry;
+            if (x < gw) cnt[y * gw + x] = v;
+            carry = __shfl_sync(0xffffffffu, v, 31);
+        }
+    }
+    __syncthreads();
+    // ---- prefix along y: a thread owns a column, eight independent loads in flight per step
+    for (int x = tid; x < gw; x += nthr) {
+        int run = 0;
+        for (int y0 = 0; y0 < gh; y0 += 8) {
+            int v[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] = y0 + k < gh ? cnt[(y0 + k) * gw + x] : 0;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                run += v[k];
+                if (y0 + k < gh) cnt[(y0 + k) * gw + x] = run;        // = pairs of tile (x, y0 + k)
+            }
+        }
+    }
+    __syncthreads();
+    // ---- exclusive scan over the tiles; a thread owns a contiguous chunk
+    const int T_n = TX * TY;
+    const int per = (T_n + nthr - 1) / nthr;
+    const int t0 = min(tid * per, T_n), t1 = min(t0 + per, T_n);
+    unsigned long long sum = 0;
+    for (int t = t0; t < t1; ++t) sum += (unsigned int)cnt[(t / TX) * gw + (t % TX)];
+    unsigned long long incl = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned long long t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    if (lane == 31) s_wtot[warp] = incl;
+    __syncthreads();
+    unsigned long long run = incl - sum, total = 0;
+    for (int w = 0; w < nwarp; ++w) {
+        const unsigned long long t = s_wtot[w];
+        if (w < warp) run += t;
+        total += t;
+    }
+    unsigned int too_long = 0;
+    for (int t = t0; t < t1; ++t) {
+        const unsigned int c = (unsigned int)cnt[(t / TX) * gw + (t % TX)];
+        const unsigned int a = (unsigned int)min(run, (unsigned long long)max_pairs);
+        const unsigned int b = (unsigned int)min(run + c, (unsigned long long)max_pairs);
+        ws.ranges[t] = make_uint2(a, b);
+        if (c > (1u << 24)) too_long = 1u;                     // k_duplicate counts a tile's entries in a float
+        run += c;
+    }
+    // the append counters of the 2x2 tile groups start at 0
+    const int n_groups = ((TX + 1) / 2) * ((TY + 1) / 2);
+    for (int g = tid; g < n_groups; g += nthr)
+        *reinterpret_cast<float4 *>(ws.cursor4 + (size_t)g * kCtrStride) = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    too_long = __syncthreads_or((int)too_long);
+    if (tid == 0) {
+        ws.hdr->n_pairs_clamped = (unsigned int)min(total, (unsigned long long)max_pairs);
+        ws.hdr->overflow = (total > max_pairs || too_long) ? 1u : 0u;
+    }
+}
+
+}  // namespace flod

@@ -19,6 +19,9 @@ constexpr int kSortThreads = 256;
 constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kSortBinsLog = 11;
 constexpr int kSortBins = 1 << kSortBinsLog;
+#ifndef FLOD_SORT_KEYS_PER_BIN_LOG
+#define FLOD_SORT_KEYS_PER_BIN_LOG 1
+#endif
 constexpr unsigned int kRankMax = 64;                     // bins up to this size are finished by per-key rank counting
 
 typedef unsigned long long u64;
@@ -29,6 +32,7 @@ struct SortSmem {
     u64 red_min[kSortWarps], red_max[kSortWarps];
     unsigned int red_u[kSortWarps];
     unsigned int wsum[kSortWarps];
+    unsigned int any_big[2];                              // per level: some bin exceeded kRankMax (set by rank_small)
 };
 
 struct BinMap { u64 kmin; int shift; unsigned int nb; };
@@ -67,7 +71,7 @@ __device__ BinMap bin_pass(const u64 *src, u64 *dst, unsigned int n, unsigned in
     m.kmin = kmin;
     const u64 range = kmax - kmin;
     const int bits = range ? 64 - __clzll(range) : 0;
-    const int want = min(kSortBinsLog, max(8, 32 - __clz(max(n, 2u) - 1)));      // about one key per bin
+    const int want = min(kSortBinsLog, max(6, 32 - FLOD_SORT_KEYS_PER_BIN_LOG - __clz(max(n, 2u) - 1)));   // about two keys per bin
     m.shift = max(0, bits - want);
     m.nb = (unsigned int)(range >> m.shift) + 1u;                                  // <= 2^want
     for (unsigned int b = tid; b < m.nb; b += kSortThreads) ends[b] = 0;
@@ -94,6 +98,9 @@ __device__ BinMap bin_pass(const u64 *src, u64 *dst, unsigned int n, unsigned in
         for (unsigned int b = b0; b < b1; ++b) { const unsigned int c = ends[b]; ends[b] = run; run += c; }
     }
     __syncthreads();
+    // (keeping the arrival rank that a value-returning histogram atomic would give, to save this second atomic,
+    // measured 9 us slower on config 1: it needs a rank array, two more barriers and a pass that turns bin starts into
+    // bin ends, and with about five keys per thread the fixed cost per tile is what counts)
     for (unsigned int j = tid; j < n; j += kSortThreads) {
         const u64 k = src[j];
         dst[atomicAdd(&ends[bin_of(m, k)], 1u)] = k;
@@ -105,13 +112,13 @@ __device__ BinMap bin_pass(const u64 *src, u64 *dst, unsigned int n, unsigned in
 // Final positions of the keys that sit in bins of at most kRankMax keys: position = bin start + number of smaller
 // keys in the bin.  buf[0, n) is the output of bin_pass; the compact indices go to out[0, n).
 __device__ __forceinline__ void rank_small(const u64 *buf, unsigned int n, const unsigned int *ends, const BinMap &m,
-                                           uint32_t *__restrict__ out, int tid)
+                                           uint32_t *__restrict__ out, unsigned int *any_big, int tid)
 {
     for (unsigned int p = tid; p < n; p += kSortThreads) {
         const u64 k = buf[p];
         const unsigned int b = bin_of(m, k);
         const unsigned int lo = b ? ends[b - 1] : 0u, hi = ends[b];
-        if (hi - lo > kRankMax) continue;
+        if (hi - lo > kRankMax) { *any_big = 1u; continue; }
         unsigned int cnt = 0;
         for (unsigned int q = lo; q < hi; ++q) cnt += buf[q] < k ? 1u : 0u;
         out[lo + cnt] = (uint32_t)k;
@@ -136,7 +143,9 @@ __device__ void finish_sort(const u64 *buf, unsigned int n, const BinMap &m, u64
                             SortSmem &S, int tid)
 {
     const unsigned int *ends = S.ends[0];
-    rank_small(buf, n, ends, m, out, tid);
+    rank_small(buf, n, ends, m, out, &S.any_big[0], tid);       // any_big was zeroed before the barriers of bin_pass
+    __syncthreads();
+    if (!S.any_big[0]) return;                                  // the usual case: no bin scan, no further barrier
     unsigned int from = 0;
     while (true) {
         const unsigned int b = next_big_bin(ends, m.nb, from, S, tid);
@@ -145,11 +154,13 @@ __device__ void finish_sort(const u64 *buf, unsigned int n, const BinMap &m, u64
         const unsigned int lo = b ? ends[b - 1] : 0u, n2 = ends[b] - lo;
         // ---- level 2: the bin over its own key range
         u64 *buf2 = scratch + lo;
+        if (tid == 0) S.any_big[1] = 0;                         // ordered by the barriers of bin_pass / next_big_bin
         const BinMap m2 = bin_pass(buf + lo, buf2, n2, S.ends[1], S, tid);
         const unsigned int *ends2 = S.ends[1];
-        rank_small(buf2, n2, ends2, m2, out + lo, tid);
+        rank_small(buf2, n2, ends2, m2, out + lo, &S.any_big[1], tid);
+        __syncthreads();
         unsigned int from2 = 0;
-        while (true) {
+        while (S.any_big[1]) {
             const unsigned int b2 = next_big_bin(ends2, m2.nb, from2, S, tid);
             if (b2 == 0xffffffffu) break;
             from2 = b2 + 1;
@@ -181,6 +192,7 @@ k_tile_sort(const WorkspaceDev ws, int n_tiles)
     uint32_t *vals = ws.vals + rg.x;
     if (L == 1) { if (tid == 0) vals[0] = (uint32_t)pairs[0]; return; }
     u64 *buf = L <= (unsigned int)kSortCap ? S.keys : ws.pairs_tmp + rg.x;
+    if (tid == 0) S.any_big[0] = 0;
     const BinMap m = bin_pass(pairs, buf, L, S.ends[0], S, tid);
     finish_sort(buf, L, m, pairs, vals, S, tid);
 }

@@ -345,6 +345,23 @@ def test_render_to_host_matches_render(config0):
     assert np.array_equal(a, b)
 
 
+def test_pipelined_render_to_host_keeps_every_frame(config0):
+    """flod_render_to_host_async: six frames with alternating level modes, kernels and copies on two streams, two
+    images in the workspace -- every host buffer must hold exactly its own frame."""
+    import torch
+    sc, cam, osc, r = config0
+    modes = [(2, 2), (1, 2), (1, 1), (2, 2), (1, 2), (1, 1)]
+    want = [r.render(cam, ls, le, 1.0).cpu().numpy() for (ls, le) in modes]
+    copy_stream = torch.cuda.Stream(device=r.device)
+    bufs = [torch.zeros((3, cam.height, cam.width), dtype=torch.float32).pin_memory() for _ in modes]
+    for (ls, le), b in zip(modes, bufs):
+        r.render_to_host_async(cam, ls, le, 1.0, b, copy_stream)
+    r.wait_host()
+    for w, b in zip(want, bufs):
+        assert np.array_equal(w, b.numpy())
+    assert not np.array_equal(want[0], want[2])
+
+
 def test_instrumented_counts_match_oracle(pkg, config0):
     """E and B of the blend stage (used for the FP32 roofline) against the oracle's per-pixel counts."""
     sc, cam, osc, _ = config0
