@@ -3,14 +3,19 @@
 // order"; clamp 0.99, skip below 1/255, stop after T < 1e-4 (R11, R12).
 //
 // One CTA of 128 threads owns one 16x16 tile; a thread owns two vertically adjacent pixels, a warp a 16x4 strip.
-// The tile's sorted list is consumed in batches of 256: threads fetch compact indices (coalesced) and gather the
-// 36 B of blend features per Gaussian (L2-resident) into shared memory.  Each warp then FILTERS the batch against
-// its own strip -- a lane tests 8 Gaussians with the exact row-segment bound of the factorised exponent
-//     e(x, y) = log2(o) - a2 w^2 - d2 dy^2,   w = (mu'x - x) + k dy          (DESIGN R25)
-// (min over x in the strip of |w| is closed-form) and the survivors are ballot-compacted, in order, into a
-// per-warp index list.  Only those are evaluated per pixel.  A filtered-out Gaussian has alpha < 2^-0.001 / 255 on
-// every pixel of the strip, so the image is bit-identical to the unfiltered loop.  A warp whose 64 pixels have
-// all terminated skips filter and loop; the CTA stops when every warp has.
+// The tile's sorted list is consumed in batches of 256: threads fetch positions (coalesced) and gather the 36 B of
+// blend features per Gaussian (L2-resident) into shared memory, mu' made relative to the tile's first pixel centre.
+// Each warp then FILTERS the batch against its own strip, 32 Gaussians per step (one per lane).  With the
+// factorised exponent (DESIGN R25)
+//     e(x, y) = log2(o) + a2 w^2 + d2 dy^2,   w = (mu'x - x) + k dy,   a2, d2 <= 0
+// everything that depends on the row only is computed ONCE per (Gaussian, row) by the filtering lane:
+//     c_r = mu'x + k dy_r,   e0_r = log2(o) + d2 dy_r^2        so that   e = a2 (c_r - x)^2 + e0_r,
+// the maximum of e over the 16 pixels of the row is closed-form, and a Gaussian whose four row maxima are all below
+// log2(1/255) is dropped.  The survivors are ballot-compacted, in order, into a per-warp buffer of 48-byte records
+// (c_0..c_3, e0_0..e0_3, a2, r, g, b); the per-pixel loop reads those and spends three packed instructions on the
+// exponent.  The filter bounds the very values the loop evaluates (same c_r, e0_r; rounding is monotone), so a
+// dropped Gaussian has alpha < 1/255 on every pixel of the strip and the image is bit-identical to the unfiltered
+// loop.  A warp whose 64 pixels have all terminated skips filter and loop; the CTA stops when every warp has.
 #include "flod_internal.cuh"
 
 namespace flod {
@@ -18,6 +23,7 @@ namespace flod {
 constexpr int kBlendThreads = 128;
 constexpr int kBatch = 256;
 constexpr int kBlendWarps = kBlendThreads / 32;
+constexpr int kWarpBuf = 64;                        // survivors a warp collects before it evaluates them
 constexpr float kTwo100 = 1.2676506002282294e30f;   // 2^100
 
 // 2^x on the MUFU unit (x <= 0 here; results below 2^-126 flush to 0, far under the 1/255 skip threshold)
@@ -33,23 +39,25 @@ __global__ void __launch_bounds__(kBlendThreads)
 k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, int n_tiles,
         float bg0, float bg1, float bg2)
 {
-    // one 48-byte record per Gaussian of the batch: (mu'x, mu'y, k, a2 | d2, log2 o, r, g | b, -, -, -)
+    // staging, one 48-byte record per Gaussian of the batch: (mu'x - x0, mu'y - y0, k, a2 | d2, log2 o, r, g | b, -, -, -)
     __shared__ float4 s_rec[kBatch * 3];
-    __shared__ unsigned short s_list[kBlendWarps][kBatch];   // per warp: byte offsets of the surviving records
+    // per warp, one 48-byte record per surviving Gaussian: (c_0, c_1, e0_0, e0_1 | c_2, c_3, e0_2, e0_3 | a2, r, g, b)
+    __shared__ float4 s_buf[kBlendWarps][kWarpBuf * 3];
+    __shared__ unsigned short s_idx[kBlendWarps][kWarpBuf];    // batch index of the survivor (counting variant only)
 
     const int tile = blockIdx.x;
     if (tile >= n_tiles || ws.hdr->overflow) return;   // an overflowed frame is undefined: its lists were not sorted
     const int tx = tile % TX, ty = tile / TX;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // warp = rows 4w..4w+3 of the tile; lanes 0-15 rows (4w, 4w+1), lanes 16-31 rows (4w+2, 4w+3)
+    const int half = lane >> 4;
     const int px = tx * kTile + (lane & 15);
-    const int py0 = ty * kTile + warp * 4 + (lane >> 4) * 2, py1 = py0 + 1;
+    const int py0 = ty * kTile + warp * 4 + half * 2, py1 = py0 + 1;
     const bool in0 = px < W && py0 < H, in1 = px < W && py1 < H;
-    const float pxc = (float)px + 0.5f, pyc0 = (float)py0 + 0.5f, pyc1 = (float)py1 + 0.5f;
-    // the warp's strip, for the filter: pixel centres x in [sx0, sx1], rows sy + {0,1,2,3}
-    const float sx0 = (float)(tx * kTile) + 0.5f, sx1 = sx0 + 15.0f;
-    const float sy = (float)(ty * kTile + warp * 4) + 0.5f;
-    const float kThr = -7.994353436858858f - 1.0e-3f;  // log2(1/255) minus a safety margin
+    const float x0c = (float)(tx * kTile) + 0.5f, y0c = (float)(ty * kTile) + 0.5f;   // centre of the tile's first pixel
+    const float nlx = -(float)(lane & 15);              // minus the pixel's column inside the tile
+    const float row0 = (float)(warp * 4);               // first row of the warp's strip inside the tile
+    const float kThr = -7.994353436858858f - 1.0e-3f;   // log2(1/255) minus a safety margin
 
     const uint2 rg = ws.ranges[tile];
     const uint32_t *__restrict__ vals = ws.vals;
@@ -60,83 +68,35 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
     // two pixels per thread, packed as float2 (.x = row py0, .y = row py1): the per-pixel arithmetic runs on the
     // packed FP32 instructions of sm_100 (FADD2 / FMUL2 / FFMA2: one issue slot for both pixels)
     float2 T = make_float2(1.0f, 1.0f), cr = make_float2(0.0f, 0.0f), cg = cr, cb2 = cr;
-    const float2 npyc = make_float2(-pyc0, -pyc1);
-    bool done0 = !in0, done1 = !in1;
     unsigned int n_eval = 0, n_blend = 0;
-    unsigned short *my_list = s_list[warp];
-    const unsigned char *rec_bytes = reinterpret_cast<const unsigned char *>(s_rec);
+    float4 *my_buf = s_buf[warp];
+    const float4 *my_half = my_buf + half;
     // done pixels: thr = +huge, so that no alpha passes the skip test (live pixels: thr = 1/255)
     float thr0 = in0 ? (1.0f / 255.0f) : 3.0e38f, thr1 = in1 ? (1.0f / 255.0f) : 3.0e38f;
+    bool warp_done = __all_sync(0xffffffffu, thr0 > 1.0f && thr1 > 1.0f);
 
-    for (unsigned int base = rg.x; base < rg.y; base += kBatch) {
-        const bool warp_done = __all_sync(0xffffffffu, done0 && done1);
-        if (__syncthreads_count(!warp_done) == 0) break;
-        const unsigned int m = min((unsigned int)kBatch, rg.y - base);
-#pragma unroll
-        for (int h = 0; h < kBatch / kBlendThreads; ++h) {
-            const unsigned int j = tid + h * kBlendThreads;
-            if (j < m) {
-                const uint32_t ci = vals[base + j];
-                s_rec[3 * j] = gA[ci];
-                s_rec[3 * j + 1] = gB[ci];
-                s_rec[3 * j + 2].x = cB[ci];
-            }
-        }
-        __syncthreads();
-        if (warp_done) continue;
-
-        // ---- filter: which Gaussians of the batch can reach alpha >= 1/255 somewhere on this warp's strip
-        unsigned int cnt = 0;
-#pragma unroll
-        for (int i = 0; i < kBatch / 32; ++i) {
-            const unsigned int j = lane + 32 * i;
-            bool hit = false;
-            if (j < m) {
-                const float4 a = s_rec[3 * j];
-                const float4 b = s_rec[3 * j + 1];
-                const float dxl = a.x - sx1, dxh = a.x - sx0;        // range of (mu'x - x) over the strip
-                float best = -INFINITY;
-#pragma unroll
-                for (int rr = 0; rr < 4; ++rr) {
-                    const float dy = a.y - (sy + (float)rr);
-                    const float kd = a.z * dy;
-                    const float wmin = fmaxf(fmaxf(dxl + kd, -(dxh + kd)), 0.0f);
-                    const float e = fmaf(a.w, wmin * wmin, fmaf(b.x, dy * dy, b.y));
-                    best = fmaxf(best, e);
-                }
-                hit = best >= kThr;
-            }
-            const unsigned int bal = __ballot_sync(0xffffffffu, hit);
-            if (hit) my_list[cnt + __popc(bal & ((1u << lane) - 1))] = (unsigned short)(j * 48u);
-            cnt += __popc(bal);
-        }
-        __syncwarp();
-
-        // ---- evaluate the survivors.  a.w and b.x are <= 0 (k_geometry clamps them), so e <= log2 o: q >= 0 holds
-        // by construction and alpha needs the 0.99 clamp only.  A pixel that is done or below 1/255 blends alpha = 0.
+    // evaluates my_buf[0, cnt) on the thread's two pixels.  a2 <= 0 and e0 <= log2 o (k_geometry clamps d2), so
+    // q >= 0 holds by construction and alpha needs the 0.99 clamp only.  A pixel that is done or below 1/255 blends 0.
+    auto evaluate = [&](unsigned int cnt, unsigned int base_in_list) {
 #pragma unroll 2
         for (unsigned int t = 0; t < cnt; ++t) {
-            const unsigned int off = my_list[t];
-            const float4 a = *reinterpret_cast<const float4 *>(rec_bytes + off);
-            const float4 b = *reinterpret_cast<const float4 *>(rec_bytes + off + 16);
-            const float cbj = *reinterpret_cast<const float *>(rec_bytes + off + 32);
-            const float dx = a.x - pxc;
-            const float2 dy = __fadd2_rn(make_float2(a.y, a.y), npyc);
-            const float2 w = __ffma2_rn(make_float2(a.z, a.z), dy, make_float2(dx, dx));
-            const float2 e = __ffma2_rn(make_float2(a.w, a.w), __fmul2_rn(w, w),
-                                        __ffma2_rn(make_float2(b.x, b.x), __fmul2_rn(dy, dy), make_float2(b.y, b.y)));
+            const float4 hrec = my_half[3 * t];
+            const float4 c = my_buf[3 * t + 2];
+            const float2 w = __fadd2_rn(make_float2(hrec.x, hrec.y), make_float2(nlx, nlx));
+            const float2 e = __ffma2_rn(make_float2(c.x, c.x), __fmul2_rn(w, w), make_float2(hrec.z, hrec.w));
             float al0 = fminf(ex2(e.x), 0.99f), al1 = fminf(ex2(e.y), 0.99f);
             al0 = al0 >= thr0 ? al0 : 0.0f;
             al1 = al1 >= thr1 ? al1 : 0.0f;
             const float2 wgt = __fmul2_rn(T, make_float2(al0, al1));
-            cr = __ffma2_rn(wgt, make_float2(b.z, b.z), cr);
-            cg = __ffma2_rn(wgt, make_float2(b.w, b.w), cg);
-            cb2 = __ffma2_rn(wgt, make_float2(cbj, cbj), cb2);
+            cr = __ffma2_rn(wgt, make_float2(c.y, c.y), cr);
+            cg = __ffma2_rn(wgt, make_float2(c.z, c.z), cg);
+            cb2 = __ffma2_rn(wgt, make_float2(c.w, c.w), cb2);
             T = __fadd2_rn(T, make_float2(-wgt.x, -wgt.y));           // T (1 - alpha)
             if (COUNT) {
                 n_blend += (al0 > 0.0f ? 1u : 0u) + (al1 > 0.0f ? 1u : 0u);
-                if (thr0 < 1.0f && T.x < 1e-4f) n_eval += (base - rg.x) + off / 48u + 1;
-                if (thr1 < 1.0f && T.y < 1e-4f) n_eval += (base - rg.x) + off / 48u + 1;
+                const unsigned int visited = base_in_list + s_idx[warp][t] + 1;
+                if (thr0 < 1.0f && T.x < 1e-4f) n_eval += visited;
+                if (thr1 < 1.0f && T.y < 1e-4f) n_eval += visited;
             }
             // blend, then stop (R12): (1e-4 - T) 2^100 is positive exactly when T < 1e-4 (the scaling by a power of
             // two and the difference of the two products are exact up to one rounding that keeps the sign), and
@@ -145,8 +105,67 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
             thr0 = fmaxf(thr0, stop.x);
             thr1 = fmaxf(thr1, stop.y);
         }
-        done0 = thr0 > 1.0f; done1 = thr1 > 1.0f;
+    };
+
+    for (unsigned int base = rg.x; base < rg.y; base += kBatch) {
+        if (__syncthreads_count(!warp_done) == 0) break;
+        const unsigned int m = min((unsigned int)kBatch, rg.y - base);
+#pragma unroll
+        for (int h = 0; h < kBatch / kBlendThreads; ++h) {
+            const unsigned int j = tid + h * kBlendThreads;
+            if (j < m) {
+                const uint32_t ci = vals[base + j];
+                float4 a = gA[ci];
+                a.x -= x0c; a.y -= y0c;
+                s_rec[3 * j] = a;
+                s_rec[3 * j + 1] = gB[ci];
+                s_rec[3 * j + 2].x = cB[ci];
+            }
+        }
+        __syncthreads();
+        if (warp_done) continue;
+
+        unsigned int cnt = 0;
+        for (unsigned int j0 = 0; j0 < m; j0 += 32) {
+            // ---- filter: can Gaussian j0 + lane reach alpha >= 1/255 somewhere on this warp's strip
+            const unsigned int j = j0 + lane;
+            bool hit = false;
+            float4 h0, h1, c;
+            if (j < m) {
+                const float4 a = s_rec[3 * j];
+                const float4 b = s_rec[3 * j + 1];
+                const float dy0 = a.y - row0, dy1 = dy0 - 1.0f, dy2 = dy0 - 2.0f, dy3 = dy0 - 3.0f;
+                h0.x = fmaf(a.z, dy0, a.x); h0.y = fmaf(a.z, dy1, a.x);
+                h1.x = fmaf(a.z, dy2, a.x); h1.y = fmaf(a.z, dy3, a.x);
+                h0.z = fmaf(b.x, dy0 * dy0, b.y); h0.w = fmaf(b.x, dy1 * dy1, b.y);
+                h1.z = fmaf(b.x, dy2 * dy2, b.y); h1.w = fmaf(b.x, dy3 * dy3, b.y);
+                // min over the row's 16 pixel columns x = 0..15 of |c_r - x|
+                const float w0 = fmaxf(fmaxf(h0.x - 15.0f, -h0.x), 0.0f), w1 = fmaxf(fmaxf(h0.y - 15.0f, -h0.y), 0.0f);
+                const float w2 = fmaxf(fmaxf(h1.x - 15.0f, -h1.x), 0.0f), w3 = fmaxf(fmaxf(h1.y - 15.0f, -h1.y), 0.0f);
+                const float best = fmaxf(fmaxf(fmaf(a.w, w0 * w0, h0.z), fmaf(a.w, w1 * w1, h0.w)),
+                                         fmaxf(fmaf(a.w, w2 * w2, h1.z), fmaf(a.w, w3 * w3, h1.w)));
+                hit = best >= kThr;
+                c = make_float4(a.w, b.z, b.w, s_rec[3 * j + 2].x);
+            }
+            const unsigned int bal = __ballot_sync(0xffffffffu, hit);
+            if (hit) {
+                const unsigned int slot = cnt + __popc(bal & ((1u << lane) - 1));
+                my_buf[3 * slot] = h0; my_buf[3 * slot + 1] = h1; my_buf[3 * slot + 2] = c;
+                if (COUNT) s_idx[warp][slot] = (unsigned short)j;
+            }
+            cnt += __popc(bal);
+            // ---- evaluate when the next step might not fit (or at the end of the batch)
+            if (cnt > kWarpBuf - 32 || j0 + 32 >= m) {
+                __syncwarp();
+                evaluate(cnt, base - rg.x);
+                cnt = 0;
+                warp_done = __all_sync(0xffffffffu, thr0 > 1.0f && thr1 > 1.0f);
+                if (warp_done) break;
+                __syncwarp();
+            }
+        }
     }
+    const bool done0 = thr0 > 1.0f, done1 = thr1 > 1.0f;
     const float T0 = T.x, T1 = T.y, r0 = cr.x, r1 = cr.y, g0 = cg.x, g1 = cg.y, b0 = cb2.x, b1 = cb2.y;
     const size_t plane = (size_t)W * H;
     if (in0) {
