@@ -3,8 +3,8 @@
 // order"; clamp 0.99, skip below 1/255, stop after T < 1e-4 (R11, R12).
 //
 // One CTA of 128 threads owns one 16x16 tile; a thread owns two vertically adjacent pixels, a warp a 16x4 strip.
-// The tile's sorted list is consumed in batches of 256: threads fetch positions (coalesced) and gather the 36 B of
-// blend features per Gaussian (L2-resident) into shared memory, mu' made relative to the tile's first pixel centre.
+// The tile's sorted list is consumed in batches of 128: a thread fetches one position (coalesced) and gathers the 36 B
+// of blend features of that Gaussian (L2-resident) into shared memory with cp.async, double-buffered.
 // Each warp then FILTERS the batch against its own strip, 32 Gaussians per step (one per lane).  With the
 // factorised exponent (DESIGN R25)
 //     e(x, y) = log2(o) + a2 w^2 + d2 dy^2,   w = (mu'x - x) + k dy,   a2, d2 <= 0
@@ -21,10 +21,30 @@
 namespace flod {
 
 constexpr int kBlendThreads = 128;
-constexpr int kBatch = 256;
+#ifndef FLOD_BLEND_BATCH
+#define FLOD_BLEND_BATCH 128
+#endif
+constexpr int kBatch = FLOD_BLEND_BATCH;             // Gaussians staged per step (a multiple of kBlendThreads)
 constexpr int kBlendWarps = kBlendThreads / 32;
-constexpr int kWarpBuf = 64;                        // survivors a warp collects before it evaluates them
-constexpr float kTwo100 = 1.2676506002282294e30f;   // 2^100
+#ifndef FLOD_BLEND_WARPBUF
+#define FLOD_BLEND_WARPBUF 32
+#endif
+#ifndef FLOD_BLEND_FLUSH
+#define FLOD_BLEND_FLUSH (FLOD_BLEND_WARPBUF - 32)
+#endif
+constexpr int kFlush = FLOD_BLEND_FLUSH;             // evaluate when more than this many survivors wait (<= kWarpBuf - 32)
+constexpr int kWarpBuf = FLOD_BLEND_WARPBUF;                        // survivors a warp collects before it evaluates them
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((unsigned int)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void *smem, const void *gmem)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned int)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // 2^x on the MUFU unit (x <= 0 here; results below 2^-126 flush to 0, far under the 1/255 skip threshold)
 __device__ __forceinline__ float ex2(float x)
@@ -34,13 +54,17 @@ __device__ __forceinline__ float ex2(float x)
     return y;
 }
 
+#ifndef FLOD_BLEND_MINBLOCKS
+#define FLOD_BLEND_MINBLOCKS 8
+#endif
 template <bool COUNT>
-__global__ void __launch_bounds__(kBlendThreads)
+__global__ void __launch_bounds__(kBlendThreads, FLOD_BLEND_MINBLOCKS)
 k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, int n_tiles,
         float bg0, float bg1, float bg2)
 {
-    // staging, one 48-byte record per Gaussian of the batch: (mu'x - x0, mu'y - y0, k, a2 | d2, log2 o, r, g | b, -, -, -)
-    __shared__ float4 s_rec[kBatch * 3];
+    // staging, 36 bytes per Gaussian of the batch: A = (mu'x, mu'y, k, a2), B = (d2, log2 o, r, g), c = b
+    __shared__ float4 s_A[2][kBatch], s_B[2][kBatch];           // double-buffered
+    __shared__ float s_c[2][kBatch];
     // per warp, one 48-byte record per surviving Gaussian: (c_0, c_1, e0_0, e0_1 | c_2, c_3, e0_2, e0_3 | a2, r, g, b)
     __shared__ float4 s_buf[kBlendWarps][kWarpBuf * 3];
     __shared__ unsigned short s_idx[kBlendWarps][kWarpBuf];    // batch index of the survivor (counting variant only)
@@ -71,9 +95,9 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
     unsigned int n_eval = 0, n_blend = 0;
     float4 *my_buf = s_buf[warp];
     const float4 *my_half = my_buf + half;
-    // done pixels: thr = +huge, so that no alpha passes the skip test (live pixels: thr = 1/255)
-    float thr0 = in0 ? (1.0f / 255.0f) : 3.0e38f, thr1 = in1 ? (1.0f / 255.0f) : 3.0e38f;
-    bool warp_done = __all_sync(0xffffffffu, thr0 > 1.0f && thr1 > 1.0f);
+    // pixels outside the image: thr = +huge, so that no alpha passes the skip test (inside: thr = 1/255)
+    const float thr0 = in0 ? (1.0f / 255.0f) : 3.0e38f, thr1 = in1 ? (1.0f / 255.0f) : 3.0e38f;
+    bool warp_done = __all_sync(0xffffffffu, !in0 && !in1);
 
     // evaluates my_buf[0, cnt) on the thread's two pixels.  a2 <= 0 and e0 <= log2 o (k_geometry clamps d2), so
     // q >= 0 holds by construction and alpha needs the 0.99 clamp only.  A pixel that is done or below 1/255 blends 0.
@@ -85,45 +109,72 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
             const float2 w = __fadd2_rn(make_float2(hrec.x, hrec.y), make_float2(nlx, nlx));
             const float2 e = __ffma2_rn(make_float2(c.x, c.x), __fmul2_rn(w, w), make_float2(hrec.z, hrec.w));
             float al0 = fminf(ex2(e.x), 0.99f), al1 = fminf(ex2(e.y), 0.99f);
-            al0 = al0 >= thr0 ? al0 : 0.0f;
-            al1 = al1 >= thr1 ? al1 : 0.0f;
+            // skip below 1/255 (R11); a pixel that has stopped (T < 1e-4 after an earlier blend, R12) blends nothing.
+            // The test reads T directly: the loop-carried chain is T -> compare -> select -> multiply -> subtract.
+#ifndef FLOD_X_BLEND_STOP_MASK
+            al0 = (al0 >= thr0 && T.x >= 1e-4f) ? al0 : 0.0f;
+            al1 = (al1 >= thr1 && T.y >= 1e-4f) ? al1 : 0.0f;
+#else
+            al0 = al0 >= fmaxf(thr0, (1e-4f - T.x) * 1.2676506002282294e30f) ? al0 : 0.0f;
+            al1 = al1 >= fmaxf(thr1, (1e-4f - T.y) * 1.2676506002282294e30f) ? al1 : 0.0f;
+#endif
             const float2 wgt = __fmul2_rn(T, make_float2(al0, al1));
             cr = __ffma2_rn(wgt, make_float2(c.y, c.y), cr);
             cg = __ffma2_rn(wgt, make_float2(c.z, c.z), cg);
             cb2 = __ffma2_rn(wgt, make_float2(c.w, c.w), cb2);
-            T = __fadd2_rn(T, make_float2(-wgt.x, -wgt.y));           // T (1 - alpha)
+            const float2 Tn = __fadd2_rn(T, make_float2(-wgt.x, -wgt.y));        // T (1 - alpha)
             if (COUNT) {
                 n_blend += (al0 > 0.0f ? 1u : 0u) + (al1 > 0.0f ? 1u : 0u);
                 const unsigned int visited = base_in_list + s_idx[warp][t] + 1;
-                if (thr0 < 1.0f && T.x < 1e-4f) n_eval += visited;
-                if (thr1 < 1.0f && T.y < 1e-4f) n_eval += visited;
+                if (T.x >= 1e-4f && Tn.x < 1e-4f) n_eval += visited;               // the blend that stops the pixel
+                if (T.y >= 1e-4f && Tn.y < 1e-4f) n_eval += visited;
             }
-            // blend, then stop (R12): (1e-4 - T) 2^100 is positive exactly when T < 1e-4 (the scaling by a power of
-            // two and the difference of the two products are exact up to one rounding that keeps the sign), and
-            // then at least 2^-37 2^100 > 0.99
-            const float2 stop = __ffma2_rn(T, make_float2(-kTwo100, -kTwo100), make_float2(1e-4f * kTwo100, 1e-4f * kTwo100));
-            thr0 = fmaxf(thr0, stop.x);
-            thr1 = fmaxf(thr1, stop.y);
+            T = Tn;
         }
     };
 
-    for (unsigned int base = rg.x; base < rg.y; base += kBatch) {
-        if (__syncthreads_count(!warp_done) == 0) break;
-        const unsigned int m = min((unsigned int)kBatch, rg.y - base);
+    // Software pipeline over the batches, one barrier per batch.  The features of batch b + 1 travel from L2 to the
+    // other staging buffer with cp.async (no registers, no wait) while batch b is filtered and evaluated; the list
+    // positions of batch b + 2 are loaded into a register at the same time, so that the dependent chain position ->
+    // feature gather never stalls a warp.
+    const unsigned int n_batches = (rg.y - rg.x + kBatch - 1) / kBatch;
+    constexpr int kPer = kBatch / kBlendThreads;                  // Gaussians a thread stages per batch
+    auto stage_batch = [&](unsigned int b, const uint32_t (&ci)[kPer]) {   // batch b -> staging buffer b & 1
 #pragma unroll
-        for (int h = 0; h < kBatch / kBlendThreads; ++h) {
+        for (int h = 0; h < kPer; ++h) {
             const unsigned int j = tid + h * kBlendThreads;
-            if (j < m) {
-                const uint32_t ci = vals[base + j];
-                float4 a = gA[ci];
-                a.x -= x0c; a.y -= y0c;
-                s_rec[3 * j] = a;
-                s_rec[3 * j + 1] = gB[ci];
-                s_rec[3 * j + 2].x = cB[ci];
+            if (rg.x + b * kBatch + j < rg.y) {
+                cp_async16(&s_A[b & 1][j], gA + ci[h]);
+                cp_async16(&s_B[b & 1][j], gB + ci[h]);
+                cp_async4(&s_c[b & 1][j], cB + ci[h]);
             }
         }
-        __syncthreads();
+        cp_async_commit();
+    };
+    auto load_positions = [&](unsigned int b, uint32_t (&ci)[kPer]) {
+#pragma unroll
+        for (int h = 0; h < kPer; ++h) {
+            const unsigned int i = rg.x + b * kBatch + tid + h * kBlendThreads;
+            if (i < rg.y) ci[h] = vals[i];
+        }
+    };
+    uint32_t ci_next[kPer] = {};                                    // positions of the batch to stage next
+    load_positions(0, ci_next);
+    if (n_batches) stage_batch(0, ci_next);
+    load_positions(1, ci_next);
+    for (unsigned int b = 0; b < n_batches; ++b) {
+        cp_async_wait_all();
+        // barrier: batch b is complete in staging buffer b & 1 for every thread, and every warp is through with batch b - 1
+        if (__syncthreads_count(!warp_done) == 0) break;
+        if (b + 1 < n_batches) {
+            stage_batch(b + 1, ci_next);
+            load_positions(b + 2, ci_next);
+        }
         if (warp_done) continue;
+        const unsigned int base = rg.x + b * kBatch;
+        const unsigned int m = min((unsigned int)kBatch, rg.y - base);
+        const float4 *recA = s_A[b & 1], *recB = s_B[b & 1];
+        const float *recC = s_c[b & 1];
 
         unsigned int cnt = 0;
         for (unsigned int j0 = 0; j0 < m; j0 += 32) {
@@ -132,8 +183,9 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
             bool hit = false;
             float4 h0, h1, c;
             if (j < m) {
-                const float4 a = s_rec[3 * j];
-                const float4 b = s_rec[3 * j + 1];
+                float4 a = recA[j];
+                const float4 b = recB[j];
+                a.x -= x0c; a.y -= y0c;                              // relative to the tile's first pixel centre
                 const float dy0 = a.y - row0, dy1 = dy0 - 1.0f, dy2 = dy0 - 2.0f, dy3 = dy0 - 3.0f;
                 h0.x = fmaf(a.z, dy0, a.x); h0.y = fmaf(a.z, dy1, a.x);
                 h1.x = fmaf(a.z, dy2, a.x); h1.y = fmaf(a.z, dy3, a.x);
@@ -145,7 +197,7 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
                 const float best = fmaxf(fmaxf(fmaf(a.w, w0 * w0, h0.z), fmaf(a.w, w1 * w1, h0.w)),
                                          fmaxf(fmaf(a.w, w2 * w2, h1.z), fmaf(a.w, w3 * w3, h1.w)));
                 hit = best >= kThr;
-                c = make_float4(a.w, b.z, b.w, s_rec[3 * j + 2].x);
+                c = make_float4(a.w, b.z, b.w, recC[j]);
             }
             const unsigned int bal = __ballot_sync(0xffffffffu, hit);
             if (hit) {
@@ -155,17 +207,17 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
             }
             cnt += __popc(bal);
             // ---- evaluate when the next step might not fit (or at the end of the batch)
-            if (cnt > kWarpBuf - 32 || j0 + 32 >= m) {
+            if (cnt > kFlush || j0 + 32 >= m) {
                 __syncwarp();
                 evaluate(cnt, base - rg.x);
                 cnt = 0;
-                warp_done = __all_sync(0xffffffffu, thr0 > 1.0f && thr1 > 1.0f);
+                warp_done = __all_sync(0xffffffffu, (!in0 || T.x < 1e-4f) && (!in1 || T.y < 1e-4f));
                 if (warp_done) break;
                 __syncwarp();
             }
         }
     }
-    const bool done0 = thr0 > 1.0f, done1 = thr1 > 1.0f;
+    const bool done0 = !in0 || T.x < 1e-4f, done1 = !in1 || T.y < 1e-4f;
     const float T0 = T.x, T1 = T.y, r0 = cr.x, r1 = cr.y, g0 = cg.x, g1 = cg.y, b0 = cb2.x, b1 = cb2.y;
     const size_t plane = (size_t)W * H;
     if (in0) {
