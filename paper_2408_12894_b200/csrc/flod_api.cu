@@ -34,7 +34,7 @@ size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 int sh_stride_for(int deg) { int k = (deg + 1) * (deg + 1); return (3 * k + 3) / 4 * 4; }
 
-constexpr int kScenePlanes = 3 + 6 + 3;   // mean xyz, cov x6, opacity, kappa, log2 o
+constexpr int kScenePlanes = 3 + 6 + 4;   // mean xyz, cov x6, opacity, kappa, log2 o, rho2
 
 size_t scene_bytes_for(int64_t n, int sh_degree)
 {
@@ -43,7 +43,8 @@ size_t scene_bytes_for(int64_t n, int sh_degree)
 }
 
 // Step a0 for one Gaussian (DESIGN §2 "O0"; Eq. 1).  fp64 from the fp32 inputs, rounded once.
-void activate_one(const float *ls, const float *q, float logit, float cov[6], float *o_out, float *kappa, float *l2o)
+void activate_one(const float *ls, const float *q, float logit, float cov[6], float *o_out, float *kappa, float *l2o,
+                  float *rho2)
 {
     const double s0 = exp((double)ls[0]), s1 = exp((double)ls[1]), s2 = exp((double)ls[2]);
     double w = q[0], x = q[1], y = q[2], z = q[3];
@@ -63,6 +64,10 @@ void activate_one(const float *ls, const float *q, float logit, float cov[6], fl
     *o_out = o;
     *kappa = dead ? -1.0f : (float)(2.0 * log(255.0 * (double)o));
     *l2o = dead ? -126.0f : (float)log2((double)o);
+    // squared radius of the sphere around the mean that holds the alpha = 1/255 ellipsoid, rounded up; k_geometry's
+    // conservative off-screen test uses it before any covariance is read.  -1 marks a dead Gaussian.
+    const double r2 = 2.0 * log(255.0 * (double)o) * std::max(v0, std::max(v1, v2)) * (1.0 + 1e-4);
+    *rho2 = dead ? -1.0f : (r2 < 3.0e38 ? nextafterf((float)r2, INFINITY) : INFINITY);
 }
 
 bool finite_all(const float *p, size_t n)
@@ -230,10 +235,10 @@ int flod_upload_levels(flod_ctx *ctx, int n_levels, const flod_level_desc *level
             for (int64_t i = b; i < e; ++i) {
                 const int64_t g = base + i;
                 pl[0][g] = d.mean[3 * i]; pl[1][g] = d.mean[3 * i + 1]; pl[2][g] = d.mean[3 * i + 2];
-                float cov[6], o, kap, l2o;
-                activate_one(d.log_scale + 3 * i, d.quat + 4 * i, d.opacity_logit[i], cov, &o, &kap, &l2o);
+                float cov[6], o, kap, l2o, rho2;
+                activate_one(d.log_scale + 3 * i, d.quat + 4 * i, d.opacity_logit[i], cov, &o, &kap, &l2o, &rho2);
                 for (int k = 0; k < 6; ++k) pl[3 + k][g] = cov[k];
-                pl[9][g] = o; pl[10][g] = kap; pl[11][g] = l2o;
+                pl[9][g] = o; pl[10][g] = kap; pl[11][g] = l2o; pl[12][g] = rho2;
                 float *dst = shp + (size_t)g * stride;
                 const float *src = d.sh + (size_t)i * 3 * K;
                 if (sh_degree == 3) {
@@ -262,7 +267,7 @@ int flod_upload_levels(flod_ctx *ctx, int n_levels, const flod_level_desc *level
     auto P = [&](int i) { return (const float *)((const unsigned char *)dev + plane * i); };
     ctx->scene.mx = P(0); ctx->scene.my = P(1); ctx->scene.mz = P(2);
     for (int k = 0; k < 6; ++k) ctx->scene.cov[k] = P(3 + k);
-    ctx->scene.opacity = P(9); ctx->scene.kappa = P(10); ctx->scene.l2o = P(11);
+    ctx->scene.opacity = P(9); ctx->scene.kappa = P(10); ctx->scene.l2o = P(11); ctx->scene.rho2 = P(12);
     ctx->scene.sh = P(kScenePlanes);
     ctx->scene.sh_stride = stride; ctx->scene.sh_degree = sh_degree;
     ctx->arena = scene_arena_dev;
@@ -351,6 +356,10 @@ int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, flo
     for (int i = 0; i < 3; ++i) p.ref[i] = ctx->has_ref ? ctx->ref[i] : p.centre[i];
     p.limx = (float)(1.3 * (double)cam->width / (2.0 * (double)cam->fx));
     p.limy = (float)(1.3 * (double)cam->height / (2.0 * (double)cam->fy));
+    {   // conservative off-screen test of k_geometry: |row of J|^2 <= pre_c1 / z^2 (R8's clamp bounds u and v)
+        const double fm = std::max((double)cam->fx, (double)cam->fy), lm = std::max((double)p.limx, (double)p.limy);
+        p.pre_c1 = (float)(fm * fm * (1.0 + lm * lm) * 1.0001);
+    }
     const int i0 = mode.l_start - ctx->first_level, i1 = mode.l_end - ctx->first_level;   // level positions
     p.n_levels = i1 - i0 + 1;
     p.first_gid = ctx->level_off[i0];

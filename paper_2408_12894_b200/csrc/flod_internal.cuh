@@ -30,6 +30,7 @@ struct SceneDev {
     const float *opacity;                 // o (debug only on the device)
     const float *kappa;                   // 2 ln(255 o); -1 when dead
     const float *l2o;                     // log2(o)
+    const float *rho2;                    // kappa * largest eigenvalue of Sigma, rounded up (squared bounding radius); -1 when dead
     const float *sh;                      // [n][sh_stride] floats, row = K*3 coefficients padded to a multiple of 4
     int sh_stride;
     int sh_degree;
@@ -76,6 +77,7 @@ struct FrameParams {
     float R[9], t[3];
     float fx, fy, cx, cy, z_near;
     float limx, limy;                     // 1.3 W / (2 fx), 1.3 H / (2 fy), fp64 -> fp32 once
+    float pre_c1;                         // max(fx, fy)^2 (1 + max(limx, limy)^2), rounded up
     float centre[3];                      // -R^T t, fp64 -> fp32 once
     float ref[3];                         // selection reference (R2)
     float bg[3];

@@ -1,10 +1,11 @@
 // Steps a1-a4 of the hot path:
 //   k_geometry  a1 level selection (Eq. 6-7), a2 cull + view transform, a3 EWA projection, conic,
-//               tile rect.  A thread owns four consecutive Gaussians (16-byte loads from every SoA plane, all
-//               loads of a phase in flight together); the block stages the records of its visible Gaussians in shared
-//               memory and copies them out, in gid order, dense and coalesced, at the front of its own segment of
-//               the per-frame arrays (no inter-block scan: see WorkspaceDev).  Every visible Gaussian also adds its rect to a 2-D
-//               difference grid of the tile counts (four integer atomics whatever the rect size);
+//               tile rect.  Phase 1: a thread owns four consecutive Gaussians (16-byte loads from the mean
+//               planes), selects, transforms, culls and applies a conservative off-screen test; the block lists the
+//               survivors.  Phase 2: one survivor per thread, all lanes busy, runs the projection; a visible Gaussian
+//               writes its records at the front of the block's segment of the per-frame arrays, in gid order (no
+//               inter-block scan: see WorkspaceDev), and adds its rect to a 2-D difference grid of the tile counts
+//               (four integer atomics whatever the rect size);
 //   k_colour    a4 SH -> RGB, one block per segment; its block 0 runs the tile scan (a5 + a8, tile_scan.cuh).
 //
 // The geometry (a1-a3 and the rect) is the canonical fp32 sequence of DESIGN §2: each operation is one IEEE
@@ -58,51 +59,39 @@ __device__ __forceinline__ void sh_basis(float x, float y, float z, float *Y)
     }
 }
 
-// Shared staging of one block's records, slot = k * kGeoThreads + tid for Gaussian k of thread tid (conflict-free).
-template <bool DEBUG>
+// Shared memory of k_geometry.
 struct GeoSmem {
-    float4 a[kGeoBlock];                              // mu'x, mu'y, k, a2
-    float4 dg[kGeoBlock];                             // mu - c_cam, gid bits
-    float2 b[kGeoBlock];                              // d2, log2 o
-    uint2 rect[kGeoBlock];                            // tx0 | ty0 << 16, tx1 | ty1 << 16
-    uint32_t depth[kGeoBlock];
-    float4 conic_o[DEBUG ? kGeoBlock : 1];            // A, B, C, o (debug records only)
-    unsigned short map[kGeoBlock];                    // block-local compact position -> slot
-    unsigned int warp_vis[kGeoThreads / 32];
+    unsigned short cand[kGeoBlock];                   // candidate slot -> index of the Gaussian inside the block (gid order)
+    unsigned int warp_cnt[kGeoThreads / 32];
+    unsigned int warp_vis[2][kGeoThreads / 32];       // double-buffered over the steps of phase 2
     unsigned int cnt[2];                              // n_sel, n_front of the block
     unsigned long long pairs;
 };
 
 template <bool DEBUG>
-__global__ void __launch_bounds__(kGeoThreads, 3)
+__global__ void __launch_bounds__(kGeoThreads)
 k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ FrameParams p)
 {
-    extern __shared__ __align__(16) unsigned char geo_smem_raw[];
-    GeoSmem<DEBUG> &S = *reinterpret_cast<GeoSmem<DEBUG> *>(geo_smem_raw);
-
+    __shared__ GeoSmem S;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) { S.cnt[0] = 0; S.cnt[1] = 0; S.pairs = 0; }
     const int bid = blockIdx.x;
-    const long long g0 = p.quad_gid + ((long long)bid * kGeoThreads + tid) * kGeoPer;   // multiple of 4
+    const long long gb = p.quad_gid + (long long)bid * kGeoBlock;           // first gid of the block (multiple of 4)
+    const long long g0 = gb + tid * kGeoPer;
     const long long g_end = p.first_gid + p.n_scan;
+    const float *R = p.R;
 
-    // ---- phase 1 loads: mean and kappa of the quad (16-byte loads; the planes are padded to 256 B)
-    float wx[4], wy[4], wz[4], kap[4];
-    const bool quad_live = g0 < g_end && g0 + kGeoPer > p.first_gid;
-    if (quad_live) {
+    // ================= phase 1: a thread owns four consecutive Gaussians (16-byte loads from the mean and rho2 planes)
+    // a1 level selection, a2 view transform and z cull (canonical fp32), then a conservative off-screen test that
+    // needs no covariance.  What survives is a CANDIDATE; the candidates of the block are listed in gid order.
+    unsigned int m_sel = 0, m_front = 0, m_cand = 0;
+    if (g0 < g_end && g0 + kGeoPer > p.first_gid) {
         const float4 X = __ldg(reinterpret_cast<const float4 *>(sc.mx + g0));
         const float4 Y = __ldg(reinterpret_cast<const float4 *>(sc.my + g0));
         const float4 Z = __ldg(reinterpret_cast<const float4 *>(sc.mz + g0));
-        const float4 K = __ldg(reinterpret_cast<const float4 *>(sc.kappa + g0));
-        wx[0] = X.x; wx[1] = X.y; wx[2] = X.z; wx[3] = X.w;
-        wy[0] = Y.x; wy[1] = Y.y; wy[2] = Y.z; wy[3] = Y.w;
-        wz[0] = Z.x; wz[1] = Z.y; wz[2] = Z.z; wz[3] = Z.w;
-        kap[0] = K.x; kap[1] = K.y; kap[2] = K.z; kap[3] = K.w;
-    }
-    const float *R = p.R;
-    unsigned int m_sel = 0, m_front = 0, m_proj = 0;       // bit k: Gaussian k selected / in front / to be projected
-    float px[4], py[4], pz[4];
-    if (quad_live) {
+        const float4 Q = __ldg(reinterpret_cast<const float4 *>(sc.rho2 + g0));
+        const float wx[4] = {X.x, X.y, X.z, X.w}, wy[4] = {Y.x, Y.y, Y.z, Y.w}, wz[4] = {Z.x, Z.y, Z.z, Z.w};
+        const float rho2[4] = {Q.x, Q.y, Q.z, Q.w};
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             const long long g = g0 + k;
@@ -119,173 +108,177 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
             if (!sel) continue;
             m_sel |= 1u << k;
             // ---- a2 (O2): p = R mu + t
-            px[k] = fadd(fadd(fadd(fmul(R[0], wx[k]), fmul(R[1], wy[k])), fmul(R[2], wz[k])), p.t[0]);
-            py[k] = fadd(fadd(fadd(fmul(R[3], wx[k]), fmul(R[4], wy[k])), fmul(R[5], wz[k])), p.t[1]);
-            pz[k] = fadd(fadd(fadd(fmul(R[6], wx[k]), fmul(R[7], wy[k])), fmul(R[8], wz[k])), p.t[2]);
-            if (!(pz[k] > p.z_near)) continue;
+            const float px = fadd(fadd(fadd(fmul(R[0], wx[k]), fmul(R[1], wy[k])), fmul(R[2], wz[k])), p.t[0]);
+            const float py = fadd(fadd(fadd(fmul(R[3], wx[k]), fmul(R[4], wy[k])), fmul(R[5], wz[k])), p.t[1]);
+            const float pz = fadd(fadd(fadd(fmul(R[6], wx[k]), fmul(R[7], wy[k])), fmul(R[8], wz[k])), p.t[2]);
+            if (!(pz > p.z_near)) continue;
             m_front |= 1u << k;
-            if (kap[k] >= 0.0f) m_proj |= 1u << k;           // kappa = -1 marks a dead Gaussian (o < 1/255)
+            if (!(rho2[k] >= 0.0f)) continue;                  // rho2 = -1 marks a dead Gaussian (o < 1/255)
+            // ---- conservative off-screen test.  O4's half extents obey h <= sqrt(kappa (lambda_max |J row|^2 + 0.3))
+            // (1 + 2^-10) + 2^-6 with |J row|^2 <= pre_c1 / z^2 and kappa <= 2 ln 255, so with the margins below
+            // (1 % and one pixel, far above the rounding of this approximate arithmetic) a Gaussian dropped here
+            // would have got an empty tile rect from the exact sequence of phase 2.
+            const float rz = __frcp_rn(pz);
+            const float ax = fmaf(p.fx * px, rz, p.cx), ay = fmaf(p.fy * py, rz, p.cy);
+            const float bnd = sqrtf(fmaf(rho2[k] * p.pre_c1, rz * rz, 3.33f)) * 1.01f + 1.0f + 1e-5f * (fabsf(ax) + fabsf(ay));
+            const bool off = ax + bnd < 0.0f || ax - bnd > (float)(p.TX * kTile) ||
+                             ay + bnd < 0.0f || ay - bnd > (float)(p.TY * kTile);
+            if (!off) m_cand |= 1u << k;                       // (a NaN or infinite bound keeps the Gaussian)
         }
     }
-
-    // ---- phase 2 loads: the six covariance planes, only for quads with something to project
-    float4 S0, S1, S2, S3, S4, S5;
-    if (m_proj) {
-        S0 = __ldg(reinterpret_cast<const float4 *>(sc.cov[0] + g0));
-        S1 = __ldg(reinterpret_cast<const float4 *>(sc.cov[1] + g0));
-        S2 = __ldg(reinterpret_cast<const float4 *>(sc.cov[2] + g0));
-        S3 = __ldg(reinterpret_cast<const float4 *>(sc.cov[3] + g0));
-        S4 = __ldg(reinterpret_cast<const float4 *>(sc.cov[4] + g0));
-        S5 = __ldg(reinterpret_cast<const float4 *>(sc.cov[5] + g0));
-    }
-    float4 L2O = make_float4(0.f, 0.f, 0.f, 0.f), OP = L2O;
-    if (m_proj) {
-        L2O = __ldg(reinterpret_cast<const float4 *>(sc.l2o + g0));
-        if (DEBUG) OP = __ldg(reinterpret_cast<const float4 *>(sc.opacity + g0));
-    }
-
-    unsigned int m_vis = 0, my_pairs = 0;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        if (!((m_proj >> k) & 1u)) continue;
-        const float Sxx = k == 0 ? S0.x : k == 1 ? S0.y : k == 2 ? S0.z : S0.w;
-        const float Sxy = k == 0 ? S1.x : k == 1 ? S1.y : k == 2 ? S1.z : S1.w;
-        const float Sxz = k == 0 ? S2.x : k == 1 ? S2.y : k == 2 ? S2.z : S2.w;
-        const float Syy = k == 0 ? S3.x : k == 1 ? S3.y : k == 2 ? S3.z : S3.w;
-        const float Syz = k == 0 ? S4.x : k == 1 ? S4.y : k == 2 ? S4.z : S4.w;
-        const float Szz = k == 0 ? S5.x : k == 1 ? S5.y : k == 2 ? S5.z : S5.w;
-        const float l2o = k == 0 ? L2O.x : k == 1 ? L2O.y : k == 2 ? L2O.z : L2O.w;
-        const float z = pz[k];
-        const float ix = fdiv(px[k], z), iy = fdiv(py[k], z);
-        const float mx2 = fadd(fmul(p.fx, ix), p.cx);
-        const float my2 = fadd(fmul(p.fy, iy), p.cy);
-        // ---- a3 (O3): J at the clamped point, M = J R, Sigma' = M Sigma M^T + 0.3 I
-        const float u = fminf(fmaxf(ix, -p.limx), p.limx);
-        const float v = fminf(fmaxf(iy, -p.limy), p.limy);
-        const float j00 = fdiv(p.fx, z);
-        const float j02 = -fdiv(fmul(p.fx, u), z);
-        const float j11 = fdiv(p.fy, z);
-        const float j12 = -fdiv(fmul(p.fy, v), z);
-        const float m00 = fadd(fmul(j00, R[0]), fmul(j02, R[6]));
-        const float m01 = fadd(fmul(j00, R[1]), fmul(j02, R[7]));
-        const float m02 = fadd(fmul(j00, R[2]), fmul(j02, R[8]));
-        const float m10 = fadd(fmul(j11, R[3]), fmul(j12, R[6]));
-        const float m11 = fadd(fmul(j11, R[4]), fmul(j12, R[7]));
-        const float m12 = fadd(fmul(j11, R[5]), fmul(j12, R[8]));
-        const float v0x = fadd(fadd(fmul(Sxx, m00), fmul(Sxy, m01)), fmul(Sxz, m02));
-        const float v0y = fadd(fadd(fmul(Sxy, m00), fmul(Syy, m01)), fmul(Syz, m02));
-        const float v0z = fadd(fadd(fmul(Sxz, m00), fmul(Syz, m01)), fmul(Szz, m02));
-        const float v1x = fadd(fadd(fmul(Sxx, m10), fmul(Sxy, m11)), fmul(Sxz, m12));
-        const float v1y = fadd(fadd(fmul(Sxy, m10), fmul(Syy, m11)), fmul(Syz, m12));
-        const float v1z = fadd(fadd(fmul(Sxz, m10), fmul(Syz, m11)), fmul(Szz, m12));
-        const float a = fadd(fadd(fadd(fmul(m00, v0x), fmul(m01, v0y)), fmul(m02, v0z)), 0.3f);
-        const float b = fadd(fadd(fmul(m10, v0x), fmul(m11, v0y)), fmul(m12, v0z));
-        const float c = fadd(fadd(fadd(fmul(m10, v1x), fmul(m11, v1y)), fmul(m12, v1z)), 0.3f);
-        const float det = fsub(fmul(a, c), fmul(b, b));
-        if (!(det > 0.0f)) continue;
-        const float cA = fdiv(c, det), cB = -fdiv(b, det), cC = fdiv(a, det);
-        // ---- O4: padded box of the alpha = 1/255 contour, in 16x16 tiles
-        const float hx = fadd(fmul(__fsqrt_rn(fmul(kap[k], a)), 1.0009765625f), 0.015625f);
-        const float hy = fadd(fmul(__fsqrt_rn(fmul(kap[k], c)), 1.0009765625f), 0.015625f);
-        const float fTX = (float)p.TX, fTY = (float)p.TY;
-        const float x0 = fminf(fmaxf(floorf(fmul(fsub(mx2, hx), 0.0625f)), 0.0f), fTX);
-        const float x1 = fminf(fmaxf(fadd(floorf(fmul(fadd(mx2, hx), 0.0625f)), 1.0f), 0.0f), fTX);
-        const float y0 = fminf(fmaxf(floorf(fmul(fsub(my2, hy), 0.0625f)), 0.0f), fTY);
-        const float y1 = fminf(fmaxf(fadd(floorf(fmul(fadd(my2, hy), 0.0625f)), 1.0f), 0.0f), fTY);
-        const int tx0 = (int)x0, tx1 = (int)x1, ty0 = (int)y0, ty1 = (int)y1;
-        const unsigned int n_tiles = (unsigned int)((tx1 - tx0) * (ty1 - ty0));
-        if (n_tiles == 0) continue;
-        m_vis |= 1u << k;
-        my_pairs += n_tiles;
-        // DESIGN R25: factorised exponent from the ROUNDED conic, derived in fp64, rounded once
-        const double LOG2E = 1.4426950408889634;
-        const double dA = (double)cA, dB = (double)cB, dC = (double)cC;
-        const float kk = (float)(dB / dA);
-        const float a2 = (float)(-0.5 * LOG2E * dA);                   // stored negated: e = log2 o + a2 w^2 + d2 dy^2
-        // <= 0 so that q >= 0 holds by construction in k_blend (the oracle clamps q at 0; a conic left indefinite by
-        // rounding differs from its clamp by less than R25's evaluation error)
-        const float d2 = fminf((float)(-0.5 * LOG2E * (dC - dB * dB / dA)), 0.0f);
-        const int slot = k * kGeoThreads + tid;
-        S.a[slot] = make_float4(mx2, my2, kk, a2);
-        S.b[slot] = make_float2(d2, l2o);
-        S.rect[slot] = make_uint2((unsigned int)tx0 | ((unsigned int)ty0 << 16), (unsigned int)tx1 | ((unsigned int)ty1 << 16));
-        S.depth[slot] = __float_as_uint(z);
-        S.dg[slot] = make_float4(wx[k] - p.centre[0], wy[k] - p.centre[1], wz[k] - p.centre[2],
-                                 __uint_as_float((unsigned int)(g0 + k)));
-        if (DEBUG) S.conic_o[slot] = make_float4(cA, cB, cC, k == 0 ? OP.x : k == 1 ? OP.y : k == 2 ? OP.z : OP.w);
-        // a5, first half: +1 over the rect in the 2-D difference grid of the per-tile pair counts
-#ifndef FLOD_X_NO_GEO_ATOMICS
-        const int gw = p.TX + 1;
-        atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx0) * kCtrStride, 1);
-        atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx1) * kCtrStride, -1);
-        atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx0) * kCtrStride, -1);
-        atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx1) * kCtrStride, 1);
-#endif
-    }
-
-    // ---- block scan of the visible counts (gid order = thread order, then k), block totals of the statistics
-    const unsigned int nv = __popc(m_vis);
-    unsigned int incl = nv;
+    // block scan of the candidate counts (gid order = thread order, then k); block totals of the statistics
+    const unsigned int nc = __popc(m_cand);
+    unsigned int incl = nc;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         const unsigned int t = __shfl_up_sync(0xffffffffu, incl, o);
         if (lane >= o) incl += t;
     }
-    unsigned int ws_sel = __popc(m_sel), ws_front = __popc(m_front), ws_pairs = my_pairs;
+    unsigned int ws_sel = __popc(m_sel), ws_front = __popc(m_front);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         ws_sel += __shfl_xor_sync(0xffffffffu, ws_sel, o);
         ws_front += __shfl_xor_sync(0xffffffffu, ws_front, o);
-        ws_pairs += __shfl_xor_sync(0xffffffffu, ws_pairs, o);
     }
-    if (lane == 31) S.warp_vis[warp] = incl;
+    if (lane == 31) S.warp_cnt[warp] = incl;
     __syncthreads();                                     // S.cnt / S.pairs were zeroed by thread 0
     if (lane == 0) {
         if (ws_sel) atomicAdd(&S.cnt[0], ws_sel);
         if (ws_front) atomicAdd(&S.cnt[1], ws_front);
-        if (ws_pairs) atomicAdd(&S.pairs, (unsigned long long)ws_pairs);
     }
-    __syncthreads();
-    unsigned int local = incl - nv;                      // block-local compact position of the thread's first visible
+    unsigned int local = incl - nc, n_cand = 0;
 #pragma unroll
-    for (int w = 0; w < kGeoThreads / 32; ++w) if (w < warp) local += S.warp_vis[w];
+    for (int w = 0; w < kGeoThreads / 32; ++w) {
+        const unsigned int t = S.warp_cnt[w];
+        if (w < warp) local += t;
+        n_cand += t;
+    }
 #pragma unroll
     for (int k = 0; k < 4; ++k)
-        if ((m_vis >> k) & 1u) S.map[local++] = (unsigned short)(k * kGeoThreads + tid);
-    unsigned int total = 0;
+        if ((m_cand >> k) & 1u) S.cand[local++] = (unsigned short)(tid * kGeoPer + k);
+    __syncthreads();
+
+    // ================= phase 2: one candidate per thread and step, all lanes busy.  a3 EWA projection, conic, tile
+    // rect: the canonical fp32 sequence of DESIGN §2 (p is recomputed from the mean by the same operations as in
+    // phase 1, so it has the same bits).  A visible Gaussian writes its records straight to the block's segment, at
+    // the position a ballot scan gives it: gid order is kept because the candidate list is in gid order.
+    const unsigned int seg_base = (unsigned int)bid * kGeoBlock;
+    unsigned int n_vis_before = 0, my_pairs = 0;
+    for (unsigned int s0 = 0, step = 0; s0 < n_cand; s0 += kGeoThreads, ++step) {
+        const unsigned int s = s0 + tid;
+        bool vis = false;
+        float mx2 = 0.f, my2 = 0.f, z = 0.f, cA = 0.f, cB = 0.f, cC = 0.f, l2o = 0.f, wxk = 0.f, wyk = 0.f, wzk = 0.f;
+        int tx0 = 0, tx1 = 0, ty0 = 0, ty1 = 0;
+        long long g = 0;
+        if (s < n_cand) {
+            g = gb + S.cand[s];
+            wxk = __ldg(sc.mx + g); wyk = __ldg(sc.my + g); wzk = __ldg(sc.mz + g);
+            const float kap = __ldg(sc.kappa + g);
+            const float Sxx = __ldg(sc.cov[0] + g), Sxy = __ldg(sc.cov[1] + g), Sxz = __ldg(sc.cov[2] + g);
+            const float Syy = __ldg(sc.cov[3] + g), Syz = __ldg(sc.cov[4] + g), Szz = __ldg(sc.cov[5] + g);
+            l2o = __ldg(sc.l2o + g);
+            const float px = fadd(fadd(fadd(fmul(R[0], wxk), fmul(R[1], wyk)), fmul(R[2], wzk)), p.t[0]);
+            const float py = fadd(fadd(fadd(fmul(R[3], wxk), fmul(R[4], wyk)), fmul(R[5], wzk)), p.t[1]);
+            z = fadd(fadd(fadd(fmul(R[6], wxk), fmul(R[7], wyk)), fmul(R[8], wzk)), p.t[2]);
+            const float ix = fdiv(px, z), iy = fdiv(py, z);
+            mx2 = fadd(fmul(p.fx, ix), p.cx);
+            my2 = fadd(fmul(p.fy, iy), p.cy);
+            // ---- a3 (O3): J at the clamped point, M = J R, Sigma' = M Sigma M^T + 0.3 I
+            const float u = fminf(fmaxf(ix, -p.limx), p.limx);
+            const float v = fminf(fmaxf(iy, -p.limy), p.limy);
+            const float j00 = fdiv(p.fx, z);
+            const float j02 = -fdiv(fmul(p.fx, u), z);
+            const float j11 = fdiv(p.fy, z);
+            const float j12 = -fdiv(fmul(p.fy, v), z);
+            const float m00 = fadd(fmul(j00, R[0]), fmul(j02, R[6]));
+            const float m01 = fadd(fmul(j00, R[1]), fmul(j02, R[7]));
+            const float m02 = fadd(fmul(j00, R[2]), fmul(j02, R[8]));
+            const float m10 = fadd(fmul(j11, R[3]), fmul(j12, R[6]));
+            const float m11 = fadd(fmul(j11, R[4]), fmul(j12, R[7]));
+            const float m12 = fadd(fmul(j11, R[5]), fmul(j12, R[8]));
+            const float v0x = fadd(fadd(fmul(Sxx, m00), fmul(Sxy, m01)), fmul(Sxz, m02));
+            const float v0y = fadd(fadd(fmul(Sxy, m00), fmul(Syy, m01)), fmul(Syz, m02));
+            const float v0z = fadd(fadd(fmul(Sxz, m00), fmul(Syz, m01)), fmul(Szz, m02));
+            const float v1x = fadd(fadd(fmul(Sxx, m10), fmul(Sxy, m11)), fmul(Sxz, m12));
+            const float v1y = fadd(fadd(fmul(Sxy, m10), fmul(Syy, m11)), fmul(Syz, m12));
+            const float v1z = fadd(fadd(fmul(Sxz, m10), fmul(Syz, m11)), fmul(Szz, m12));
+            const float a = fadd(fadd(fadd(fmul(m00, v0x), fmul(m01, v0y)), fmul(m02, v0z)), 0.3f);
+            const float b = fadd(fadd(fmul(m10, v0x), fmul(m11, v0y)), fmul(m12, v0z));
+            const float c = fadd(fadd(fadd(fmul(m10, v1x), fmul(m11, v1y)), fmul(m12, v1z)), 0.3f);
+            const float det = fsub(fmul(a, c), fmul(b, b));
+            if (det > 0.0f) {
+                cA = fdiv(c, det); cB = -fdiv(b, det); cC = fdiv(a, det);
+                // ---- O4: padded box of the alpha = 1/255 contour, in 16x16 tiles
+                const float hx = fadd(fmul(__fsqrt_rn(fmul(kap, a)), 1.0009765625f), 0.015625f);
+                const float hy = fadd(fmul(__fsqrt_rn(fmul(kap, c)), 1.0009765625f), 0.015625f);
+                const float fTX = (float)p.TX, fTY = (float)p.TY;
+                const float x0 = fminf(fmaxf(floorf(fmul(fsub(mx2, hx), 0.0625f)), 0.0f), fTX);
+                const float x1 = fminf(fmaxf(fadd(floorf(fmul(fadd(mx2, hx), 0.0625f)), 1.0f), 0.0f), fTX);
+                const float y0 = fminf(fmaxf(floorf(fmul(fsub(my2, hy), 0.0625f)), 0.0f), fTY);
+                const float y1 = fminf(fmaxf(fadd(floorf(fmul(fadd(my2, hy), 0.0625f)), 1.0f), 0.0f), fTY);
+                tx0 = (int)x0; tx1 = (int)x1; ty0 = (int)y0; ty1 = (int)y1;
+                vis = (tx1 - tx0) * (ty1 - ty0) > 0;
+            }
+        }
+        // ---- position of the visible ones: ballot inside the warp, warp totals through shared memory
+        const unsigned int bal = __ballot_sync(0xffffffffu, vis);
+        if (lane == 0) S.warp_vis[step & 1][warp] = __popc(bal);
+        __syncthreads();
+        unsigned int pos = n_vis_before + __popc(bal & ((1u << lane) - 1)), step_total = 0;
 #pragma unroll
-    for (int w = 0; w < kGeoThreads / 32; ++w) total += S.warp_vis[w];
+        for (int w = 0; w < kGeoThreads / 32; ++w) {
+            const unsigned int t = S.warp_vis[step & 1][w];
+            if (w < warp) pos += t;
+            step_total += t;
+        }
+        n_vis_before += step_total;
+        if (vis) {
+            my_pairs += (unsigned int)((tx1 - tx0) * (ty1 - ty0));
+            // DESIGN R25: factorised exponent from the ROUNDED conic, derived in fp64, rounded once
+            const double LOG2E = 1.4426950408889634;
+            const double dA = (double)cA, dB = (double)cB, dC = (double)cC;
+            const double rA = 1.0 / dA;
+            const float kk = (float)(dB * rA);
+            const float a2 = (float)(-0.5 * LOG2E * dA);               // stored negated: e = log2 o + a2 w^2 + d2 dy^2
+            // <= 0 so that q >= 0 holds by construction in k_blend (the oracle clamps q at 0; a conic left indefinite by
+            // rounding differs from its clamp by less than R25's evaluation error)
+            const float d2 = fminf((float)(-0.5 * LOG2E * (dC - dB * dB * rA)), 0.0f);
+            const size_t c = (size_t)seg_base + pos;
+            ws.gA[c] = make_float4(mx2, my2, kk, a2);
+            reinterpret_cast<float2 *>(ws.gB)[2 * c] = make_float2(d2, l2o);          // (r, g) by k_colour
+            ws.rect[c] = make_ushort4((unsigned short)tx0, (unsigned short)ty0, (unsigned short)tx1, (unsigned short)ty1);
+            ws.depth[c] = __float_as_uint(z);
+            ws.dirgid[c] = make_float4(wxk - p.centre[0], wyk - p.centre[1], wzk - p.centre[2], __uint_as_float((unsigned int)g));
+            if (DEBUG) {
+                flod_dbg_projected d;
+                d.gid = (unsigned int)g; d.mu2d[0] = mx2; d.mu2d[1] = my2; d.depth = z;
+                d.conic[0] = cA; d.conic[1] = cB; d.conic[2] = cC; d.opacity = __ldg(sc.opacity + g);
+                d.rgb[0] = 0.0f; d.rgb[1] = 0.0f; d.rgb[2] = 0.0f;                                // by k_colour
+                d.rect[0] = tx0; d.rect[1] = ty0; d.rect[2] = tx1; d.rect[3] = ty1;
+                ws.dbg[c] = d;
+            }
+            // a5, first half: +1 over the rect in the 2-D difference grid of the per-tile pair counts
+#ifndef FLOD_X_NO_GEO_ATOMICS
+            const int gw = p.TX + 1;
+            atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx0) * kCtrStride, 1);
+            atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx1) * kCtrStride, -1);
+            atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx0) * kCtrStride, -1);
+            atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx1) * kCtrStride, 1);
+#endif
+        }
+    }
+    // ---- block totals
+    unsigned int ws_pairs = my_pairs;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) ws_pairs += __shfl_xor_sync(0xffffffffu, ws_pairs, o);
+    if (lane == 0 && ws_pairs) atomicAdd(&S.pairs, (unsigned long long)ws_pairs);
     __syncthreads();
     if (tid == 0) {
-        ws.seg_count[bid] = total;
-        if (total) atomicAdd(&ws.hdr->n_vis32, total);
+        ws.seg_count[bid] = n_vis_before;
+        if (n_vis_before) atomicAdd(&ws.hdr->n_vis32, n_vis_before);
         if (S.cnt[0]) atomicAdd(&ws.hdr->n_sel, (unsigned long long)S.cnt[0]);
         if (S.cnt[1]) atomicAdd(&ws.hdr->n_front, (unsigned long long)S.cnt[1]);
         if (S.pairs) atomicAdd(&ws.hdr->n_pairs, S.pairs);
-    }
-
-    // ---- copy-out: the block's visible records, dense and coalesced, at the front of the block's segment
-    const unsigned int base = (unsigned int)bid * kGeoBlock;
-    for (unsigned int j = tid; j < total; j += kGeoThreads) {
-        const int slot = S.map[j];
-        const size_t c = (size_t)base + j;
-        ws.gA[c] = S.a[slot];
-        reinterpret_cast<float2 *>(ws.gB)[2 * c] = S.b[slot];          // (r, g) by k_colour
-        const uint2 rc = S.rect[slot];
-        ws.rect[c] = make_ushort4((unsigned short)(rc.x & 0xffffu), (unsigned short)(rc.x >> 16),
-                                  (unsigned short)(rc.y & 0xffffu), (unsigned short)(rc.y >> 16));
-        ws.depth[c] = S.depth[slot];
-        ws.dirgid[c] = S.dg[slot];
-        if (DEBUG) {
-            const float4 a = S.a[slot], co = S.conic_o[slot];
-            flod_dbg_projected d;
-            d.gid = __float_as_uint(S.dg[slot].w); d.mu2d[0] = a.x; d.mu2d[1] = a.y; d.depth = __uint_as_float(S.depth[slot]);
-            d.conic[0] = co.x; d.conic[1] = co.y; d.conic[2] = co.z; d.opacity = co.w;
-            d.rgb[0] = 0.0f; d.rgb[1] = 0.0f; d.rgb[2] = 0.0f;                                // by k_colour
-            d.rect[0] = (int)(rc.x & 0xffffu); d.rect[1] = (int)(rc.x >> 16);
-            d.rect[2] = (int)(rc.y & 0xffffu); d.rect[3] = (int)(rc.y >> 16);
-            ws.dbg[c] = d;
-        }
     }
 }
 
@@ -365,14 +358,8 @@ k_colour(const SceneDev sc, const WorkspaceDev ws, int TX, int TY, unsigned int 
 int launch_geometry(const Context &c, const FrameParams &p, cudaStream_t s)
 {
     if (p.n_pre_blocks <= 0) return 0;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(k_geometry<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GeoSmem<true>));
-        cudaFuncSetAttribute(k_geometry<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GeoSmem<false>));
-        attr_set = true;
-    }
-    if (c.flags & FLOD_OPT_DEBUG) k_geometry<true><<<p.n_pre_blocks, kGeoThreads, sizeof(GeoSmem<true>), s>>>(c.scene, c.ws, p);
-    else k_geometry<false><<<p.n_pre_blocks, kGeoThreads, sizeof(GeoSmem<false>), s>>>(c.scene, c.ws, p);
+    if (c.flags & FLOD_OPT_DEBUG) k_geometry<true><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(c.scene, c.ws, p);
+    else k_geometry<false><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(c.scene, c.ws, p);
     return 1;
 }
 
