@@ -46,6 +46,18 @@ __device__ __forceinline__ void cp_async4(void *smem, const void *gmem)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
+// alpha if alpha >= 1/255 and T >= 1e-4, else 0 (FSETP, FSETP.AND, FSEL)
+__device__ __forceinline__ float keep_if_live(float alpha, float T)
+{
+    float r;
+    asm("{\n\t.reg .pred p, q;\n\t"
+        "setp.ge.f32 q, %2, 0f38D1B717;\n\t"            // 1e-4f
+        "setp.ge.and.f32 p, %1, 0f3B808081, q;\n\t"     // (float)(1/255)
+        "selp.f32 %0, %1, 0f00000000, p;\n\t}"
+        : "=f"(r) : "f"(alpha), "f"(T));
+    return r;
+}
+
 // 2^x on the MUFU unit (x <= 0 here; results below 2^-126 flush to 0, far under the 1/255 skip threshold)
 __device__ __forceinline__ float ex2(float x)
 {
@@ -54,6 +66,10 @@ __device__ __forceinline__ float ex2(float x)
     return y;
 }
 
+#ifndef FLOD_BLEND_UNROLL
+#define FLOD_BLEND_UNROLL 4
+#endif
+constexpr int kBlendUnroll = FLOD_BLEND_UNROLL;     // `#pragma unroll` takes a constant expression, not a macro
 #ifndef FLOD_BLEND_MINBLOCKS
 #define FLOD_BLEND_MINBLOCKS 8
 #endif
@@ -91,33 +107,27 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
 
     // two pixels per thread, packed as float2 (.x = row py0, .y = row py1): the per-pixel arithmetic runs on the
     // packed FP32 instructions of sm_100 (FADD2 / FMUL2 / FFMA2: one issue slot for both pixels)
-    float2 T = make_float2(1.0f, 1.0f), cr = make_float2(0.0f, 0.0f), cg = cr, cb2 = cr;
+    float2 T = make_float2(in0 ? 1.0f : 0.0f, in1 ? 1.0f : 0.0f), cr = make_float2(0.0f, 0.0f), cg = cr, cb2 = cr;
     unsigned int n_eval = 0, n_blend = 0;
     float4 *my_buf = s_buf[warp];
     const float4 *my_half = my_buf + half;
-    // pixels outside the image: thr = +huge, so that no alpha passes the skip test (inside: thr = 1/255)
-    const float thr0 = in0 ? (1.0f / 255.0f) : 3.0e38f, thr1 = in1 ? (1.0f / 255.0f) : 3.0e38f;
-    bool warp_done = __all_sync(0xffffffffu, !in0 && !in1);
+    bool warp_done = __all_sync(0xffffffffu, !in0 && !in1);         // pixels outside the image start with T = 0
 
     // evaluates my_buf[0, cnt) on the thread's two pixels.  a2 <= 0 and e0 <= log2 o (k_geometry clamps d2), so
     // q >= 0 holds by construction and alpha needs the 0.99 clamp only.  A pixel that is done or below 1/255 blends 0.
     auto evaluate = [&](unsigned int cnt, unsigned int base_in_list) {
-#pragma unroll 2
+#pragma unroll kBlendUnroll
         for (unsigned int t = 0; t < cnt; ++t) {
             const float4 hrec = my_half[3 * t];
             const float4 c = my_buf[3 * t + 2];
             const float2 w = __fadd2_rn(make_float2(hrec.x, hrec.y), make_float2(nlx, nlx));
             const float2 e = __ffma2_rn(make_float2(c.x, c.x), __fmul2_rn(w, w), make_float2(hrec.z, hrec.w));
             float al0 = fminf(ex2(e.x), 0.99f), al1 = fminf(ex2(e.y), 0.99f);
-            // skip below 1/255 (R11); a pixel that has stopped (T < 1e-4 after an earlier blend, R12) blends nothing.
-            // The test reads T directly: the loop-carried chain is T -> compare -> select -> multiply -> subtract.
-#ifndef FLOD_X_BLEND_STOP_MASK
-            al0 = (al0 >= thr0 && T.x >= 1e-4f) ? al0 : 0.0f;
-            al1 = (al1 >= thr1 && T.y >= 1e-4f) ? al1 : 0.0f;
-#else
-            al0 = al0 >= fmaxf(thr0, (1e-4f - T.x) * 1.2676506002282294e30f) ? al0 : 0.0f;
-            al1 = al1 >= fmaxf(thr1, (1e-4f - T.y) * 1.2676506002282294e30f) ? al1 : 0.0f;
-#endif
+            // skip below 1/255 (R11); a pixel that has stopped (T < 1e-4 after an earlier blend, R12) or lies outside
+            // the image (T = 0 from the start) blends nothing.  The test reads T directly, so the loop-carried chain is
+            // T -> compare -> select -> multiply -> subtract; one predicate per pixel carries both conditions.
+            al0 = keep_if_live(al0, T.x);
+            al1 = keep_if_live(al1, T.y);
             const float2 wgt = __fmul2_rn(T, make_float2(al0, al1));
             cr = __ffma2_rn(wgt, make_float2(c.y, c.y), cr);
             cg = __ffma2_rn(wgt, make_float2(c.z, c.z), cg);
@@ -211,13 +221,13 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
                 __syncwarp();
                 evaluate(cnt, base - rg.x);
                 cnt = 0;
-                warp_done = __all_sync(0xffffffffu, (!in0 || T.x < 1e-4f) && (!in1 || T.y < 1e-4f));
+                warp_done = __all_sync(0xffffffffu, T.x < 1e-4f && T.y < 1e-4f);
                 if (warp_done) break;
                 __syncwarp();
             }
         }
     }
-    const bool done0 = !in0 || T.x < 1e-4f, done1 = !in1 || T.y < 1e-4f;
+    const bool done0 = T.x < 1e-4f, done1 = T.y < 1e-4f;
     const float T0 = T.x, T1 = T.y, r0 = cr.x, r1 = cr.y, g0 = cg.x, g1 = cg.y, b0 = cb2.x, b1 = cb2.y;
     const size_t plane = (size_t)W * H;
     if (in0) {
