@@ -168,6 +168,38 @@ FLOD_API int flod_render_to_host_async(flod_ctx *ctx, const flod_camera *cam, fl
 /* Blocks the calling host thread until every copy issued by flod_render_to_host_async has landed. */
 FLOD_API int flod_wait_host(flod_ctx *ctx);
 
+/* ---- Materialised G_sel (Eq. 6) reused over a run of frames and rebuilt in the background, the paper's
+ * runtime for long trajectories: "G_sel ... is updated every 50 views" on a second thread.  A SNAPSHOT
+ * is the stable (gid-order) compaction of the Gaussians of the level range that pass Eq. 6 for ONE reference
+ * position (R2's "position at the last rebuild"; P:681's average training camera is the same call with that
+ * position).  The subset arena holds two snapshots: frames are rendered from the FRONT one while the BACK one is
+ * rebuilt on another stream; flod_subset_swap exchanges them between two frames.  A frame rendered from a snapshot
+ * equals flod_render with flod_set_selection_reference(ref_pos) and the same fx and gamma, bit for bit. ---- */
+
+/* Bytes of a subset arena for the level range `mode` (two snapshots, each sized for every Gaussian of the range:
+ * 60 B per Gaussian and snapshot; SH rows stay in the scene arena).  0 on invalid input or before upload. */
+FLOD_API size_t flod_subset_bytes(const flod_ctx *ctx, flod_level_mode mode);
+
+/* Hand the subset arena (256-byte aligned device pointer, caller-owned) to the context and fix the level range. */
+FLOD_API int flod_subset_set_arena(flod_ctx *ctx, void *arena_dev, size_t bytes, flod_level_mode mode);
+
+/* Enqueue on `stream` the rebuild of the BACK snapshot: Eq. 6-7 with d_G = |mu - ref_pos| (fp32, as O1), thresholds
+ * d_proj^(l) = s_min^(l) fx / gamma computed in fp64 and rounded once; selected Gaussians are copied in gid order.
+ * Returns without waiting; `stream` may differ from the render stream (the library orders the rebuild after the last
+ * frame that read the back snapshot).  FLOD_E_INVALID_ARG for a non-finite position, fx <= 0 or gamma <= 0. */
+FLOD_API int flod_subset_build(flod_ctx *ctx, const float ref_pos[3], float fx, float gamma, void *stream);
+
+/* 1 if the enqueued rebuild has completed (flod_subset_swap would not block), 0 if not, negative on error. */
+FLOD_API int flod_subset_ready(flod_ctx *ctx);
+
+/* Waits (host) for the rebuild, then makes the back snapshot the front one.  *n_selected (may be NULL) receives its
+ * size N_sel.  FLOD_E_INVALID_ARG if no rebuild was enqueued since the last swap. */
+FLOD_API int flod_subset_swap(flod_ctx *ctx, int64_t *n_selected);
+
+/* flod_render from the FRONT snapshot: steps a2-a9 over its N_sel Gaussians (a1 was done by the rebuild).  The
+ * camera's fx should be the one the snapshot was built with (Eq. 7); this is not checked. */
+FLOD_API int flod_render_subset(flod_ctx *ctx, const flod_camera *cam, float *out_rgb_dev, void *stream);
+
 /* Waits for the last frame's stream, then reports its counters (and FLOD_E_CAPACITY if it overflowed). */
 FLOD_API int flod_get_stats(flod_ctx *ctx, flod_stats *out);
 

@@ -92,6 +92,13 @@ def load_library():
     L.flod_render_to_host.argtypes = [vp, C.POINTER(CameraStruct), LevelMode, C.c_float, vp, vp]
     L.flod_render_to_host_async.argtypes = [vp, C.POINTER(CameraStruct), LevelMode, C.c_float, vp, vp, vp]
     L.flod_wait_host.argtypes = [vp]
+    L.flod_subset_bytes.restype = sz
+    L.flod_subset_bytes.argtypes = [vp, LevelMode]
+    L.flod_subset_set_arena.argtypes = [vp, vp, sz, LevelMode]
+    L.flod_subset_build.argtypes = [vp, C.POINTER(C.c_float), C.c_float, C.c_float, vp]
+    L.flod_subset_ready.argtypes = [vp]
+    L.flod_subset_swap.argtypes = [vp, C.POINTER(i64)]
+    L.flod_render_subset.argtypes = [vp, C.POINTER(CameraStruct), vp, vp]
     L.flod_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.flod_debug_copy.argtypes = [vp, C.c_int, vp, sz]
     L.flod_launches_per_frame.argtypes = [vp]
@@ -223,6 +230,39 @@ class Renderer:
 
     def wait_host(self):
         self._check(self.lib.flod_wait_host(self._h))
+
+    # ---- materialised G_sel: flod_subset_bytes + flod_subset_set_arena, flod_subset_build / ready / swap, flod_render_subset
+    def subset_set_arena(self, l_start: int, l_end: int):
+        nbytes = self.lib.flod_subset_bytes(self._h, LevelMode(l_start, l_end))
+        if nbytes == 0:
+            raise FlodError(-2, "flod_subset_bytes rejected the level range (or no scene uploaded)")
+        self.subset_arena = self._torch.empty(nbytes, dtype=self._torch.uint8, device=self.device)
+        self._check(self.lib.flod_subset_set_arena(self._h, C.c_void_p(self.subset_arena.data_ptr()), nbytes,
+                                                   LevelMode(l_start, l_end)))
+        return nbytes
+
+    def subset_build(self, ref_pos, fx: float, gamma: float, stream=None):
+        arr = (C.c_float * 3)(*[float(np.float32(v)) for v in ref_pos])
+        st = self._stream() if stream is None else C.c_void_p(stream.cuda_stream)
+        self._check(self.lib.flod_subset_build(self._h, arr, float(fx), float(gamma), st))
+
+    def subset_ready(self) -> bool:
+        rc = self.lib.flod_subset_ready(self._h)
+        if rc < 0:
+            self._check(rc)
+        return rc == 1
+
+    def subset_swap(self) -> int:
+        n = C.c_int64(0)
+        self._check(self.lib.flod_subset_swap(self._h, C.byref(n)))
+        return n.value
+
+    def render_subset(self, cam, out=None):
+        cs = cam if isinstance(cam, CameraStruct) else camera_struct(cam)
+        if out is None:
+            out = self._torch.empty((3, cs.height, cs.width), dtype=self._torch.float32, device=self.device)
+        self._check(self.lib.flod_render_subset(self._h, C.byref(cs), C.c_void_p(out.data_ptr()), self._stream()))
+        return out
 
     def launches_per_frame(self) -> int:
         return self.lib.flod_launches_per_frame(self._h)

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libflod.so")
-SOURCES = ["flod_api.cu", "preprocess.cu", "binning.cu", "tile_sort.cu", "blend.cu"]
+SOURCES = ["flod_api.cu", "preprocess.cu", "binning.cu", "tile_sort.cu", "blend.cu", "subset.cu"]
 HEADERS = [os.path.join(CSRC, "flod_internal.cuh"), os.path.join(HERE, "..", "include", "flod.h")]
 
 NVCC_FLAGS = [

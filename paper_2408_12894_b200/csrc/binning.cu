@@ -13,7 +13,7 @@ namespace flod {
 // ------------------------------------------------------------------------------------------------ a6
 // One block per segment of k_geometry (up to kGeoBlock visible Gaussians, four per thread).  The kernel is bound by the
 // throughput of value-returning global atomics on scattered addresses (about 5 cycles per lane and SM, measured:
-// profiles/r1f_notes.md), so it issues as few as possible: the append counters of a 2x2 GROUP of tiles are one float4
+// profiles/r1h_launches.md), so it issues as few as possible: the append counters of a 2x2 GROUP of tiles are one float4
 // and one ATOMG.ADD.F32x4 reserves a slot in each of the (up to four) tiles of the group that the rect covers.  The
 // counters are relative to the tile's range start and exact as floats below 2^24 (k_colour's tile scan raises the
 // capacity flag for a longer list).  A block scan of the per-Gaussian group counts lets the block expand its rects

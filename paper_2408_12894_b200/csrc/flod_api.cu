@@ -149,6 +149,9 @@ int flod_create(flod_ctx **out, int device)
         return FLOD_E_CUDA;
     }
     for (auto &ev : c->ev) cudaEventCreate(&ev);
+    cudaEventCreateWithFlags(&c->ev_sub_built, cudaEventDisableTiming);
+    for (auto &ev : c->ev_sub_read) cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+    if (cudaHostAlloc((void **)&c->sub_n_host, 64, cudaHostAllocDefault) != cudaSuccess) { delete c; return FLOD_E_CUDA; }
     for (int i = 0; i < 2; ++i) {
         cudaEventCreateWithFlags(&c->ev_rendered[i], cudaEventDisableTiming);
         cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming);
@@ -161,6 +164,9 @@ int flod_destroy(flod_ctx *ctx)
 {
     if (!ctx) return FLOD_E_INVALID_ARG;
     for (auto &ev : ctx->ev) if (ev) cudaEventDestroy(ev);
+    if (ctx->ev_sub_built) cudaEventDestroy(ctx->ev_sub_built);
+    for (auto &ev : ctx->ev_sub_read) if (ev) cudaEventDestroy(ev);
+    if (ctx->sub_n_host) cudaFreeHost(ctx->sub_n_host);
     for (int i = 0; i < 2; ++i) {
         if (ctx->ev_rendered[i]) cudaEventDestroy(ctx->ev_rendered[i]);
         if (ctx->ev_copied[i]) cudaEventDestroy(ctx->ev_copied[i]);
@@ -271,7 +277,7 @@ int flod_upload_levels(flod_ctx *ctx, int n_levels, const flod_level_desc *level
     ctx->scene.sh = P(kScenePlanes);
     ctx->scene.sh_stride = stride; ctx->scene.sh_degree = sh_degree;
     ctx->arena = scene_arena_dev;
-    ctx->uploaded = true; ctx->has_ws = false; ctx->rendered = false;
+    ctx->uploaded = true; ctx->has_ws = false; ctx->rendered = false; ctx->has_subset = false;
     return FLOD_OK;
 }
 
@@ -325,13 +331,16 @@ int flod_launches_per_frame(const flod_ctx *ctx)
     return 5;   // geometry, colour (+ tile scan in its block 0), duplication, tile sort, blend
 }
 
-int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, float *out_rgb_dev, void *stream)
+}  // extern "C"
+
+namespace {
+
+// host-side checks shared by flod_render and flod_render_subset
+int check_frame_args(flod_ctx *ctx, const flod_camera *cam, const float *out_rgb_dev)
 {
-    if (!ctx) return FLOD_E_INVALID_ARG;
     if (!cam || !out_rgb_dev) return fail(ctx, FLOD_E_INVALID_ARG, "render: null pointer");
     if (!ctx->uploaded) return fail(ctx, FLOD_E_NOT_UPLOADED, "render: no scene uploaded");
     if (!ctx->has_ws) return fail(ctx, FLOD_E_NO_WORKSPACE, "render: no workspace set");
-    if (!(gamma > 0.0f) || !isfinite(gamma)) return fail(ctx, FLOD_E_INVALID_ARG, "render: gamma must be finite and > 0");
     if (!(cam->fx > 0.0f) || !(cam->fy > 0.0f) || !isfinite(cam->fx) || !isfinite(cam->fy) || cam->width < 1 || cam->height < 1)
         return fail(ctx, FLOD_E_INVALID_ARG, "render: fx, fy must be > 0 and width, height >= 1");
     if (!(cam->z_near >= 0.0f) || !isfinite(cam->z_near)) return fail(ctx, FLOD_E_INVALID_ARG, "render: z_near must be >= 0");
@@ -340,47 +349,50 @@ int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, flo
     for (int i = 0; i < 9; ++i) if (!isfinite(cam->R[i])) return fail(ctx, FLOD_E_INVALID_ARG, "render: non-finite R");
     for (int i = 0; i < 3; ++i) if (!isfinite(cam->t[i]) || !isfinite(cam->bg[i])) return fail(ctx, FLOD_E_INVALID_ARG, "render: non-finite t / bg");
     if (!isfinite(cam->cx) || !isfinite(cam->cy)) return fail(ctx, FLOD_E_INVALID_ARG, "render: non-finite principal point");
-    const int last_level = ctx->first_level + ctx->n_levels - 1;
-    if (mode.l_start < ctx->first_level || mode.l_end > last_level || mode.l_start > mode.l_end)
-        return fail(ctx, FLOD_E_LEVEL_RANGE, "render: need first_level <= l_start <= l_end <= last_level");
+    return FLOD_OK;
+}
 
-    FrameParams p{};
+// camera half of the per-frame constants: fp64, rounded once
+void camera_params(FrameParams &p, const flod_camera *cam)
+{
     memcpy(p.R, cam->R, sizeof(p.R)); memcpy(p.t, cam->t, sizeof(p.t)); memcpy(p.bg, cam->bg, sizeof(p.bg));
     p.fx = cam->fx; p.fy = cam->fy; p.cx = cam->cx; p.cy = cam->cy; p.z_near = cam->z_near;
     p.W = cam->width; p.H = cam->height;
     p.TX = (p.W + kTile - 1) / kTile; p.TY = (p.H + kTile - 1) / kTile;
-    // per-frame constants: fp64, rounded once
     for (int i = 0; i < 3; ++i)
         p.centre[i] = (float)(-(((double)cam->R[i] * (double)cam->t[0] + (double)cam->R[3 + i] * (double)cam->t[1]) +
                                 (double)cam->R[6 + i] * (double)cam->t[2]));
-    for (int i = 0; i < 3; ++i) p.ref[i] = ctx->has_ref ? ctx->ref[i] : p.centre[i];
     p.limx = (float)(1.3 * (double)cam->width / (2.0 * (double)cam->fx));
     p.limy = (float)(1.3 * (double)cam->height / (2.0 * (double)cam->fy));
     {   // conservative off-screen test of k_geometry: |row of J|^2 <= pre_c1 / z^2 (R8's clamp bounds u and v)
         const double fm = std::max((double)cam->fx, (double)cam->fy), lm = std::max((double)p.limx, (double)p.limy);
         p.pre_c1 = (float)(fm * fm * (1.0 + lm * lm) * 1.0001);
     }
-    const int i0 = mode.l_start - ctx->first_level, i1 = mode.l_end - ctx->first_level;   // level positions
-    p.n_levels = i1 - i0 + 1;
-    p.first_gid = ctx->level_off[i0];
-    const int64_t n_scan = ctx->level_off[i1 + 1] - ctx->level_off[i0];
-    p.n_scan = (int)n_scan;
+    p.n_tiles = p.TX * p.TY;
+}
+
+// Eq. 7 thresholds of the level positions i0..i1 (squared, fp64 -> fp32 once): lo2[k], hi2[k], level_end[k]
+void band_params(const flod_ctx *ctx, int i0, int i1, float fx, float gamma, int *level_end, float *lo2, float *hi2)
+{
     for (int l = i0; l <= i1; ++l) {
         const int k = l - i0;
-        p.level_end[k] = (int)(ctx->level_off[l + 1] - ctx->level_off[i0]);
-        if (l == i1) p.lo2[k] = 0.0f;                                   // d_proj^(L_end) = 0
+        level_end[k] = (int)(ctx->level_off[l + 1] - ctx->level_off[i0]);
+        if (l == i1) lo2[k] = 0.0f;                                     // d_proj^(L_end) = 0
         else {
-            const double d = (double)ctx->s_min[l] * (double)cam->fx / (double)gamma;   // Eq. 7
-            p.lo2[k] = (float)(d * d);
+            const double d = (double)ctx->s_min[l] * (double)fx / (double)gamma;   // Eq. 7
+            lo2[k] = (float)(d * d);
         }
     }
-    for (int k = 0; k < p.n_levels; ++k) p.hi2[k] = (k == 0) ? INFINITY : p.lo2[k - 1];  // d_proj^(L_start-1) = inf
+    for (int k = 0; k <= i1 - i0; ++k) hi2[k] = (k == 0) ? INFINITY : lo2[k - 1];  // d_proj^(L_start-1) = inf
+}
+
+// memset + the five kernels of a frame over `sc` (the scene, or a snapshot of it)
+int enqueue_frame(flod_ctx *ctx, const SceneDev &sc, FrameParams &p, float *out_rgb_dev, cudaStream_t s)
+{
+    const int64_t n_scan = p.n_scan;
     p.max_pairs = (unsigned int)ctx->max_pairs;
     p.quad_gid = p.first_gid & ~3ll;
     p.n_pre_blocks = (int)((p.first_gid - p.quad_gid + n_scan + kGeoBlock - 1) / kGeoBlock);
-    p.n_tiles = p.TX * p.TY;
-
-    cudaStream_t s = (cudaStream_t)stream;
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     const bool prof = ctx->flags & FLOD_OPT_PROFILE;
     // zero the header and the tile difference grid (contiguous in the workspace)
@@ -391,7 +403,7 @@ int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, flo
         CUDA_TRY(ctx, cudaMemsetAsync(ctx->ws.mask, 0, (size_t)std::max<int64_t>(ctx->n_total, 1), s));
     int stage = 0;
     auto mark = [&]() { if (prof) cudaEventRecord(ctx->ev[stage], s); ++stage; };
-    mark(); launch_geometry(*ctx, p, s);
+    mark(); launch_geometry(*ctx, sc, p, s);
     mark(); launch_colour(*ctx, p, s);
     mark(); launch_duplicate(*ctx, p, s);
     mark(); launch_tile_sort(*ctx, p, s);
@@ -403,6 +415,29 @@ int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, flo
     ctx->last_n_scan = n_scan; ctx->last_n_segs = p.n_pre_blocks;
     ctx->last_w = p.W; ctx->last_h = p.H; ctx->last_tx = p.TX; ctx->last_ty = p.TY; ctx->last_first_gid = p.first_gid;
     return FLOD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, float *out_rgb_dev, void *stream)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    if (int rc = check_frame_args(ctx, cam, out_rgb_dev)) return rc;
+    if (!(gamma > 0.0f) || !isfinite(gamma)) return fail(ctx, FLOD_E_INVALID_ARG, "render: gamma must be finite and > 0");
+    const int last_level = ctx->first_level + ctx->n_levels - 1;
+    if (mode.l_start < ctx->first_level || mode.l_end > last_level || mode.l_start > mode.l_end)
+        return fail(ctx, FLOD_E_LEVEL_RANGE, "render: need first_level <= l_start <= l_end <= last_level");
+    FrameParams p{};
+    camera_params(p, cam);
+    for (int i = 0; i < 3; ++i) p.ref[i] = ctx->has_ref ? ctx->ref[i] : p.centre[i];
+    const int i0 = mode.l_start - ctx->first_level, i1 = mode.l_end - ctx->first_level;   // level positions
+    p.n_levels = i1 - i0 + 1;
+    p.first_gid = ctx->level_off[i0];
+    p.n_scan = (int)(ctx->level_off[i1 + 1] - ctx->level_off[i0]);
+    band_params(ctx, i0, i1, cam->fx, gamma, p.level_end, p.lo2, p.hi2);
+    return enqueue_frame(ctx, ctx->scene, p, out_rgb_dev, (cudaStream_t)stream);
 }
 
 int flod_render_to_host_async(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, float *out_rgb_host,
@@ -442,6 +477,149 @@ int flod_render_to_host(flod_ctx *ctx, const flod_camera *cam, flod_level_mode m
     int rc = flod_render_to_host_async(ctx, cam, mode, gamma, out_rgb_host, stream, stream);
     if (rc != FLOD_OK) return rc;
     return flod_wait_host(ctx);
+}
+
+// ---------------------------------------------------------------- materialised G_sel (subset.cu)
+}  // extern "C"
+
+namespace {
+
+struct SubLayout { SnapshotDev snap[2]; unsigned int *blk; size_t bytes; };
+
+// two snapshots of up to n_range Gaussians + the per-block counters of the rebuild
+SubLayout carve_subset(unsigned char *base, int64_t n_range)
+{
+    SubLayout L{};
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return (unsigned char *)((uintptr_t)base + o); };
+    const size_t cap = (size_t)std::max<int64_t>(n_range, 1) + 8;       // k_geometry loads whole quads
+    for (int i = 0; i < 2; ++i) {
+        L.snap[i].n_sel = (unsigned int *)take(sizeof(unsigned int));
+        for (int a = 0; a < 13; ++a) L.snap[i].plane[a] = (float *)take(cap * sizeof(float));
+        L.snap[i].src_gid = (unsigned int *)take(cap * sizeof(unsigned int));
+    }
+    L.blk = (unsigned int *)take(((size_t)n_range / kGeoBlock + 4) * sizeof(unsigned int));
+    L.bytes = off;
+    return L;
+}
+
+bool subset_range(const flod_ctx *ctx, flod_level_mode mode, int *i0, int *i1)
+{
+    if (!ctx || !ctx->uploaded) return false;
+    const int last_level = ctx->first_level + ctx->n_levels - 1;
+    if (mode.l_start < ctx->first_level || mode.l_end > last_level || mode.l_start > mode.l_end) return false;
+    *i0 = mode.l_start - ctx->first_level; *i1 = mode.l_end - ctx->first_level;
+    return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t flod_subset_bytes(const flod_ctx *ctx, flod_level_mode mode)
+{
+    int i0, i1;
+    if (!subset_range(ctx, mode, &i0, &i1)) return 0;
+    return carve_subset(nullptr, ctx->level_off[i1 + 1] - ctx->level_off[i0]).bytes;
+}
+
+int flod_subset_set_arena(flod_ctx *ctx, void *arena_dev, size_t bytes, flod_level_mode mode)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    if (!ctx->uploaded) return fail(ctx, FLOD_E_NOT_UPLOADED, "subset_set_arena: no scene uploaded");
+    int i0, i1;
+    if (!subset_range(ctx, mode, &i0, &i1))
+        return fail(ctx, FLOD_E_LEVEL_RANGE, "subset_set_arena: need first_level <= l_start <= l_end <= last_level");
+    if (!arena_dev || (uintptr_t)arena_dev % 256) return fail(ctx, FLOD_E_INVALID_ARG, "subset_set_arena: null or unaligned pointer");
+    SubLayout L = carve_subset((unsigned char *)arena_dev, ctx->level_off[i1 + 1] - ctx->level_off[i0]);
+    if (bytes < L.bytes) return fail(ctx, FLOD_E_ARENA_TOO_SMALL, "subset_set_arena: arena too small");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    if (ctx->sub_build_pending) cudaEventSynchronize(ctx->ev_sub_built);
+    ctx->snap[0] = L.snap[0]; ctx->snap[1] = L.snap[1]; ctx->sub_blk = L.blk;
+    ctx->sub_i0 = i0; ctx->sub_i1 = i1;
+    ctx->sub_front = 0; ctx->sub_front_valid = false; ctx->sub_build_pending = false;
+    ctx->sub_read_pending[0] = ctx->sub_read_pending[1] = false;
+    ctx->has_subset = true;
+    return FLOD_OK;
+}
+
+int flod_subset_build(flod_ctx *ctx, const float ref_pos[3], float fx, float gamma, void *stream)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    if (!ctx->has_subset) return fail(ctx, FLOD_E_NO_WORKSPACE, "subset_build: no subset arena set");
+    if (!ref_pos) return fail(ctx, FLOD_E_INVALID_ARG, "subset_build: null reference position");
+    for (int i = 0; i < 3; ++i)
+        if (!isfinite(ref_pos[i]) || fabsf(ref_pos[i]) > 1e15f) return fail(ctx, FLOD_E_INVALID_ARG, "subset_build: reference must be finite, |x| <= 1e15");
+    if (!(fx > 0.0f) || !isfinite(fx) || !(gamma > 0.0f) || !isfinite(gamma))
+        return fail(ctx, FLOD_E_INVALID_ARG, "subset_build: fx and gamma must be finite and > 0");
+    if (ctx->sub_build_pending) return fail(ctx, FLOD_E_INVALID_ARG, "subset_build: a rebuild is already enqueued (swap first)");
+    cudaStream_t s = (cudaStream_t)stream;
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    const int back = ctx->sub_front_valid ? ctx->sub_front ^ 1 : ctx->sub_front;
+    // frames that still read the back snapshot (it was the front one before the last swap) come first
+    if (ctx->sub_read_pending[back]) { CUDA_TRY(ctx, cudaStreamWaitEvent(s, ctx->ev_sub_read[back], 0)); ctx->sub_read_pending[back] = false; }
+    SubsetParams q{};
+    memcpy(q.ref, ref_pos, sizeof(q.ref));
+    const int i0 = ctx->sub_i0, i1 = ctx->sub_i1;
+    q.first_gid = ctx->level_off[i0];
+    q.n_scan = (int)(ctx->level_off[i1 + 1] - ctx->level_off[i0]);
+    q.n_levels = i1 - i0 + 1;
+    band_params(ctx, i0, i1, fx, gamma, q.level_end, q.lo2, q.hi2);
+    q.n_blocks = (int)((q.first_gid - (q.first_gid & ~3ll) + q.n_scan + kGeoBlock - 1) / kGeoBlock);
+    launch_subset_build(*ctx, ctx->snap[back], q, s);
+    CUDA_TRY(ctx, cudaGetLastError());
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->sub_n_host, ctx->snap[back].n_sel, sizeof(unsigned int), cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(ctx, cudaEventRecord(ctx->ev_sub_built, s));
+    ctx->sub_build_pending = true;
+    return FLOD_OK;
+}
+
+int flod_subset_ready(flod_ctx *ctx)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    if (!ctx->sub_build_pending) return 0;
+    const cudaError_t e = cudaEventQuery(ctx->ev_sub_built);
+    if (e == cudaSuccess) return 1;
+    if (e == cudaErrorNotReady) return 0;
+    return fail(ctx, FLOD_E_CUDA, cudaGetErrorString(e));
+}
+
+int flod_subset_swap(flod_ctx *ctx, int64_t *n_selected)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    if (!ctx->sub_build_pending) return fail(ctx, FLOD_E_INVALID_ARG, "subset_swap: no rebuild enqueued");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    CUDA_TRY(ctx, cudaEventSynchronize(ctx->ev_sub_built));
+    const int back = ctx->sub_front_valid ? ctx->sub_front ^ 1 : ctx->sub_front;
+    ctx->sub_n[back] = (int64_t)*ctx->sub_n_host;
+    ctx->sub_front = back; ctx->sub_front_valid = true; ctx->sub_build_pending = false;
+    if (n_selected) *n_selected = ctx->sub_n[back];
+    return FLOD_OK;
+}
+
+int flod_render_subset(flod_ctx *ctx, const flod_camera *cam, float *out_rgb_dev, void *stream)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    if (int rc = check_frame_args(ctx, cam, out_rgb_dev)) return rc;
+    if (!ctx->has_subset || !ctx->sub_front_valid) return fail(ctx, FLOD_E_INVALID_ARG, "render_subset: no snapshot built and swapped in");
+    const int f = ctx->sub_front;
+    const SnapshotDev &sn = ctx->snap[f];
+    SceneDev sc = ctx->scene;                                 // SH rows stay in the scene arena (read by gid)
+    sc.mx = sn.plane[0]; sc.my = sn.plane[1]; sc.mz = sn.plane[2]; sc.rho2 = sn.plane[3]; sc.kappa = sn.plane[4];
+    for (int k = 0; k < 6; ++k) sc.cov[k] = sn.plane[5 + k];
+    sc.l2o = sn.plane[11]; sc.opacity = sn.plane[12];
+    sc.src_gid = sn.src_gid;
+    FrameParams p{};
+    camera_params(p, cam);
+    for (int i = 0; i < 3; ++i) p.ref[i] = p.centre[i];      // every entry of a snapshot is selected: one band [0, inf)
+    p.n_levels = 1; p.first_gid = 0; p.n_scan = (int)ctx->sub_n[f];
+    p.level_end[0] = p.n_scan; p.lo2[0] = 0.0f; p.hi2[0] = INFINITY;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int rc = enqueue_frame(ctx, sc, p, out_rgb_dev, s);
+    if (rc != FLOD_OK) return rc;
+    CUDA_TRY(ctx, cudaEventRecord(ctx->ev_sub_read[f], s));
+    ctx->sub_read_pending[f] = true;
+    return FLOD_OK;
 }
 
 int flod_get_stats(flod_ctx *ctx, flod_stats *out)

@@ -34,6 +34,24 @@ struct SceneDev {
     const float *sh;                      // [n][sh_stride] floats, row = K*3 coefficients padded to a multiple of 4
     int sh_stride;
     int sh_degree;
+    const unsigned int *src_gid;          // snapshots only (subset.cu): scene gid of every entry; nullptr for the scene itself
+};
+
+// One materialised G_sel (subset.cu): compacted copies of the planes k_geometry reads, in gid order.
+struct SnapshotDev {
+    float *plane[13];                     // mx, my, mz, rho2, kappa, cov[0..5], l2o, opacity
+    unsigned int *src_gid;
+    unsigned int *n_sel;                  // device copy of the count (written by the rebuild)
+};
+
+// Selection parameters of a rebuild (the selection half of FrameParams).
+struct SubsetParams {
+    float ref[3];
+    long long first_gid;
+    int n_scan, n_levels;
+    int level_end[FLOD_MAX_LEVELS];
+    float lo2[FLOD_MAX_LEVELS], hi2[FLOD_MAX_LEVELS];
+    int n_blocks;
 };
 
 // Per-frame counters, zeroed (with the tile difference grid) by one memset at the start of every frame.
@@ -128,10 +146,23 @@ struct Context {
     int img_turn = 0;
     cudaStream_t last_copy_stream = nullptr;
     bool ev_valid = false;
+    // materialised G_sel (subset.cu)
+    bool has_subset = false;
+    int sub_i0 = 0, sub_i1 = 0;           // level positions of the range
+    SnapshotDev snap[2]{};
+    unsigned int *sub_blk = nullptr;      // [n_blocks + 1] per-block counts, then exclusive offsets
+    int sub_front = 0;                    // snap[sub_front] is rendered from, the other one is rebuilt
+    bool sub_front_valid = false, sub_build_pending = false;
+    int64_t sub_n[2] = {0, 0};            // N_sel of each snapshot (host copy, valid after the swap)
+    unsigned int *sub_n_host = nullptr;   // pinned: the rebuild's count lands here
+    cudaEvent_t ev_sub_built = nullptr;   // rebuild complete (on the build stream)
+    cudaEvent_t ev_sub_read[2] = {nullptr, nullptr};   // last frame that read snap[i] (on the render stream)
+    bool sub_read_pending[2] = {false, false};
 };
 
 // kernel launchers (each enqueues on `s` and returns the number of kernels launched)
-int launch_geometry(const Context &c, const FrameParams &p, cudaStream_t s);    // a1-a3 + tile-count grid + visible list
+int launch_geometry(const Context &c, const SceneDev &sc, const FrameParams &p, cudaStream_t s);   // a1-a3 + tile-count grid + visible list
+int launch_subset_build(const Context &c, const SnapshotDev &dst, const SubsetParams &q, cudaStream_t s);   // a1 materialised
 int launch_colour(const Context &c, const FrameParams &p, cudaStream_t s);      // a4, and a5 + a8 (tile scan) in block 0
 int launch_duplicate(const Context &c, const FrameParams &p, cudaStream_t s);   // a6
 int launch_tile_sort(const Context &c, const FrameParams &p, cudaStream_t s);   // a7

@@ -104,7 +104,7 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
             const float dx = fsub(wx[k], p.ref[0]), dy = fsub(wy[k], p.ref[1]), dz = fsub(wz[k], p.ref[2]);
             const float d2 = fadd(fadd(fmul(dx, dx), fmul(dy, dy)), fmul(dz, dz));
             const bool sel = (d2 >= p.lo2[lv]) && (d2 < p.hi2[lv]);
-            if (DEBUG) ws.mask[g] = sel ? 1 : 0;
+            if (DEBUG) ws.mask[sc.src_gid ? (long long)__ldg(sc.src_gid + g) : g] = sel ? 1 : 0;   // (a snapshot holds selected ones only)
             if (!sel) continue;
             m_sel |= 1u << k;
             // ---- a2 (O2): p = R mu + t
@@ -248,10 +248,11 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
             reinterpret_cast<float2 *>(ws.gB)[2 * c] = make_float2(d2, l2o);          // (r, g) by k_colour
             ws.rect[c] = make_ushort4((unsigned short)tx0, (unsigned short)ty0, (unsigned short)tx1, (unsigned short)ty1);
             ws.depth[c] = __float_as_uint(z);
-            ws.dirgid[c] = make_float4(wxk - p.centre[0], wyk - p.centre[1], wzk - p.centre[2], __uint_as_float((unsigned int)g));
+            const unsigned int g_scene = sc.src_gid ? __ldg(sc.src_gid + g) : (unsigned int)g;     // the SH row's gid
+            ws.dirgid[c] = make_float4(wxk - p.centre[0], wyk - p.centre[1], wzk - p.centre[2], __uint_as_float(g_scene));
             if (DEBUG) {
                 flod_dbg_projected d;
-                d.gid = (unsigned int)g; d.mu2d[0] = mx2; d.mu2d[1] = my2; d.depth = z;
+                d.gid = g_scene; d.mu2d[0] = mx2; d.mu2d[1] = my2; d.depth = z;
                 d.conic[0] = cA; d.conic[1] = cB; d.conic[2] = cC; d.opacity = __ldg(sc.opacity + g);
                 d.rgb[0] = 0.0f; d.rgb[1] = 0.0f; d.rgb[2] = 0.0f;                                // by k_colour
                 d.rect[0] = tx0; d.rect[1] = ty0; d.rect[2] = tx1; d.rect[3] = ty1;
@@ -355,11 +356,11 @@ k_colour(const SceneDev sc, const WorkspaceDev ws, int TX, int TY, unsigned int 
     }
 }
 
-int launch_geometry(const Context &c, const FrameParams &p, cudaStream_t s)
+int launch_geometry(const Context &c, const SceneDev &sc, const FrameParams &p, cudaStream_t s)
 {
     if (p.n_pre_blocks <= 0) return 0;
-    if (c.flags & FLOD_OPT_DEBUG) k_geometry<true><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(c.scene, c.ws, p);
-    else k_geometry<false><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(c.scene, c.ws, p);
+    if (c.flags & FLOD_OPT_DEBUG) k_geometry<true><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(sc, c.ws, p);
+    else k_geometry<false><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(sc, c.ws, p);
     return 1;
 }
 
