@@ -43,6 +43,9 @@ def parse_args():
     ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--mode", default=None, help="max | level<l> | sel<ls><le> e.g. sel345; default per config")
     ap.add_argument("--gamma", type=float, default=1.0)
+    ap.add_argument("--subset-period", type=int, default=0,
+                    help="selective modes only: render from a materialised G_sel (flod_render_subset) that is rebuilt "
+                         "every N frames on a second stream and swapped in when ready (P:699-711); 0 = Eq. 6 per frame")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--count-scale", type=float, default=1.0, help="shrink the scene (debugging only; reported)")
     return ap.parse_args()
@@ -179,6 +182,20 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def ncu_traffic(stage):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernel, from the committed summary of the
+    latest `ncu --set full` capture of the default workload (profiles/*_ncu_full.csv; None when there is none)."""
+    import csv
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "*_ncu_full.csv")))
+    if not files:
+        return None, None
+    for row in csv.DictReader(open(files[-1])):
+        if row["stage"] == stage:
+            return (float(row["dram_read_mb"]) + float(row["dram_write_mb"])) * 1e6, os.path.relpath(files[-1], ROOT)
+    return None, None
+
+
 def workload_config(args, scene, cam, mode, ls, le):
     return {
         "workload": f"BASELINE.json configs[{args.config}]: {len(scene.levels)}-level synthetic scene, "
@@ -187,6 +204,8 @@ def workload_config(args, scene, cam, mode, ls, le):
                     + (f", gamma {args.gamma} px" if ls != le else "") + ")",
         "levels": [ls, le], "gamma": args.gamma, "n_gaussians": scene.n_total, "width": cam.width, "height": cam.height,
         "count_scale": args.count_scale,
+        "selection": (f"materialised G_sel, asynchronous rebuild every {args.subset_period} frames at the current camera "
+                      "centre, swapped in when ready (value and stages; e2e uses the per-frame predicate)" if args.subset_period > 0 and ls != le else "Eq. 6 evaluated per frame"),
         "l2": "inputs larger than L2 (scanned level planes + SH exceed 126 MB), no flush between frames",
         "parallelism": f"replicas x{args.gpus} (poses sharded, no collective)",
     }
@@ -236,6 +255,28 @@ def run_ours(args):
     from paper_2408_12894_b200.shard import max_over_ranks, pose_index
     my_pose = lambda k: cs[pose_index(k, rank, world, len(cs))]       # poses sharded over ranks
 
+    use_subset = args.subset_period > 0 and ls != le
+    sub = {"pending": False}
+    if use_subset:
+        r.subset_set_arena(ls, le)
+        side = torch.cuda.Stream(device=r.device)
+
+        def centre(c):     # -R^T t, fp64 from the fp32 fields, rounded once
+            R, t = np.asarray(c.R[:], dtype=np.float64).reshape(3, 3), np.asarray(c.t[:], dtype=np.float64)
+            return np.array([-((R[0, i] * t[0] + R[1, i] * t[1]) + R[2, i] * t[2]) for i in range(3)]).astype(np.float32)
+
+        r.subset_build(centre(my_pose(0)), my_pose(0).fx, args.gamma)
+        r.subset_swap()
+
+    def render_frame(k, out_t):
+        if not use_subset:
+            return r.render(my_pose(k), ls, le, args.gamma, out_t)
+        if sub["pending"] and r.subset_ready():
+            r.subset_swap(); sub["pending"] = False
+        if k % args.subset_period == 0 and not sub["pending"]:
+            r.subset_build(centre(my_pose(k)), my_pose(k).fx, args.gamma, stream=side); sub["pending"] = True
+        return r.render_subset(my_pose(k), out_t)
+
     # ---- capacity check on every pose this rank will touch (un-timed)
     r.set_options(0)
     need = 0
@@ -248,7 +289,7 @@ def run_ours(args):
 
     # ---- timed region 1: device-resident output (value)
     for k in range(W):
-        r.render(my_pose(k), ls, le, args.gamma, out)
+        render_frame(k, out)
     barrier()
     sampler = ClockSampler(local_rank)
     if rank == 0:
@@ -256,7 +297,7 @@ def run_ours(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for k in range(K):
-        r.render(my_pose(k), ls, le, args.gamma, out)
+        render_frame(k, out)
     e1.record()
     barrier()
     ms = e0.elapsed_time(e1)
@@ -285,7 +326,7 @@ def run_ours(args):
     stage_ms = np.zeros(len(STAGE_NAMES))
     agg = dict(n_scan=0, n_sel=0, n_front=0, n_vis=0, n_pairs=0)
     for k in range(n_diag):
-        r.render(my_pose(k), ls, le, args.gamma, out)
+        r.render_subset(my_pose(k), out) if use_subset else r.render(my_pose(k), ls, le, args.gamma, out)
         st = r.get_stats()
         stage_ms += np.array(st["ms_stage"])
         for key in agg:
@@ -296,7 +337,7 @@ def run_ours(args):
     r.set_options(pkg.FLOD_OPT_COUNT)
     E = B = 0
     for k in range(n_diag):
-        r.render(my_pose(k), ls, le, args.gamma, out)
+        r.render_subset(my_pose(k), out) if use_subset else r.render(my_pose(k), ls, le, args.gamma, out)
         st = r.get_stats()
         E += st["evals"]; B += st["blends"]
     E /= n_diag; B /= n_diag
@@ -343,7 +384,10 @@ def run_ours(args):
     sort_vs_model["frac"] = sort_vs_model["achieved"] / hbm
     dominant = max(stages, key=lambda n: stages[n]["ns"])
     roof = {k: stages[dominant][k] for k in ("bound", "achieved", "peak", "unit", "frac")}
-    roof.update({"kernel": dominant, "traffic": None, "peak_source": f"{peak_src} MEASURED_PEAKS.json" if dominant != "blend"
+    traffic, traffic_src = ncu_traffic(dominant) if (args.config, mode, args.count_scale) == (1, "max", 1.0) else (None, None)
+    roof.update({"kernel": dominant, "traffic": traffic, "traffic_unit": "bytes per launch (DRAM read + write)",
+                 "traffic_source": traffic_src,
+                 "peak_source": f"{peak_src} MEASURED_PEAKS.json" if dominant != "blend"
                  else f"{sm_count} SMs x 128 FP32 lanes x 2 x {sm_max_mhz:.0f} MHz (DESIGN §6.3)"})
 
     fps = world * K / (ms * 1e-3)
