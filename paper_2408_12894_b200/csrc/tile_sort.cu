@@ -51,13 +51,40 @@ __device__ __forceinline__ unsigned int block_min_u32(SortSmem &S, unsigned int 
     return v;
 }
 
+#ifndef FLOD_SORT_UNROLL
+#define FLOD_SORT_UNROLL 8
+#endif
+constexpr int kSortU = FLOD_SORT_UNROLL;                  // keys a thread holds in registers / loads in flight per step
+
+// f(key) for src[from .. n) strided over the block, kSortU independent loads in flight per thread and step.
+template <class F>
+__device__ __forceinline__ void for_keys(const u64 *src, unsigned int from, unsigned int n, int tid, F f)
+{
+    for (unsigned int j0 = from + tid; j0 < n; j0 += kSortU * kSortThreads) {
+        u64 k[kSortU];
+#pragma unroll
+        for (int i = 0; i < kSortU; ++i) { const unsigned int j = j0 + i * kSortThreads; k[i] = j < n ? src[j] : 0ull; }
+#pragma unroll
+        for (int i = 0; i < kSortU; ++i) if (j0 + i * kSortThreads < n) f(k[i]);
+    }
+}
+
 // Distributes src[0, n) into dst[0, n) by bin (src and dst must not overlap).  On return ends[b] is the exclusive end
 // of bin b in dst (its start is ends[b-1], 0 for b = 0), and all writes are visible to the block.
 __device__ BinMap bin_pass(const u64 *src, u64 *dst, unsigned int n, unsigned int *ends, SortSmem &S, int tid)
 {
     const int lane = tid & 31, warp = tid >> 5;
+    // the first kSortU * kSortThreads keys (the whole list of an average tile) stay in registers over the three passes
+    u64 r[kSortU];
+#pragma unroll
+    for (int i = 0; i < kSortU; ++i) { const unsigned int j = tid + i * kSortThreads; r[i] = j < n ? src[j] : 0ull; }
+    auto each = [&](auto f) {
+#pragma unroll
+        for (int i = 0; i < kSortU; ++i) if (tid + i * kSortThreads < n) f(r[i]);
+        for_keys(src, kSortU * kSortThreads, n, tid, f);
+    };
     u64 kmin = ~0ull, kmax = 0ull;
-    for (unsigned int j = tid; j < n; j += kSortThreads) { const u64 k = src[j]; kmin = min(kmin, k); kmax = max(kmax, k); }
+    each([&](u64 k) { kmin = min(kmin, k); kmax = max(kmax, k); });
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         kmin = min(kmin, __shfl_xor_sync(0xffffffffu, kmin, o));
@@ -76,7 +103,7 @@ __device__ BinMap bin_pass(const u64 *src, u64 *dst, unsigned int n, unsigned in
     m.nb = (unsigned int)(range >> m.shift) + 1u;                                  // <= 2^want
     for (unsigned int b = tid; b < m.nb; b += kSortThreads) ends[b] = 0;
     __syncthreads();
-    for (unsigned int j = tid; j < n; j += kSortThreads) atomicAdd(&ends[bin_of(m, src[j])], 1u);
+    each([&](u64 k) { atomicAdd(&ends[bin_of(m, k)], 1u); });
     __syncthreads();
     // exclusive scan of ends[0, nb): a thread owns ipt consecutive bins
     {
@@ -101,10 +128,7 @@ __device__ BinMap bin_pass(const u64 *src, u64 *dst, unsigned int n, unsigned in
     // (keeping the arrival rank that a value-returning histogram atomic would give, to save this second atomic,
     // measured 9 us slower on config 1: it needs a rank array, two more barriers and a pass that turns bin starts into
     // bin ends, and with about five keys per thread the fixed cost per tile is what counts)
-    for (unsigned int j = tid; j < n; j += kSortThreads) {
-        const u64 k = src[j];
-        dst[atomicAdd(&ends[bin_of(m, k)], 1u)] = k;
-    }
+    each([&](u64 k) { dst[atomicAdd(&ends[bin_of(m, k)], 1u)] = k; });
     __syncthreads();
     return m;
 }
@@ -176,7 +200,7 @@ __device__ void finish_sort(const u64 *buf, unsigned int n, const BinMap &m, u64
     }
 }
 
-__global__ void __launch_bounds__(kSortThreads)
+__global__ void __launch_bounds__(kSortThreads, 4)      // 4 CTAs per SM is what the 49 KB of shared memory allow
 k_tile_sort(const WorkspaceDev ws, int n_tiles)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
