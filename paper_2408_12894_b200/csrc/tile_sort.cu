@@ -22,6 +22,11 @@ constexpr int kSortBins = 1 << kSortBinsLog;
 #ifndef FLOD_SORT_KEYS_PER_BIN_LOG
 #define FLOD_SORT_KEYS_PER_BIN_LOG 1
 #endif
+#ifndef FLOD_SORT_SLICE_LOG
+#define FLOD_SORT_SLICE_LOG 10
+#endif
+constexpr int kCoarseBinsLog = 8;
+constexpr int kCoarseBins = 1 << kCoarseBinsLog;
 constexpr unsigned int kRankMax = 64;                     // bins up to this size are finished by per-key rank counting
 
 typedef unsigned long long u64;
@@ -33,6 +38,7 @@ struct SortSmem {
     unsigned int red_u[kSortWarps];
     unsigned int wsum[kSortWarps];
     unsigned int any_big[2];                              // per level: some bin exceeded kRankMax (set by rank_small)
+    unsigned int cends[kCoarseBins];                      // lists longer than kSortCap: ends of the coarse depth slices
 };
 
 struct BinMap { u64 kmin; int shift; unsigned int nb; };
@@ -71,7 +77,8 @@ __device__ __forceinline__ void for_keys(const u64 *src, unsigned int from, unsi
 
 // Distributes src[0, n) into dst[0, n) by bin (src and dst must not overlap).  On return ends[b] is the exclusive end
 // of bin b in dst (its start is ends[b-1], 0 for b = 0), and all writes are visible to the block.
-__device__ BinMap bin_pass(const u64 *src, u64 *dst, unsigned int n, unsigned int *ends, SortSmem &S, int tid)
+__device__ BinMap bin_pass(const u64 *src, u64 *dst, unsigned int n, unsigned int *ends, SortSmem &S, int tid,
+                           int per_bin_log = FLOD_SORT_KEYS_PER_BIN_LOG, int min_bins_log = 6, int max_bins_log = kSortBinsLog)
 {
     const int lane = tid & 31, warp = tid >> 5;
     // the first kSortU * kSortThreads keys (the whole list of an average tile) stay in registers over the three passes
@@ -98,7 +105,7 @@ __device__ BinMap bin_pass(const u64 *src, u64 *dst, unsigned int n, unsigned in
     m.kmin = kmin;
     const u64 range = kmax - kmin;
     const int bits = range ? 64 - __clzll(range) : 0;
-    const int want = min(kSortBinsLog, max(6, 32 - FLOD_SORT_KEYS_PER_BIN_LOG - __clz(max(n, 2u) - 1)));   // about two keys per bin
+    const int want = min(max_bins_log, max(min_bins_log, 32 - per_bin_log - __clz(max(n, 2u) - 1)));   // about 2^per_bin_log keys per bin
     m.shift = max(0, bits - want);
     m.nb = (unsigned int)(range >> m.shift) + 1u;                                  // <= 2^want
     for (unsigned int b = tid; b < m.nb; b += kSortThreads) ends[b] = 0;
@@ -215,10 +222,32 @@ k_tile_sort(const WorkspaceDev ws, int n_tiles)
     u64 *pairs = ws.pairs + rg.x;
     uint32_t *vals = ws.vals + rg.x;
     if (L == 1) { if (tid == 0) vals[0] = (uint32_t)pairs[0]; return; }
-    u64 *buf = L <= (unsigned int)kSortCap ? S.keys : ws.pairs_tmp + rg.x;
     if (tid == 0) S.any_big[0] = 0;
-    const BinMap m = bin_pass(pairs, buf, L, S.ends[0], S, tid);
-    finish_sort(buf, L, m, pairs, vals, S, tid);
+    if (L <= (unsigned int)kSortCap) {
+        const BinMap m = bin_pass(pairs, S.keys, L, S.ends[0], S, tid);
+        finish_sort(S.keys, L, m, pairs, vals, S, tid);
+        return;
+    }
+    // ---- a long list: cut it into depth slices of 512-1024 keys (one pass through global memory), then sort every
+    // slice in shared memory like a short list: ranking a 30 000-key list straight from 2048 bins costs 15 L2 reads
+    // per key, the slices cost one more scatter.  A slice that is still longer than kSortCap (a cluster of nearly
+    // equal depths) goes through global memory.
+    u64 *tmp = ws.pairs_tmp + rg.x;
+    const BinMap mc = bin_pass(pairs, tmp, L, S.cends, S, tid, FLOD_SORT_SLICE_LOG, 1, kCoarseBinsLog);
+    for (unsigned int b = 0; b < mc.nb; ++b) {
+        const unsigned int lo = b ? S.cends[b - 1] : 0u, n2 = S.cends[b] - lo;
+        if (n2 == 0) continue;
+        if (n2 == 1) { if (tid == 0) vals[lo] = (uint32_t)tmp[lo]; continue; }
+        if (n2 <= (unsigned int)kSortCap) {
+            const BinMap m = bin_pass(tmp + lo, S.keys, n2, S.ends[0], S, tid);
+            finish_sort(S.keys, n2, m, pairs + lo, vals + lo, S, tid);
+        } else {
+            const BinMap m = bin_pass(tmp + lo, pairs + lo, n2, S.ends[0], S, tid);
+            finish_sort(pairs + lo, n2, m, tmp + lo, vals + lo, S, tid);
+        }
+        __syncthreads();
+        if (tid == 0) S.any_big[0] = 0;                  // ordered before its next readers by the barriers of bin_pass
+    }
 }
 
 int launch_tile_sort(const Context &c, const FrameParams &p, cudaStream_t s)
