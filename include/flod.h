@@ -97,7 +97,9 @@ typedef struct {
 enum {                               /* flod_set_options bits */
     FLOD_OPT_DEBUG   = 1,            /* also write the selection mask and per-Gaussian projection records */
     FLOD_OPT_PROFILE = 2,            /* record CUDA events between stages (flod_get_stats reports ms) */
-    FLOD_OPT_COUNT   = 4             /* instrumented blend kernel counting evaluations and blends */
+    FLOD_OPT_COUNT   = 4,            /* instrumented blend kernel counting evaluations and blends */
+    FLOD_OPT_SMALL_WINDOWS = 8       /* test knob: the large-rect duplication kernel walks the tiles in windows of 1024 (the
+                                        path an image of more than 48 Ki tiles takes) */
 };
 
 enum {                               /* flod_debug_copy selectors; host_dst sizes in bytes */

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libflod.so")
 HEADER = os.path.join(HERE, "..", "include", "flod.h")
 
-FLOD_OPT_DEBUG, FLOD_OPT_PROFILE, FLOD_OPT_COUNT = 1, 2, 4
+FLOD_OPT_DEBUG, FLOD_OPT_PROFILE, FLOD_OPT_COUNT, FLOD_OPT_SMALL_WINDOWS = 1, 2, 4, 8
 FLOD_DBG_MASK, FLOD_DBG_TILE_COUNTS, FLOD_DBG_PROJECTED, FLOD_DBG_SORTED_PAIRS, FLOD_DBG_ACTIVATED = range(5)
 FLOD_N_STAGES = 5
 STAGE_NAMES = ("geometry", "colour", "duplicate", "tile_sort", "blend")

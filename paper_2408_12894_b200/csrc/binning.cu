@@ -20,6 +20,20 @@ namespace flod {
 // cooperatively, one group per thread per step, whatever the individual rect sizes.
 constexpr int kDupPer = kGeoBlock / kPreBlock;
 
+// Which of the two duplication kernels serves the frame (both are launched, the other one exits at once): the mean
+// rect area, known on the device since k_geometry.  Small rects (config 1: 4.3 tiles per Gaussian): k_duplicate, one
+// value-returning global atomic per 2x2 tile group.  Large rects (a coarse level alone: hundreds of tiles per
+// Gaussian on a few hundred counters): those atomics serialise on their addresses (config 3, level 1: 979 us), so
+// k_duplicate_shared counts in shared memory and goes to the global counters once per block and tile.
+#ifndef FLOD_DUP_LARGE_AREA
+#define FLOD_DUP_LARGE_AREA 128
+#endif
+constexpr unsigned int kDupLargeArea = FLOD_DUP_LARGE_AREA;
+__device__ __forceinline__ bool dup_large_rects(const WorkspaceDev &ws)
+{
+    return ws.hdr->n_pairs > (unsigned long long)kDupLargeArea * ws.hdr->n_vis32;
+}
+
 __global__ void __launch_bounds__(kPreBlock)
 k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs)
 {
@@ -31,7 +45,7 @@ k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned int seg = blockIdx.x;
     const unsigned int n_here = ws.seg_count[seg];
-    if (n_here == 0) return;
+    if (n_here == 0 || dup_large_rects(ws)) return;       // frames of large rects are served by k_duplicate_shared
     const unsigned int p0 = seg * kGeoBlock;
     // thread t owns entries kDupPer t .. kDupPer t + kDupPer - 1 (consecutive, so that the scan is a plain block scan)
     unsigned int ng[kDupPer], mine = 0;
@@ -96,11 +110,157 @@ k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs)
     }
 }
 
+// ------------------------------------------------------------------------------------------------ a6, large rects
+// Persistent: one block of 1024 threads per SM.  The (segment, chunk of 32 entries) units of the frame are dealt
+// round-robin to the warps of the whole grid; a block appends its share in two passes with a per-tile counter array in
+// SHARED memory:
+//   count    every pair adds 1 to its tile's shared counter;
+//   reserve  one global atomicAdd per touched tile reserves the block's share of that tile's list;
+//   emit     every pair takes the next slot of its tile from the shared counter and stores its key.
+// A lane walks its own rect when it has at most kDupInline tiles, a larger rect is expanded by the whole warp.
+// Images with more tiles than fit in shared memory are processed in windows of `win_cap` tiles (both passes each).
+constexpr int kDupSThreads = 1024;
+constexpr int kDupSWarps = kDupSThreads / 32;
+constexpr int kDupSegRound = 256;          // segments of the block whose chunk counts are scanned at a time
+constexpr unsigned int kDupInline = 8;     // rects up to this many tiles are walked by their own lane
+constexpr int kDupWinCap = 48 * 1024;      // tiles per window: 192 KB of shared counters
+
+template <bool kEmit>
+__device__ __forceinline__ void dup_pair(unsigned int *s_cnt, unsigned int t, unsigned int win0, unsigned int win_n,
+                                         unsigned long long key, unsigned long long *__restrict__ pairs, unsigned int max_pairs)
+{
+    const unsigned int r = t - win0;
+    if (r >= win_n) return;
+    if (kEmit) {
+        const unsigned int pos = atomicAdd(&s_cnt[r], 1u);
+        if (pos < max_pairs) pairs[pos] = key;
+    } else {
+        atomicAdd(&s_cnt[r], 1u);
+    }
+}
+
+template <bool kEmit>
+__device__ __forceinline__ void dup_pass(const WorkspaceDev &ws, unsigned int *s_cnt, unsigned int *s_pref, unsigned int *s_segn,
+                                         unsigned int *s_wtot, unsigned int TX, unsigned int n_segs, unsigned int win0,
+                                         unsigned int win_n, unsigned int max_pairs)
+{
+    const unsigned int tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    // every block walks ALL segments, kDupSegRound at a time, and takes every (32 gridDim)-th unit of the round: a coarse
+    // level has few Gaussians (config 3, level 1: 30 segments) with hundreds of tiles each, so units, not segments,
+    // are what is dealt out, and consecutive units go to different SMs
+    for (unsigned int k0 = 0; k0 < n_segs; k0 += kDupSegRound) {
+        const unsigned int nr = min((unsigned int)kDupSegRound, n_segs - k0);
+        // exclusive scan of the chunk counts of the round's segments -> s_pref[0 .. nr]
+        if (tid < kDupSegRound) {
+            const unsigned int n = tid < nr ? ws.seg_count[k0 + tid] : 0u;
+            unsigned int incl = (n + 31u) >> 5;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const unsigned int t = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += t;
+            }
+            if (lane == 31) s_wtot[warp] = incl;
+            s_pref[tid + 1] = incl;                         // warp-local for now
+            if (tid < nr) s_segn[tid] = n;
+        }
+        __syncthreads();
+        if (tid < kDupSegRound) {
+            unsigned int add = 0;
+            for (unsigned int w = 0; w < warp; ++w) add += s_wtot[w];
+            s_pref[tid + 1] += add;
+            if (tid == 0) s_pref[0] = 0;
+        }
+        __syncthreads();
+        const unsigned int n_units = s_pref[nr];
+        for (unsigned int v = warp * gridDim.x + blockIdx.x; v < n_units; v += kDupSWarps * gridDim.x) {
+            {
+                unsigned int lo = 0, hi = nr - 1u;          // the segment k with s_pref[k] <= v < s_pref[k + 1]
+                while (lo < hi) {
+                    const unsigned int mid = (lo + hi + 1u) >> 1;
+                    if (s_pref[mid] <= v) lo = mid; else hi = mid - 1u;
+                }
+                const unsigned int k = lo, c = v - s_pref[lo];
+                const unsigned int seg = k0 + k;
+                const unsigned int j = (c << 5) + lane;
+                const unsigned int p = seg * kGeoBlock + j;
+                unsigned int xy0 = 0, w = 0, area = 0, depth = 0;
+                if (j < s_segn[k]) {
+                    const ushort4 rc = ws.rect[p];
+                    xy0 = (unsigned int)rc.x | ((unsigned int)rc.y << 16);
+                    w = (unsigned int)rc.z - rc.x;
+                    area = w * ((unsigned int)rc.w - rc.y);
+                    if (kEmit) depth = ws.depth[p];
+                }
+                if (area <= kDupInline) {                   // small rects: every lane walks its own
+                    const unsigned long long key = ((unsigned long long)depth << 32) | p;
+                    unsigned int t = (xy0 >> 16) * TX + (xy0 & 0xffffu), x = 0;
+                    for (unsigned int i = 0; i < area; ++i) {
+                        dup_pair<kEmit>(s_cnt, t, win0, win_n, key, ws.pairs, max_pairs);
+                        ++t;
+                        if (++x == w) { x = 0; t += TX - w; }
+                    }
+                }
+                unsigned int big = __ballot_sync(0xffffffffu, area > kDupInline);
+                while (big) {                               // large rects: the whole warp expands one at a time
+                    const int r = __ffs((int)big) - 1;
+                    big &= big - 1u;
+                    const unsigned int rxy = __shfl_sync(0xffffffffu, xy0, r), rw = __shfl_sync(0xffffffffu, w, r);
+                    const unsigned int ra = __shfl_sync(0xffffffffu, area, r), rd = __shfl_sync(0xffffffffu, depth, r);
+                    const unsigned long long key = ((unsigned long long)rd << 32) | (p - lane + (unsigned int)r);
+                    const unsigned int t0 = (rxy >> 16) * TX + (rxy & 0xffffu);
+                    // q / rw by multiplication: exact for q < 2^16 (inv = ceil(2^32 / rw), rw < 2^16)
+                    const unsigned int inv = rw > 1u ? 0xffffffffu / rw + 1u : 0u;
+                    const bool fast = ra <= 65536u && rw > 1u;
+                    for (unsigned int q = lane; q < ra; q += 32u) {
+                        const unsigned int dy = fast ? __umulhi(q, inv) : q / rw;
+                        dup_pair<kEmit>(s_cnt, t0 + dy * TX + (q - dy * rw), win0, win_n, key, ws.pairs, max_pairs);
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(kDupSThreads, 1)
+k_duplicate_shared(const WorkspaceDev ws, unsigned int TX, unsigned int T_n, unsigned int n_segs, unsigned int win_cap,
+                   unsigned int max_pairs)
+{
+    extern __shared__ unsigned int s_cnt[];         // [win_cap] pairs of the block per tile, then the next free slot
+    __shared__ unsigned int s_pref[kDupSegRound + 1];
+    __shared__ unsigned int s_segn[kDupSegRound];
+    __shared__ unsigned int s_wtot[kDupSegRound / 32];
+    if (!dup_large_rects(ws)) return;
+    const unsigned int tid = threadIdx.x;
+    for (unsigned int win0 = 0; win0 < T_n; win0 += win_cap) {
+        const unsigned int win_n = min(win_cap, T_n - win0);
+        for (unsigned int r = tid; r < win_n; r += kDupSThreads) s_cnt[r] = 0;
+        __syncthreads();
+        dup_pass<false>(ws, s_cnt, s_pref, s_segn, s_wtot, TX, n_segs, win0, win_n, max_pairs);
+        for (unsigned int r = tid; r < win_n; r += kDupSThreads) {      // (dup_pass ends with a barrier)
+            const unsigned int c = s_cnt[r];
+            if (c) s_cnt[r] = ws.ranges[win0 + r].x + atomicAdd(&ws.cursor[win0 + r], c);
+        }
+        __syncthreads();
+        dup_pass<true>(ws, s_cnt, s_pref, s_segn, s_wtot, TX, n_segs, win0, win_n, max_pairs);
+    }
+}
+
+int init_duplicate()
+{
+    return cudaFuncSetAttribute(k_duplicate_shared, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                kDupWinCap * (int)sizeof(unsigned int)) == cudaSuccess ? 0 : -1;
+}
+
 int launch_duplicate(const Context &c, const FrameParams &p, cudaStream_t s)
 {
     if (p.n_pre_blocks <= 0) return 0;
     k_duplicate<<<p.n_pre_blocks, kPreBlock, 0, s>>>(c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs);
-    return 1;
+    const unsigned int T_n = (unsigned int)p.n_tiles;
+    const unsigned int win_cap = (c.flags & FLOD_OPT_SMALL_WINDOWS) ? 1024u : min(T_n, (unsigned int)kDupWinCap);
+    k_duplicate_shared<<<c.sm_count, kDupSThreads, win_cap * sizeof(unsigned int), s>>>(
+        c.ws, (unsigned int)p.TX, T_n, (unsigned int)p.n_pre_blocks, win_cap, p.max_pairs);
+    return 2;
 }
 
 }  // namespace flod

@@ -109,6 +109,7 @@ WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_p
     L.ws.tile_cnt = (int *)take((tx + 1) * (ty + 1) * sizeof(int));
     L.ws.ranges = (uint2 *)take(tiles * sizeof(uint2));
     L.ws.cursor4 = (float *)take(((tx + 1) / 2) * ((ty + 1) / 2) * kCtrStride * sizeof(float));
+    L.ws.cursor = (unsigned int *)take(tiles * sizeof(unsigned int));
     L.ws.gA = (float4 *)take(nt * sizeof(float4));
     L.ws.gB = (float4 *)take(nt * sizeof(float4));
     L.ws.cB = (float *)take(nt * sizeof(float));
@@ -144,7 +145,8 @@ int flod_create(flod_ctx **out, int device)
     flod_ctx *c = new flod_ctx();
     c->device = device;
     if (cudaSetDevice(device) != cudaSuccess ||
-        cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) {
+        cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
+        init_duplicate() != 0) {
         delete c;
         return FLOD_E_CUDA;
     }
@@ -328,7 +330,7 @@ int flod_set_options(flod_ctx *ctx, unsigned flags)
 int flod_launches_per_frame(const flod_ctx *ctx)
 {
     if (!ctx || !ctx->has_ws) return 0;
-    return 5;   // geometry, colour (+ tile scan in its block 0), duplication, tile sort, blend
+    return 6;   // geometry, colour (+ tile scan in its block 0), duplication (two kernels, one of which exits), tile sort, blend
 }
 
 }  // extern "C"

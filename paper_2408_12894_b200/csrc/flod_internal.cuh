@@ -77,6 +77,7 @@ struct WorkspaceDev {
     uint2 *ranges;                        // [T_n] (start, end) of every tile's pair list
     float *cursor4;                       // [ceil(TX/2) * ceil(TY/2)][kCtrStride] first 4 floats: entries appended so far to the
                                           // lists of the 2x2 tile group (x, y), (x+1, y), (x, y+1), (x+1, y+1); zeroed by the tile scan
+    unsigned int *cursor;                 // [T_n] the same per tile, dense (k_duplicate_shared); zeroed by the tile scan
     float4 *gA, *gB;                      // [n_total + 2 kGeoBlock]
     float *cB;                            // [n_total + 2 kGeoBlock]
     float4 *dirgid;                       // [n_total + 2 kGeoBlock] (mu - c_cam, gid bits): input of the colour kernel
@@ -165,6 +166,7 @@ int launch_geometry(const Context &c, const SceneDev &sc, const FrameParams &p, 
 int launch_subset_build(const Context &c, const SnapshotDev &dst, const SubsetParams &q, cudaStream_t s);   // a1 materialised
 int launch_colour(const Context &c, const FrameParams &p, cudaStream_t s);      // a4, and a5 + a8 (tile scan) in block 0
 int launch_duplicate(const Context &c, const FrameParams &p, cudaStream_t s);   // a6
+int init_duplicate();                                                            // once per device: shared-memory opt-in
 int launch_tile_sort(const Context &c, const FrameParams &p, cudaStream_t s);   // a7
 int launch_blend(const Context &c, const FrameParams &p, float *out_rgb, cudaStream_t s);   // a9
 

@@ -76,6 +76,7 @@ __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, 
         const unsigned int a = (unsigned int)min(run, (unsigned long long)max_pairs);
         const unsigned int b = (unsigned int)min(run + c, (unsigned long long)max_pairs);
         ws.ranges[t] = make_uint2(a, b);
+        ws.cursor[t] = 0;                                      // k_duplicate_shared: entries appended so far
         if (c > (1u << 24)) too_long = 1u;                     // k_duplicate counts a tile's entries in a float
         run += c;
     }

@@ -159,3 +159,25 @@ def test_materialised_subset_async_rebuild(full):
         assert n_sel == st_f["n_sel"] and (st["n_vis"], st["n_pairs"]) == (st_f["n_vis"], st_f["n_pairs"])
         assert np.array_equal(img, fused)
     assert not r.subset_ready()                                  # nothing enqueued after the last swap
+
+
+def test_coarse_level_duplication_shared_counters_and_windows(full):
+    """A coarse level alone (level 1: rects of hundreds of tiles) is duplicated by k_duplicate_shared (per-tile counters
+    in shared memory), which walks the tiles in windows when an image has more tiles than fit (48 Ki);
+    FLOD_OPT_SMALL_WINDOWS forces windows of 1024 on the 4056 tiles of config 1.  The final (tile, depth, gid)
+    sequence must be the oracle's either way."""
+    import paper_2408_12894_b200 as pkg
+    scene, cams, osc, r = full
+    fr = osc.frame(cams[3], 1, 1, 1.0)
+    assert fr.counts["n_pairs"] > 128 * fr.counts["n_vis"]          # the large-rect kernel's condition
+    tile, depth, gid = fr.sorted_pairs()
+    for flags in (pkg.FLOD_OPT_DEBUG, pkg.FLOD_OPT_DEBUG | pkg.FLOD_OPT_SMALL_WINDOWS):
+        r.set_options(flags)
+        try:
+            r.render(cams[3], 1, 1, 1.0)
+            st = r.get_stats()
+            sp = r.debug_sorted_pairs(st["n_pairs"])
+        finally:
+            r.set_options(pkg.FLOD_OPT_DEBUG)
+        assert st["n_pairs"] == fr.counts["n_pairs"]
+        assert np.array_equal(sp["tile"], tile) and np.array_equal(sp["depth"], depth) and np.array_equal(sp["gid"], gid)
