@@ -100,13 +100,16 @@ k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs)
         const bool cx0 = x >= tx0, cx1 = x + 1u < tx1, cy0 = y >= ty0, cy1 = y + 1u < ty1;   // x < tx1 and y < ty1 always hold
         const float4 add = make_float4(cx0 && cy0 ? 1.0f : 0.0f, cx1 && cy0 ? 1.0f : 0.0f,
                                        cx0 && cy1 ? 1.0f : 0.0f, cx1 && cy1 ? 1.0f : 0.0f);
-        const float4 old = atomicAdd(reinterpret_cast<float4 *>(ws.cursor4 + (size_t)(gy * (unsigned int)GX + gx) * kCtrStride), add);
-        const unsigned long long key = ((unsigned long long)s_depth[r] << 32) | (p0 + r);
+        // the four range starts are fetched BEFORE the atomic, so that their L2 round trips overlap its latency
         const unsigned int t00 = y * (unsigned int)TX + x;
-        if (cx0 && cy0) { const unsigned int pos = ws.ranges[t00].x + (unsigned int)old.x; if (pos < max_pairs) ws.pairs[pos] = key; }
-        if (cx1 && cy0) { const unsigned int pos = ws.ranges[t00 + 1].x + (unsigned int)old.y; if (pos < max_pairs) ws.pairs[pos] = key; }
-        if (cx0 && cy1) { const unsigned int pos = ws.ranges[t00 + TX].x + (unsigned int)old.z; if (pos < max_pairs) ws.pairs[pos] = key; }
-        if (cx1 && cy1) { const unsigned int pos = ws.ranges[t00 + TX + 1].x + (unsigned int)old.w; if (pos < max_pairs) ws.pairs[pos] = key; }
+        const unsigned int s00 = cx0 && cy0 ? ws.ranges[t00].x : 0u, s10 = cx1 && cy0 ? ws.ranges[t00 + 1].x : 0u;
+        const unsigned int s01 = cx0 && cy1 ? ws.ranges[t00 + TX].x : 0u, s11 = cx1 && cy1 ? ws.ranges[t00 + TX + 1].x : 0u;
+        const unsigned long long key = ((unsigned long long)s_depth[r] << 32) | (p0 + r);
+        const float4 old = atomicAdd(reinterpret_cast<float4 *>(ws.cursor4 + (size_t)(gy * (unsigned int)GX + gx) * kCtrStride), add);
+        if (cx0 && cy0) { const unsigned int pos = s00 + (unsigned int)old.x; if (pos < max_pairs) ws.pairs[pos] = key; }
+        if (cx1 && cy0) { const unsigned int pos = s10 + (unsigned int)old.y; if (pos < max_pairs) ws.pairs[pos] = key; }
+        if (cx0 && cy1) { const unsigned int pos = s01 + (unsigned int)old.z; if (pos < max_pairs) ws.pairs[pos] = key; }
+        if (cx1 && cy1) { const unsigned int pos = s11 + (unsigned int)old.w; if (pos < max_pairs) ws.pairs[pos] = key; }
     }
 }
 
