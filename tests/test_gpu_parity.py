@@ -373,3 +373,60 @@ def test_instrumented_counts_match_oracle(pkg, config0):
     assert abs(st["evals"] - int(E.sum())) <= max(20, 1e-3 * E.sum())
     assert st["ms_total"] > 0 and all(m >= 0 for m in st["ms_stage"])
     r.close()
+
+
+# ------------------------------------------------------------------------------------ materialised G_sel
+
+def test_subset_small_scenes_errors_and_empty_selection(pkg):
+    """flod_subset_* on small inputs: three levels with the paper's rho = 4 ladder, reference positions on and off the
+    camera; the error conventions; a snapshot that selects nothing renders the background."""
+    rng = np.random.default_rng(21)
+    lv = _rand_levels(rng, (300, 700, 2100), (0.2, 0.05, 0.0))
+    osc = OracleScene(lv, 0)
+    cam = camera(width=80, height=48, f=70.0, bg=(0.1, 0.2, 0.3))
+    r = make_renderer(pkg, lv, 0, 80, 48)
+    with pytest.raises(pkg.FlodError) as e:                      # no arena yet
+        r.subset_build((0.0, 0.0, 0.0), cam.fx, 1.0)
+    assert e.value.code == -7
+    with pytest.raises(pkg.FlodError) as e:
+        r.subset_set_arena(2, 4)
+    assert e.value.code == -2
+    r.subset_set_arena(1, 3)
+    with pytest.raises(pkg.FlodError) as e:                      # nothing built yet
+        r.render_subset(cam)
+    assert e.value.code == -1
+    with pytest.raises(pkg.FlodError) as e:
+        r.subset_swap()
+    assert e.value.code == -1
+    for bad in ((float("nan"), 0.0, 0.0, cam.fx, 1.0), (0.0, 0.0, 0.0, 0.0, 1.0), (0.0, 0.0, 0.0, cam.fx, -2.0)):
+        with pytest.raises(pkg.FlodError) as e:
+            r.subset_build(bad[:3], bad[3], bad[4])
+        assert e.value.code == -1
+    for ref, gamma in (((0.0, 0.0, 0.0), 1.0), ((0.3, -0.2, 1.0), 2.0), ((5.0, 5.0, -20.0), 0.5)):
+        r.subset_build(ref, cam.fx, gamma)
+        with pytest.raises(pkg.FlodError) as e:                  # one rebuild at a time
+            r.subset_build(ref, cam.fx, gamma)
+        assert e.value.code == -1
+        n_sel = r.subset_swap()
+        img = r.render_subset(cam).cpu().numpy()
+        st = r.get_stats()
+        fr = osc.frame(cam, 1, 3, gamma, ref_pos=ref)
+        c = fr.counts
+        assert n_sel == c["n_sel"] and (st["n_front"], st["n_vis"], st["n_pairs"]) == (c["n_front"], c["n_vis"], c["n_pairs"])
+        assert np.array_equal(r.debug_mask(), fr.mask)
+        assert np.array_equal(r.debug_tile_counts(fr.TX * fr.TY), fr.tile_counts)
+        pr = r.debug_projected(st["n_vis"])
+        vis = np.nonzero(fr.state == oracle.ST_VISIBLE)[0]
+        assert np.array_equal(pr["gid"], vis.astype(np.uint32)) and np.array_equal(pr["rect"], fr.rect[vis])
+        check_image(img, fr)
+    r.close()
+    # an empty coarse level and a reference far from everything: the fine level's band [0, d) holds nothing
+    lv2 = _rand_levels(rng, (0, 400), (0.05, 0.0))
+    r = make_renderer(pkg, lv2, 0, 80, 48)
+    r.subset_set_arena(1, 2)
+    r.subset_build((0.0, 0.0, -1000.0), cam.fx, 1.0)
+    assert r.subset_swap() == 0
+    img = r.render_subset(cam).cpu().numpy()
+    assert r.get_stats()["n_pairs"] == 0
+    assert np.array_equal(img, np.broadcast_to(np.float32(cam.bg)[:, None, None], img.shape))
+    r.close()
