@@ -24,9 +24,9 @@
  * Pins (tests/test_oracle_*.py, all run with -m "not gpu"): worked values of SPEC.md, closed form
  * of one isotropic Gaussian's footprint, two-layer compositing example, invariants on T and alpha,
  * band partition, tiled == brute force bit-exactly, numerical Jacobian of the pinhole map, SH
- * orthonormality by quadrature.
- * parity unpinned: the SH sign convention (R16) and the inherited constants 0.3, 1.3, 1e-4, 0.5
- * -- nothing in the paper fixes them.
+ * orthonormality by quadrature, SH basis == real combinations of scipy's complex harmonics.
+ * parity unpinned: the inherited constants 0.3, 1.3, 1e-4, 0.5 and which SH sign convention a
+ * trained model would use -- nothing in the paper fixes them.
  */
 #include <math.h>
 #include <stdint.h>

@@ -564,3 +564,22 @@ def test_sh_degree0_colour_and_view_dependence():
     # low-order bands against their textbook Cartesian forms: Y1 ~ (-y, z, -x), Y2[2] ~ 2z^2 - x^2 - y^2
     assert Y[1] == pytest.approx(-math.sqrt(3 / (4 * math.pi)) * d[1])
     assert Y[6] == pytest.approx(0.25 * math.sqrt(5 / math.pi) * (3 * d[2] ** 2 - 1))
+
+
+def test_sh_basis_equals_library_spherical_harmonics():
+    """R16 against a library routine: the 16 basis functions are the real combinations of scipy's complex spherical
+    harmonics Y_l^m (which carry the Condon-Shortley phase): sqrt(2) Im Y_l^|m| for m < 0, Y_l^0, sqrt(2) Re Y_l^m for
+    m > 0, in the order (l, m = -l..l).  This pins every sign of R16 to that stated definition (which sign convention a
+    trained model uses stays a convention)."""
+    from scipy.special import sph_harm_y
+    rng = np.random.default_rng(11)
+    for _ in range(50):
+        d = rng.normal(size=3)
+        d /= np.linalg.norm(d)
+        theta, phi = math.acos(d[2]), math.atan2(d[1], d[0])            # polar angle from +z, azimuth from +x
+        want = []
+        for l in range(4):
+            for m in range(-l, l + 1):
+                y = complex(sph_harm_y(l, abs(m), theta, phi))
+                want.append(math.sqrt(2) * y.imag if m < 0 else (y.real if m == 0 else math.sqrt(2) * y.real))
+        np.testing.assert_allclose(oracle.sh_basis(3, d), want, atol=1e-12)
