@@ -13,8 +13,12 @@ namespace flod {
 
 constexpr int kTile = FLOD_TILE;
 constexpr int kPreBlock = 256;            // duplication: visible Gaussians per block step
-constexpr int kGeoThreads = 256;          // geometry: threads per block, four consecutive Gaussians per thread
-constexpr int kGeoPer = 4;
+#ifndef FLOD_GEO_THREADS
+#define FLOD_GEO_THREADS 128
+#endif
+constexpr int kGeoThreads = FLOD_GEO_THREADS;   // geometry: threads per block, kGeoPer consecutive Gaussians per thread
+constexpr int kGeoPer = 1024 / kGeoThreads;     // a block scans 1024 Gaussians = one segment
+static_assert(kGeoPer % 4 == 0 && kGeoPer * kGeoThreads == 1024, "whole quads per thread, 1024 per block");
 constexpr int kGeoBlock = kGeoThreads * kGeoPer;
 constexpr int kSortCap = 4096;            // per-tile sort: lists up to this many keys are scattered into shared memory
 #ifndef FLOD_CTR_STRIDE

@@ -68,8 +68,11 @@ struct GeoSmem {
     unsigned long long pairs;
 };
 
+#ifndef FLOD_GEO_MINBLOCKS
+#define FLOD_GEO_MINBLOCKS 1
+#endif
 template <bool DEBUG>
-__global__ void __launch_bounds__(kGeoThreads)
+__global__ void __launch_bounds__(kGeoThreads, FLOD_GEO_MINBLOCKS)
 k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ FrameParams p)
 {
     __shared__ GeoSmem S;
@@ -85,15 +88,28 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
     // a1 level selection, a2 view transform and z cull (canonical fp32), then a conservative off-screen test that
     // needs no covariance.  What survives is a CANDIDATE; the candidates of the block are listed in gid order.
     unsigned int m_sel = 0, m_front = 0, m_cand = 0;
-    if (g0 < g_end && g0 + kGeoPer > p.first_gid) {
-        const float4 X = __ldg(reinterpret_cast<const float4 *>(sc.mx + g0));
-        const float4 Y = __ldg(reinterpret_cast<const float4 *>(sc.my + g0));
-        const float4 Z = __ldg(reinterpret_cast<const float4 *>(sc.mz + g0));
-        const float4 Q = __ldg(reinterpret_cast<const float4 *>(sc.rho2 + g0));
-        const float wx[4] = {X.x, X.y, X.z, X.w}, wy[4] = {Y.x, Y.y, Y.z, Y.w}, wz[4] = {Z.x, Z.y, Z.z, Z.w};
-        const float rho2[4] = {Q.x, Q.y, Q.z, Q.w};
+    {
+        // kGeoPer / 4 quads per thread, every load issued before the first use (bytes in flight are what a streaming
+        // kernel of short blocks lives on)
+        constexpr int NQ = kGeoPer / 4;
+        float wx[kGeoPer], wy[kGeoPer], wz[kGeoPer], rho2[kGeoPer];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
+        for (int q = 0; q < NQ; ++q) {
+            const long long gq = g0 + 4 * q;
+            float4 X = make_float4(0.f, 0.f, 0.f, 0.f), Y = X, Z = X, Q = X;
+            if (gq < g_end && gq + 4 > p.first_gid) {
+                X = __ldg(reinterpret_cast<const float4 *>(sc.mx + gq));
+                Y = __ldg(reinterpret_cast<const float4 *>(sc.my + gq));
+                Z = __ldg(reinterpret_cast<const float4 *>(sc.mz + gq));
+                Q = __ldg(reinterpret_cast<const float4 *>(sc.rho2 + gq));
+            }
+            wx[4 * q] = X.x; wx[4 * q + 1] = X.y; wx[4 * q + 2] = X.z; wx[4 * q + 3] = X.w;
+            wy[4 * q] = Y.x; wy[4 * q + 1] = Y.y; wy[4 * q + 2] = Y.z; wy[4 * q + 3] = Y.w;
+            wz[4 * q] = Z.x; wz[4 * q + 1] = Z.y; wz[4 * q + 2] = Z.z; wz[4 * q + 3] = Z.w;
+            rho2[4 * q] = Q.x; rho2[4 * q + 1] = Q.y; rho2[4 * q + 2] = Q.z; rho2[4 * q + 3] = Q.w;
+        }
+#pragma unroll
+        for (int k = 0; k < kGeoPer; ++k) {
             const long long g = g0 + k;
             if (g < p.first_gid || g >= g_end) continue;
             const int i = (int)(g - p.first_gid);
@@ -154,7 +170,7 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
         n_cand += t;
     }
 #pragma unroll
-    for (int k = 0; k < 4; ++k)
+    for (int k = 0; k < kGeoPer; ++k)
         if ((m_cand >> k) & 1u) S.cand[local++] = (unsigned short)(tid * kGeoPer + k);
     __syncthreads();
 
