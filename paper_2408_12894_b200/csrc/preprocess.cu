@@ -299,6 +299,9 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
     }
 }
 
+#ifndef FLOD_COLOUR_UNROLL
+#define FLOD_COLOUR_UNROLL 2
+#endif
 // ---- a4: colour of every visible Gaussian.  rgb = max(0, 0.5 + sum_k Y_k(dir) sh_k)  (R16)
 // LANES threads share one Gaussian.  LANES = 4 needs the degree-3 row layout written by the upload: the row is 12
 // float4; float4 number (4 i + j), i = 0..2, holds floats [4 i, 4 i + 4) of the 12 floats (k, channel) of the
@@ -313,61 +316,82 @@ k_colour(const SceneDev sc, const WorkspaceDev ws, int TX, int TY, unsigned int 
     const unsigned int per_block = 256 / LANES;
     const unsigned int seg = blockIdx.x - 1;             // one block per segment of k_geometry
     const unsigned int n_here = ws.seg_count[seg];
-    for (unsigned int j0 = 0; j0 < n_here; j0 += per_block) {
-        const unsigned int j = j0 + threadIdx.x / LANES;
-        const bool ok = j < n_here;
-        const unsigned int slot = seg * kGeoBlock + j;
-        float r = 0.0f, g = 0.0f, b = 0.0f;
-        unsigned int ci = 0;
-        if (ok) {
-            ci = slot;
-            const float4 dg = ws.dirgid[ci];
-            const float *row = sc.sh + (size_t)__float_as_uint(dg.w) * sc.sh_stride;
-            float Y[K];
-            const float inv = DEG >= 1 ? 1.0f / sqrtf(dg.x * dg.x + dg.y * dg.y + dg.z * dg.z) : 0.0f;
-            if constexpr (LANES == 4) {
-                static_assert(DEG == 3 || LANES == 1, "4-lane layout is degree 3 only");
-                const float4 *r4 = reinterpret_cast<const float4 *>(row);
-                const float4 f0 = __ldg(r4 + sub), f1 = __ldg(r4 + 4 + sub), f2 = __ldg(r4 + 8 + sub);
-                sh_basis<DEG>(dg.x * inv, dg.y * inv, dg.z * inv, Y);
+    // U Gaussians per lane group and step: the U direction records are loaded first, then the U SH rows, then the
+    // arithmetic -- two dependent round trips to memory per step instead of per Gaussian
+    constexpr int U = FLOD_COLOUR_UNROLL;
+    for (unsigned int j0 = 0; j0 < n_here; j0 += U * per_block) {
+        bool ok[U];
+        unsigned int ci[U];
+        float4 dg[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const unsigned int j = j0 + u * per_block + threadIdx.x / LANES;
+            ok[u] = j < n_here;
+            ci[u] = seg * kGeoBlock + j;
+            dg[u] = ok[u] ? ws.dirgid[ci[u]] : make_float4(0.f, 0.f, 1.f, 0.f);
+        }
+        float r[U], g[U], b[U];
+        if constexpr (LANES == 4) {
+            static_assert(DEG == 3 || LANES == 1, "4-lane layout is degree 3 only");
+            float4 f0[U], f1[U], f2[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                f0[u] = f1[u] = f2[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (ok[u]) {
+                    const float4 *r4 = reinterpret_cast<const float4 *>(sc.sh + (size_t)__float_as_uint(dg[u].w) * sc.sh_stride);
+                    f0[u] = __ldg(r4 + sub); f1[u] = __ldg(r4 + 4 + sub); f2[u] = __ldg(r4 + 8 + sub);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                float Y[K];
+                const float inv = 1.0f / sqrtf(dg[u].x * dg[u].x + dg[u].y * dg[u].y + dg[u].z * dg[u].z);
+                sh_basis<DEG>(dg[u].x * inv, dg[u].y * inv, dg[u].z * inv, Y);
                 const float y0 = sub == 0 ? Y[0] : sub == 1 ? Y[4] : sub == 2 ? Y[8] : Y[12];
                 const float y1 = sub == 0 ? Y[1] : sub == 1 ? Y[5] : sub == 2 ? Y[9] : Y[13];
                 const float y2 = sub == 0 ? Y[2] : sub == 1 ? Y[6] : sub == 2 ? Y[10] : Y[14];
                 const float y3 = sub == 0 ? Y[3] : sub == 1 ? Y[7] : sub == 2 ? Y[11] : Y[15];
-                r = fmaf(y0, f0.x, fmaf(y1, f0.w, fmaf(y2, f1.z, y3 * f2.y)));
-                g = fmaf(y0, f0.y, fmaf(y1, f1.x, fmaf(y2, f1.w, y3 * f2.z)));
-                b = fmaf(y0, f0.z, fmaf(y1, f1.y, fmaf(y2, f2.x, y3 * f2.w)));
-            } else {
+                r[u] = fmaf(y0, f0[u].x, fmaf(y1, f0[u].w, fmaf(y2, f1[u].z, y3 * f2[u].y)));
+                g[u] = fmaf(y0, f0[u].y, fmaf(y1, f1[u].x, fmaf(y2, f1[u].w, y3 * f2[u].z)));
+                b[u] = fmaf(y0, f0[u].z, fmaf(y1, f1[u].y, fmaf(y2, f2[u].x, y3 * f2[u].w)));
+#pragma unroll
+                for (int o = 1; o < 4; o <<= 1) {
+                    r[u] += __shfl_xor_sync(0xffffffffu, r[u], o);
+                    g[u] += __shfl_xor_sync(0xffffffffu, g[u], o);
+                    b[u] += __shfl_xor_sync(0xffffffffu, b[u], o);
+                }
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                r[u] = g[u] = b[u] = 0.0f;
+                if (!ok[u]) continue;
                 constexpr int NF = (3 * K + 3) / 4 * 4;
-                float f[NF];
-                const float4 *r4 = reinterpret_cast<const float4 *>(row);
+                float f[NF], Y[K];
+                const float4 *r4 = reinterpret_cast<const float4 *>(sc.sh + (size_t)__float_as_uint(dg[u].w) * sc.sh_stride);
 #pragma unroll
                 for (int q = 0; q < NF / 4; ++q) {
                     const float4 t = __ldg(r4 + q);
                     f[4 * q] = t.x; f[4 * q + 1] = t.y; f[4 * q + 2] = t.z; f[4 * q + 3] = t.w;
                 }
-                sh_basis<DEG>(dg.x * inv, dg.y * inv, dg.z * inv, Y);
+                const float inv = DEG >= 1 ? 1.0f / sqrtf(dg[u].x * dg[u].x + dg[u].y * dg[u].y + dg[u].z * dg[u].z) : 0.0f;
+                sh_basis<DEG>(dg[u].x * inv, dg[u].y * inv, dg[u].z * inv, Y);
 #pragma unroll
                 for (int k = 0; k < K; ++k) {
-                    r = fmaf(Y[k], f[3 * k], r);
-                    g = fmaf(Y[k], f[3 * k + 1], g);
-                    b = fmaf(Y[k], f[3 * k + 2], b);
+                    r[u] = fmaf(Y[k], f[3 * k], r[u]);
+                    g[u] = fmaf(Y[k], f[3 * k + 1], g[u]);
+                    b[u] = fmaf(Y[k], f[3 * k + 2], b[u]);
                 }
             }
         }
-        if constexpr (LANES == 4) {
 #pragma unroll
-            for (int o = 1; o < 4; o <<= 1) {
-                r += __shfl_xor_sync(0xffffffffu, r, o);
-                g += __shfl_xor_sync(0xffffffffu, g, o);
-                b += __shfl_xor_sync(0xffffffffu, b, o);
+        for (int u = 0; u < U; ++u) {
+            if (ok[u] && sub == 0) {
+                const float rr = fmaxf(r[u] + 0.5f, 0.0f), gg = fmaxf(g[u] + 0.5f, 0.0f), bb = fmaxf(b[u] + 0.5f, 0.0f);
+                reinterpret_cast<float2 *>(ws.gB)[2 * (size_t)ci[u] + 1] = make_float2(rr, gg);
+                ws.cB[ci[u]] = bb;
+                if (DEBUG) { ws.dbg[ci[u]].rgb[0] = rr; ws.dbg[ci[u]].rgb[1] = gg; ws.dbg[ci[u]].rgb[2] = bb; }
             }
-        }
-        if (ok && sub == 0) {
-            r = fmaxf(r + 0.5f, 0.0f); g = fmaxf(g + 0.5f, 0.0f); b = fmaxf(b + 0.5f, 0.0f);
-            reinterpret_cast<float2 *>(ws.gB)[2 * (size_t)ci + 1] = make_float2(r, g);
-            ws.cB[ci] = b;
-            if (DEBUG) { ws.dbg[ci].rgb[0] = r; ws.dbg[ci].rgb[1] = g; ws.dbg[ci].rgb[2] = b; }
         }
     }
 }
