@@ -58,7 +58,7 @@ __device__ __forceinline__ unsigned int block_min_u32(SortSmem &S, unsigned int 
 }
 
 #ifndef FLOD_SORT_UNROLL
-#define FLOD_SORT_UNROLL 8
+#define FLOD_SORT_UNROLL 6
 #endif
 constexpr int kSortU = FLOD_SORT_UNROLL;                  // keys a thread holds in registers / loads in flight per step
 
