@@ -1,6 +1,8 @@
 """Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (config 1 / config 2):
 5.35M Gaussians, SH degree 3, 1237x822.  Masks, frame counters and per-tile pair counts are checked exactly on
 several poses and gammas; full images are checked on sampled poses (the oracle needs seconds per frame)."""
+import os
+
 import numpy as np
 import pytest
 
@@ -79,7 +81,9 @@ def test_config1_max_level_other_poses(full, pose):
 def test_config2_selective_masks_and_counts_exact(full, gamma):
     """BASELINE.json config 2: selective {3,4,5}, gamma in {1,2,4}: masks and per-tile pair counts exactly."""
     scene, cams, osc, r = full
-    for pose in (0, 50, 150):
+    # FLOD_FULL_SWEEP=1: all 200 poses (SURVEY 8(d) config 2; ~3 minutes per gamma, so not the default)
+    poses = range(len(cams)) if os.environ.get("FLOD_FULL_SWEEP") else (0, 50, 150)
+    for pose in poses:
         img, fr, st = _geometry_exact(r, osc, cams[pose], 3, 5, gamma)
         if pose == 50:
             check_image(img, fr)
