@@ -430,3 +430,33 @@ def test_subset_small_scenes_errors_and_empty_selection(pkg):
     assert r.get_stats()["n_pairs"] == 0
     assert np.array_equal(img, np.broadcast_to(np.float32(cam.bg)[:, None, None], img.shape))
     r.close()
+
+
+@pytest.mark.parametrize("seed", [100, 102, 105, 108, 111, 114, 120, 132])
+def test_random_scenes_every_kernel_path(pkg, seed):
+    """Random level counts, SH degrees, image sizes and footprints (every third seed: large footprints, mean rect area
+    up to hundreds of tiles -> k_duplicate_shared; every fourth: its tile windows), every checked intermediate and the
+    image on the fused path, then the materialised-subset path at a random reference: bit-identical to the fused
+    predicate and within tolerance of the oracle."""
+    rng = np.random.default_rng(seed)
+    L = int(rng.integers(1, 4)); deg = int(rng.integers(0, 4))
+    counts = tuple(int(x) for x in rng.integers(0, 6000, L))
+    s_min = np.sort(np.exp(rng.uniform(-4, -1, L)))[::-1].copy(); s_min[-1] = 0.0
+    lv = _rand_levels(rng, counts, s_min, sh_degree=deg, logs=((-1.5, 0.5) if seed % 3 == 0 else (-4.0, -1.0)))
+    W, H = int(rng.integers(16, 400)), int(rng.integers(16, 300))
+    cam = camera(width=W, height=H, f=float(rng.uniform(40, 300)), bg=tuple(rng.uniform(0, 1, 3)))
+    osc = OracleScene(lv, deg)
+    r = make_renderer(pkg, lv, deg, W, H, max_pairs=1 << 23)
+    if seed % 4 == 0:
+        r.set_options(pkg.FLOD_OPT_DEBUG | pkg.FLOD_OPT_SMALL_WINDOWS)
+    check_frame(r, osc, cam, L, L, 1.0)
+    check_frame(r, osc, cam, 1, L, float(rng.uniform(0.5, 4)))
+    ref = rng.uniform(-2, 2, 3).astype(np.float32); gamma = float(rng.uniform(0.5, 4))
+    r.subset_set_arena(1, L); r.subset_build(ref, cam.fx, gamma); r.subset_swap()
+    a = r.render_subset(cam).cpu().numpy()
+    r.set_selection_reference(ref)
+    b = r.render(cam, 1, L, gamma).cpu().numpy()
+    r.set_selection_reference(None)
+    assert np.array_equal(a, b)
+    check_image(a, osc.frame(cam, 1, L, gamma, ref_pos=ref))
+    r.close()
