@@ -43,12 +43,20 @@ def parse_args():
     ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--mode", default=None, help="max | level<l> | sel<ls><le> e.g. sel345; default per config")
     ap.add_argument("--gamma", type=float, default=1.0)
+    ap.add_argument("--size", default=None, help="WxH, e.g. 1920x1080 (config 4's second image size); default per config")
     ap.add_argument("--subset-period", type=int, default=0,
                     help="selective modes only: render from a materialised G_sel (flod_render_subset) that is rebuilt "
                          "every N frames on a second stream and swapped in when ready (P:699-711); 0 = Eq. 6 per frame")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--count-scale", type=float, default=1.0, help="shrink the scene (debugging only; reported)")
     return ap.parse_args()
+
+
+def image_size(args):
+    if not args.size:
+        return (None, None)
+    w, h = args.size.lower().split("x")
+    return (int(w), int(h))
 
 
 def mode_levels(args, n_levels):
@@ -181,7 +189,7 @@ def run_reference(args):
     import flod_synth as fs
     import oracle
     scene = fs.make_scene(args.config, count_scale=args.count_scale)
-    cams = fs.make_poses(args.config)
+    cams = fs.make_poses(args.config, *image_size(args))
     mode, ls, le = mode_levels(args, len(scene.levels))
     K = args.steps if args.steps is not None else 5
     W = args.warmup if args.warmup is not None else 1
@@ -276,7 +284,7 @@ def run_ours(args):
     W = args.warmup if args.warmup is not None else 10
     W = max(W, 3)
     scene = fs.make_scene(args.config, count_scale=args.count_scale)
-    cams = fs.make_poses(args.config)
+    cams = fs.make_poses(args.config, *image_size(args))
     mode, ls, le = mode_levels(args, len(scene.levels))
     cs = [camera_struct(c) for c in cams]
     cam0 = cams[0]
