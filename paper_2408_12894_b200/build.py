@@ -47,5 +47,20 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_peak_fp32() -> str:
+    """The standalone FP32-pipe microbenchmark (csrc/peak_fp32.cu) -> paper_2408_12894_b200/peak_fp32."""
+    out = os.path.join(HERE, "peak_fp32")
+    src = os.path.join(CSRC, "peak_fp32.cu")
+    if os.path.exists(out) and os.path.getmtime(out) >= os.path.getmtime(src):
+        return out
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    r = subprocess.run([nvcc, "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", src, "-o", out],
+                       capture_output=True, text=True)
+    if r.returncode:
+        sys.stderr.write(r.stdout + r.stderr)
+        raise RuntimeError("nvcc failed building peak_fp32")
+    return out
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
