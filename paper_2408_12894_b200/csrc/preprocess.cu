@@ -13,6 +13,11 @@
 #include "flod_internal.cuh"
 #include "tile_scan.cuh"
 
+// An SH row is read once per frame and never again: evict-first (ld.global.cs) loads keep the 300 MB of rows from
+// pushing the frame's L2-resident workspace out (k_colour 63 -> 56 us on config 1).  The same on the planes k_geometry
+// reads changed nothing.
+#define FLOD_LD_STREAM(p) __ldcs(p)
+
 namespace flod {
 
 __device__ __forceinline__ float fmul(float a, float b) { return __fmul_rn(a, b); }
@@ -339,7 +344,7 @@ k_colour(const SceneDev sc, const WorkspaceDev ws, int TX, int TY, unsigned int 
                 f0[u] = f1[u] = f2[u] = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (ok[u]) {
                     const float4 *r4 = reinterpret_cast<const float4 *>(sc.sh + (size_t)__float_as_uint(dg[u].w) * sc.sh_stride);
-                    f0[u] = __ldg(r4 + sub); f1[u] = __ldg(r4 + 4 + sub); f2[u] = __ldg(r4 + 8 + sub);
+                    f0[u] = FLOD_LD_STREAM(r4 + sub); f1[u] = FLOD_LD_STREAM(r4 + 4 + sub); f2[u] = FLOD_LD_STREAM(r4 + 8 + sub);
                 }
             }
 #pragma unroll
@@ -371,7 +376,7 @@ k_colour(const SceneDev sc, const WorkspaceDev ws, int TX, int TY, unsigned int 
                 const float4 *r4 = reinterpret_cast<const float4 *>(sc.sh + (size_t)__float_as_uint(dg[u].w) * sc.sh_stride);
 #pragma unroll
                 for (int q = 0; q < NF / 4; ++q) {
-                    const float4 t = __ldg(r4 + q);
+                    const float4 t = FLOD_LD_STREAM(r4 + q);
                     f[4 * q] = t.x; f[4 * q + 1] = t.y; f[4 * q + 2] = t.z; f[4 * q + 3] = t.w;
                 }
                 const float inv = DEG >= 1 ? 1.0f / sqrtf(dg[u].x * dg[u].x + dg[u].y * dg[u].y + dg[u].z * dg[u].z) : 0.0f;
