@@ -391,27 +391,39 @@ orc_frame *orc_frame_create(const orc_scene *sc, const orc_camera *cam, int l_st
     }
     fr->n_sel = n_sel; fr->n_front = n_front; fr->n_vis = n_vis; fr->n_pairs = n_pairs; fr->n_bf = n_bf;
 
-    /* O6: pairs in ascending gid, tiles of the rect in row-major order; then the canonical order */
+    /* O6: every tile's list = the visible Gaussians whose rect holds the tile, appended in ascending gid, then ordered
+     * by (depth, gid) ("in depth order"; DESIGN R15).  The lists are stored tile after tile, so the whole array
+     * is in (tile, depth, gid) order -- the same unique sequence one sort of all pairs by that triple gives (the
+     * first version of this function did exactly that; per-tile lists sort in parallel and are what O7 walks). */
     fr->pairs = (orc_pair *)malloc(sizeof(orc_pair) * (size_t)(n_pairs > 0 ? n_pairs : 1));
     fr->bf_list = (uint32_t *)malloc(sizeof(uint32_t) * (size_t)(n_bf > 0 ? n_bf : 1));
-    int64_t p = 0, q = 0;
+    int T_n = fr->TX * fr->TY;
+    fr->tile_start = (uint32_t *)calloc((size_t)T_n + 1, sizeof(uint32_t));
+    int64_t q = 0;
     for (int64_t g = 0; g < n; ++g) {
         if (fr->state[g] >= ST_EMPTY_RECT) fr->bf_list[q++] = (uint32_t)g;
         if (fr->state[g] != ST_VISIBLE) continue;
         const int32_t *r = fr->rect + 4 * g;
         for (int ty = r[1]; ty < r[3]; ++ty)
+            for (int tx = r[0]; tx < r[2]; ++tx) fr->tile_start[ty * fr->TX + tx + 1]++;
+    }
+    for (int tI = 0; tI < T_n; ++tI) fr->tile_start[tI + 1] += fr->tile_start[tI];
+    uint32_t *fill = (uint32_t *)malloc(sizeof(uint32_t) * (size_t)(T_n > 0 ? T_n : 1));
+    memcpy(fill, fr->tile_start, sizeof(uint32_t) * (size_t)T_n);
+    for (int64_t g = 0; g < n; ++g) {
+        if (fr->state[g] != ST_VISIBLE) continue;
+        const int32_t *r = fr->rect + 4 * g;
+        for (int ty = r[1]; ty < r[3]; ++ty)
             for (int tx = r[0]; tx < r[2]; ++tx) {
-                fr->pairs[p].tile = (uint32_t)(ty * fr->TX + tx);
-                fr->pairs[p].depth = fr->depth[g];
-                fr->pairs[p].gid = (uint32_t)g;
-                ++p;
+                uint32_t tile = (uint32_t)(ty * fr->TX + tx);
+                orc_pair *pp = fr->pairs + fill[tile]++;
+                pp->tile = tile; pp->depth = fr->depth[g]; pp->gid = (uint32_t)g;
             }
     }
-    qsort(fr->pairs, (size_t)n_pairs, sizeof(orc_pair), cmp_pair);
-    int T_n = fr->TX * fr->TY;
-    fr->tile_start = (uint32_t *)calloc((size_t)T_n + 1, sizeof(uint32_t));
-    for (int64_t i = 0; i < n_pairs; ++i) fr->tile_start[fr->pairs[i].tile + 1]++;
-    for (int tI = 0; tI < T_n; ++tI) fr->tile_start[tI + 1] += fr->tile_start[tI];
+    free(fill);
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int tI = 0; tI < T_n; ++tI)
+        qsort(fr->pairs + fr->tile_start[tI], (size_t)(fr->tile_start[tI + 1] - fr->tile_start[tI]), sizeof(orc_pair), cmp_pair);
     return fr;
 }
 

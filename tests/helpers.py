@@ -29,11 +29,11 @@ def level(level_id, s_min, mean, scale, quat=None, opacity=None, rgb=None, sh=No
                            sh=np.ascontiguousarray(sh, dtype=np.float32))
 
 
-def camera(width=33, height=33, f=100.0, R=None, t=None, z_near=0.2, bg=(0.0, 0.0, 0.0), cx=None, cy=None):
-    """Identity pose by default: camera at the origin looking down +z, +x right, +y down."""
+def camera(width=33, height=33, f=100.0, R=None, t=None, z_near=0.2, bg=(0.0, 0.0, 0.0), cx=None, cy=None, fy=None):
+    """Identity pose by default: camera at the origin looking down +z, +x right, +y down.  f is fx; fy defaults to it."""
     return SimpleNamespace(R=np.eye(3, dtype=np.float32) if R is None else np.asarray(R, dtype=np.float32),
                            t=np.zeros(3, dtype=np.float32) if t is None else np.asarray(t, dtype=np.float32),
-                           fx=float(np.float32(f)), fy=float(np.float32(f)),
+                           fx=float(np.float32(f)), fy=float(np.float32(f if fy is None else fy)),
                            cx=float(np.float32(width / 2.0 if cx is None else cx)),
                            cy=float(np.float32(height / 2.0 if cy is None else cy)),
                            width=width, height=height, z_near=float(np.float32(z_near)), bg=tuple(bg))

@@ -317,6 +317,107 @@ def test_tile_rect_covers_the_threshold_contour():
     assert fr.counts["n_pairs"] == int(fr.n_tiles[fr.state == oracle.ST_VISIBLE].sum()) == int(fr.tile_counts.sum())
 
 
+def _aniso_camera(rng=None, **kw):
+    """fx != fy and a principal point off the image centre: every fy / cy / lim_y term of O2-O4 and R4's choice of fx
+    are invisible to a camera with fx == fy, cx = W/2, cy = H/2 (a swap changes nothing there)."""
+    d = dict(width=208, height=136, f=190.0, fy=127.0, cx=81.25, cy=90.5)
+    d.update(kw)
+    return camera(**d)
+
+
+def test_anisotropic_camera_projection_and_covariance():
+    """P:110, S:142-146 with fx != fy, cx != W/2, cy != H/2: on-axis point -> (cx, cy); mu' = (fx x/z + cx, fy y/z + cy);
+    isotropic on-axis Sigma' = diag((fx s/d)^2, (fy s/d)^2) + 0.3 I; Sigma' against the numerical Jacobian."""
+    cam = _aniso_camera()
+    f, s, d = 250.0, 0.05, 4.0
+    fr = OracleScene([level(1, 0.0, [[0, 0, d]], s)], 0).frame(cam, 1, 1, 1.0)
+    np.testing.assert_array_equal(fr.mu2d[0], [np.float32(81.25), np.float32(90.5)])
+    a, b, c = fr.cov2d[0]
+    assert a == pytest.approx((cam.fx * s / d) ** 2 + 0.3, rel=1e-6) and c == pytest.approx((cam.fy * s / d) ** 2 + 0.3, rel=1e-6)
+    assert abs(b) < 1e-6 and a > 1.5 * c
+    rng = np.random.default_rng(211)
+    for _ in range(30):
+        Rc, _ = random_rotation(rng)
+        eye = rng.normal(0, 1, 3)
+        cam = _aniso_camera(R=Rc, t=-Rc @ eye, f=float(rng.uniform(100, 300)), fy=float(rng.uniform(100, 300)),
+                            cx=float(rng.uniform(40, 160)), cy=float(rng.uniform(30, 100)))
+        p_cam = np.array([rng.uniform(-0.3, 0.3), rng.uniform(-0.2, 0.2), 1.0]) * rng.uniform(1.0, 6.0)
+        mu = Rc.T @ p_cam + eye
+        sc3 = np.exp(rng.uniform(-3.5, -1.5, 3))
+        Rg, q = random_rotation(rng)
+        fr = OracleScene([level(1, 0.0, [mu], [sc3], quat=[q])], 0).frame(cam, 1, 1, 1.0)
+        pc = cam.R.astype(np.float64) @ np.float32(mu).astype(np.float64) + cam.t.astype(np.float64)
+        np.testing.assert_allclose(fr.mu2d[0], _pinhole(pc, cam), rtol=2e-6, atol=2e-4)
+        h = 1e-5
+        J = np.stack([(_pinhole(pc + h * e, cam) - _pinhole(pc - h * e, cam)) / (2 * h) for e in np.eye(3)], axis=1)
+        want = J @ cam.R.astype(np.float64) @ (Rg @ np.diag(sc3 * sc3) @ Rg.T) @ cam.R.astype(np.float64).T @ J.T
+        a, b, c = fr.cov2d[0].astype(np.float64)
+        np.testing.assert_allclose([[a - 0.3, b], [b, c - 0.3]], want, rtol=2e-4, atol=2e-5 * np.abs(want).max())
+
+
+def test_anisotropic_camera_jacobian_clamp_uses_its_own_axis():
+    """R8 with fx != fy: x/z is clamped at 1.3 W / (2 fx), y/z at 1.3 H / (2 fy) -- each with its own focal length and
+    image extent (a swapped pair of limits changes Sigma' of a Gaussian beside the frustum)."""
+    cam = _aniso_camera(width=208, height=136, f=120.0, fy=210.0)
+    limx, limy = 1.3 * cam.width / (2 * cam.fx), 1.3 * cam.height / (2 * cam.fy)
+    assert abs(limx - limy) > 0.1
+    s, z = 0.05, 2.0
+    pos = [[3.0 * limx * z, 0, z], [0, 3.0 * limy * z, z], [0.9 * limx * z, 0.9 * limy * z, z]]
+    fr = OracleScene([level(1, 0.0, pos, s)], 0).frame(cam, 1, 1, 1.0)
+    for g, (u, v) in enumerate(((limx, 0.0), (0.0, limy), (0.9 * limx, 0.9 * limy))):
+        J = np.array([[cam.fx / z, 0, -cam.fx * u / z], [0, cam.fy / z, -cam.fy * v / z]])
+        want = J @ (s * s * np.eye(3)) @ J.T + 0.3 * np.eye(2)
+        a, b, c = fr.cov2d[g]
+        np.testing.assert_allclose([[a, b], [b, c]], want, rtol=1e-5, atol=1e-6)
+
+
+def test_band_thresholds_use_fx_when_fx_differs_from_fy():
+    """R4 (Eq. 7 "the focal length f"): f = fx.  fx = 1000, fy = 500, s_min = 0.05, gamma = 1 puts the
+    edge at 50 (25 if fy were taken): a Gaussian at distance 40 belongs to the finer level, one at 60 to the coarser."""
+    pos = np.array([[40.0, 0.0, 0.0], [60.0, 0.0, 0.0], [0.0, 24.0, 0.0], [0.0, 26.0, 0.0]])
+    sc = _same_positions_scene(pos, [4, 5], [0.05, 0.0])
+    fr = sc.frame(_aniso_camera(f=1000.0, fy=500.0), 4, 5, 1.0, ref_pos=[0.0, 0.0, 0.0])
+    assert fr.mask.reshape(2, 4).tolist() == [[0, 1, 0, 0], [1, 0, 1, 1]]
+    lo, hi = fr.thresholds()
+    assert lo[0] == np.float32(2500.0)
+
+
+def test_anisotropic_camera_tile_rect_and_footprint():
+    """R13 / O4 with fx != fy and an off-centre principal point: the rect is still the padded box of the alpha = 1/255
+    contour around mu' = (fx x/z + cx, fy y/z + cy); the blended pixels of one isotropic on-axis Gaussian are exactly
+    those inside the axis-aligned ellipse with semi-axes sigma'_x,y sqrt(2 ln(255 o)) centred on (cx, cy)."""
+    rng = np.random.default_rng(45)
+    cam = _aniso_camera()
+    n = 300
+    pos = np.stack([rng.uniform(-3, 3, n), rng.uniform(-2, 2, n), rng.uniform(0.5, 6, n)], axis=1)
+    lv = level(1, 0.0, pos, np.exp(rng.uniform(-4, -1, (n, 3))), quat=rng.normal(size=(n, 4)), opacity=rng.uniform(0.01, 0.99, n))
+    sc = OracleScene([lv], 0)
+    fr = sc.frame(cam, 1, 1, 1.0)
+    TX, TY = fr.TX, fr.TY
+    for g in np.nonzero(fr.state >= oracle.ST_EMPTY_RECT)[0]:
+        a, b, c = fr.cov2d[g].astype(np.float64)
+        kap = 2 * math.log(255 * float(sc.opacity[g]))
+        hx, hy = math.sqrt(kap * a), math.sqrt(kap * c)
+        pc = np.float32(pos[g]).astype(np.float64)
+        mx, my = cam.fx * pc[0] / pc[2] + cam.cx, cam.fy * pc[1] / pc[2] + cam.cy     # from the definition, not from fr
+        x0 = min(max(math.floor((mx - hx) / 16), 0), TX); x1 = min(max(math.floor((mx + hx) / 16) + 1, 0), TX)
+        y0 = min(max(math.floor((my - hy) / 16), 0), TY); y1 = min(max(math.floor((my + hy) / 16) + 1, 0), TY)
+        r = fr.rect[g]
+        assert r[0] <= x0 and r[1] <= y0 and r[2] >= x1 and r[3] >= y1
+        assert r[0] >= x0 - 1 and r[1] >= y0 - 1 and r[2] <= x1 + 1 and r[3] <= y1 + 1
+    o, s, d = 0.8, 0.1, 2.0
+    fr = OracleScene([level(1, 0.0, [[0, 0, d]], s, opacity=o, rgb=[1.0, 1.0, 1.0])], 0).frame(cam, 1, 1, 1.0)
+    img, E, B, T = fr.composite(stats=True)
+    sx2, sy2 = (cam.fx * s / d) ** 2 + 0.3, (cam.fy * s / d) ** 2 + 0.3
+    jj, ii = np.mgrid[0:cam.height, 0:cam.width]
+    q = 0.5 * ((ii + 0.5 - cam.cx) ** 2 / sx2 + (jj + 0.5 - cam.cy) ** 2 / sy2)
+    alpha = np.minimum(0.99, float(np.float32(1 / (1 + math.exp(-math.log(o / (1 - o)))))) * np.exp(-q))
+    inside = alpha >= SKIP_THR
+    edge = np.abs(alpha - SKIP_THR) < 1e-6
+    assert np.array_equal(B[~edge] > 0, inside[~edge]) and inside.sum() > 500
+    np.testing.assert_allclose(img[0][inside & ~edge], alpha[inside & ~edge], rtol=2e-5)
+
+
 # ------------------------------------------------------------------------- compositing (O7)
 
 def test_empty_set_renders_background():
@@ -500,6 +601,28 @@ def test_depth_ties_break_by_gid():
     lo = [level(1, 0.1, [pos[0]], 0.2, opacity=0.5, rgb=[rgb[1]]), level(2, 0.05, [pos[1]], 0.2, opacity=0.5, rgb=[rgb[0]])]
     same = OracleScene([level(1, 0.0, pos, 0.2, opacity=0.5, rgb=[rgb[1], rgb[0]])], 0).frame(camera(33, 33, 100.0), 1, 1, 1.0)
     np.testing.assert_allclose(same.composite()[:, 16, 16], [0.25, 0.0, 0.5], atol=1e-7)
+
+
+def test_pair_sequence_equals_one_global_sort_of_all_pairs():
+    """O6 / R15: the oracle's per-tile lists, tile after tile, are the unique sequence that sorting ALL
+    (tile, depth, gid) triples with a library sort gives (numpy lexsort over the pairs expanded from the rects here)."""
+    import flod_synth as fs
+    sc = fs.make_scene(1, count_scale=0.01)
+    cam = fs.make_poses(1, 320, 208)[7]
+    fr = OracleScene(sc.levels, sc.sh_degree).frame(cam, 3, 5, 2.0)
+    vis = np.nonzero(fr.state == oracle.ST_VISIBLE)[0]
+    rect, depth = fr.rect[vis], fr.depth[vis]
+    tiles, deps, gids = [], [], []
+    for g, r, d in zip(vis, rect, depth):
+        ty, tx = np.mgrid[r[1]:r[3], r[0]:r[2]]
+        t = (ty * fr.TX + tx).ravel()
+        tiles.append(t); deps.append(np.full(t.size, d, np.float32)); gids.append(np.full(t.size, g, np.uint32))
+    tiles, deps, gids = np.concatenate(tiles).astype(np.uint32), np.concatenate(deps), np.concatenate(gids)
+    order = np.lexsort((gids, deps, tiles))
+    tile, dep, gid = fr.sorted_pairs()
+    assert tile.size == fr.counts["n_pairs"] > 10000
+    assert np.array_equal(tile, tiles[order]) and np.array_equal(dep, deps[order]) and np.array_equal(gid, gids[order])
+    assert np.array_equal(fr.tile_counts, np.bincount(tiles, minlength=fr.TX * fr.TY).astype(np.uint32))
 
 
 def test_rigid_motion_invariance():
