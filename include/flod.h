@@ -88,7 +88,8 @@ typedef struct {
     int64_t n_vis;                   /* also alive, det > 0, non-empty tile rect */
     int64_t n_pairs;                 /* (Gaussian, tile) pairs the frame REQUIRES (may exceed max_pairs) */
     int64_t max_pairs;               /* capacity given to flod_set_workspace */
-    int     overflow;                /* 1 when n_pairs > max_pairs: out_rgb of that frame is undefined */
+    int     overflow;                /* non-zero: out_rgb of that frame is undefined.  bit 0: n_pairs > max_pairs (grow the
+                                        workspace); bit 1: one tile's list exceeds 2^24 entries (a larger workspace does not help) */
     int64_t evals, blends;           /* E, B of DESIGN §6 when FLOD_OPT_COUNT is on, else 0 */
     float   ms_stage[FLOD_N_STAGES]; /* device time per stage when FLOD_OPT_PROFILE is on, else 0 */
     float   ms_total;
@@ -150,12 +151,14 @@ FLOD_API int flod_set_options(flod_ctx *ctx, unsigned flags);
 /* Steps a1-a9 for one frame, asynchronous on `stream` (a cudaStream_t passed as void*).
  * out_rgb_dev: [3][height][width] planar fp32.  Errors detected on the host are returned here; a capacity
  * overflow is detected on the device: the frame is not silently truncated -- out_rgb is undefined, and
- * flod_get_stats reports overflow = 1 and the required n_pairs so the caller can grow the workspace. */
+ * flod_get_stats reports the overflow bits and the required n_pairs so the caller can grow the workspace.
+ * cam->R must be a rotation (max |R R^T - I| <= 1e-4), else FLOD_E_INVALID_ARG. */
 FLOD_API int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma,
                 float *out_rgb_dev, void *stream);
 
 /* Same, end to end with HOST buffers: renders into an image of the workspace and copies it to out_rgb_host
- * ([3][height][width] fp32, ideally pinned) on `stream`, then waits for the copy. */
+ * ([3][height][width] fp32, ideally pinned) on `stream`, then waits for the copy.  The frame's overflow word travels
+ * with the image: FLOD_E_CAPACITY is returned (and the image is undefined) when the frame overflowed. */
 FLOD_API int flod_render_to_host(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma,
                         float *out_rgb_host, void *stream);
 
@@ -167,7 +170,8 @@ FLOD_API int flod_render_to_host(flod_ctx *ctx, const flod_camera *cam, flod_lev
 FLOD_API int flod_render_to_host_async(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma,
                               float *out_rgb_host, void *stream, void *copy_stream);
 
-/* Blocks the calling host thread until every copy issued by flod_render_to_host_async has landed. */
+/* Blocks the calling host thread until every copy issued by flod_render_to_host_async has landed.  Returns
+ * FLOD_E_CAPACITY if one of the frames waited for overflowed (its image is undefined). */
 FLOD_API int flod_wait_host(flod_ctx *ctx);
 
 /* ---- Materialised G_sel (Eq. 6) reused over a run of frames and rebuilt in the background, the paper's

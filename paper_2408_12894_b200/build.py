@@ -14,7 +14,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libflod.so")
 SOURCES = ["flod_api.cu", "preprocess.cu", "binning.cu", "tile_sort.cu", "blend.cu", "subset.cu"]
-HEADERS = [os.path.join(CSRC, "flod_internal.cuh"), os.path.join(HERE, "..", "include", "flod.h")]
+import glob
+HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h")) +
+                 glob.glob(os.path.join(HERE, "..", "include", "*.h")))
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -25,10 +25,7 @@ constexpr int kDupPer = kGeoBlock / kPreBlock;
 // value-returning global atomic per 2x2 tile group.  Large rects (a coarse level alone: hundreds of tiles per
 // Gaussian on a few hundred counters): those atomics serialise on their addresses (config 3, level 1: 979 us), so
 // k_duplicate_shared counts in shared memory and goes to the global counters once per block and tile.
-#ifndef FLOD_DUP_LARGE_AREA
-#define FLOD_DUP_LARGE_AREA 128
-#endif
-constexpr unsigned int kDupLargeArea = FLOD_DUP_LARGE_AREA;
+constexpr unsigned int kDupLargeArea = 128;
 __device__ __forceinline__ bool dup_large_rects(const WorkspaceDev &ws)
 {
     return ws.hdr->n_pairs > (unsigned long long)kDupLargeArea * ws.hdr->n_vis32;

@@ -21,19 +21,10 @@
 namespace flod {
 
 constexpr int kBlendThreads = 128;
-#ifndef FLOD_BLEND_BATCH
-#define FLOD_BLEND_BATCH 128
-#endif
-constexpr int kBatch = FLOD_BLEND_BATCH;             // Gaussians staged per step (a multiple of kBlendThreads)
+constexpr int kBatch = 128;             // Gaussians staged per step (a multiple of kBlendThreads)
 constexpr int kBlendWarps = kBlendThreads / 32;
-#ifndef FLOD_BLEND_WARPBUF
-#define FLOD_BLEND_WARPBUF 32
-#endif
-#ifndef FLOD_BLEND_FLUSH
-#define FLOD_BLEND_FLUSH (FLOD_BLEND_WARPBUF - 32)
-#endif
-constexpr int kFlush = FLOD_BLEND_FLUSH;             // evaluate when more than this many survivors wait (<= kWarpBuf - 32)
-constexpr int kWarpBuf = FLOD_BLEND_WARPBUF;                        // survivors a warp collects before it evaluates them
+constexpr int kWarpBuf = 32;                         // survivors a warp collects before it evaluates them
+constexpr int kFlush = kWarpBuf - 32;                // evaluate when more than this many survivors wait (<= kWarpBuf - 32)
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
 {
@@ -66,15 +57,10 @@ __device__ __forceinline__ float ex2(float x)
     return y;
 }
 
-#ifndef FLOD_BLEND_UNROLL
-#define FLOD_BLEND_UNROLL 4
-#endif
-constexpr int kBlendUnroll = FLOD_BLEND_UNROLL;     // `#pragma unroll` takes a constant expression, not a macro
-#ifndef FLOD_BLEND_MINBLOCKS
-#define FLOD_BLEND_MINBLOCKS 8
-#endif
+constexpr int kBlendUnroll = 4;
+constexpr int kBlendMinBlocks = 8;                   // 64 registers per thread
 template <bool COUNT>
-__global__ void __launch_bounds__(kBlendThreads, FLOD_BLEND_MINBLOCKS)
+__global__ void __launch_bounds__(kBlendThreads, kBlendMinBlocks)
 k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, int n_tiles,
         float bg0, float bg1, float bg2)
 {

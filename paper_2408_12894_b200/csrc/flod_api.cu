@@ -32,6 +32,13 @@ int fail(const flod_ctx *c, int code, const std::string &msg)
 
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
+// FrameHeader.overflow: bit 0 = the frame needs more pairs than max_pairs, bit 1 = one tile's list exceeds 2^24 entries
+const char *overflow_text(unsigned int bits)
+{
+    if (bits & 1u) return "frame needed more pairs than max_pairs (image undefined); grow the workspace to the reported n_pairs and re-render";
+    return "one tile's list holds more than 2^24 entries (image undefined); a larger workspace does not help: render fewer levels or a larger image";
+}
+
 int sh_stride_for(int deg) { int k = (deg + 1) * (deg + 1); return (3 * k + 3) / 4 * 4; }
 
 constexpr int kScenePlanes = 3 + 6 + 4;   // mean xyz, cov x6, opacity, kappa, log2 o, rho2
@@ -121,6 +128,8 @@ WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_p
     L.ws.pairs = (unsigned long long *)take((size_t)max_pairs * 8);
     L.ws.pairs_tmp = (unsigned long long *)take((size_t)max_pairs * 8);
     L.ws.vals = (uint32_t *)take((size_t)max_pairs * 4);
+    L.ws.ovf_slots = (unsigned int *)take(4 * sizeof(unsigned int));
+    L.ws.ovf_out = L.ws.ovf_slots + 2;
     L.ws.image[0] = (float *)take((size_t)3 * w * h * sizeof(float));
     L.ws.image[1] = (float *)take((size_t)3 * w * h * sizeof(float));
     L.bytes = off;
@@ -144,20 +153,25 @@ int flod_create(flod_ctx **out, int device)
     if (e != cudaSuccess || device < 0 || device >= count) return FLOD_E_CUDA;
     flod_ctx *c = new flod_ctx();
     c->device = device;
+    // the shared-memory opt-ins are per-device function attributes: set them for THIS device, every time
     if (cudaSetDevice(device) != cudaSuccess ||
         cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
-        init_duplicate() != 0) {
+        init_duplicate() != 0 || init_tile_sort() != 0) {
         delete c;
         return FLOD_E_CUDA;
     }
-    for (auto &ev : c->ev) cudaEventCreate(&ev);
-    cudaEventCreateWithFlags(&c->ev_sub_built, cudaEventDisableTiming);
-    for (auto &ev : c->ev_sub_read) cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
-    if (cudaHostAlloc((void **)&c->sub_n_host, 64, cudaHostAllocDefault) != cudaSuccess) { delete c; return FLOD_E_CUDA; }
+    bool ok = true;
+    for (auto &ev : c->ev) ok &= cudaEventCreate(&ev) == cudaSuccess;
+    ok &= cudaEventCreateWithFlags(&c->ev_sub_built, cudaEventDisableTiming) == cudaSuccess;
+    for (auto &ev : c->ev_sub_read) ok &= cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) == cudaSuccess;
     for (int i = 0; i < 2; ++i) {
-        cudaEventCreateWithFlags(&c->ev_rendered[i], cudaEventDisableTiming);
-        cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming);
+        ok &= cudaEventCreateWithFlags(&c->ev_rendered[i], cudaEventDisableTiming) == cudaSuccess;
+        ok &= cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming) == cudaSuccess;
     }
+    // pinned words the device reports into: [0] N_sel of a rebuild, [1], [2] overflow flag of the frame in image[0], image[1]
+    ok &= cudaHostAlloc((void **)&c->sub_n_host, 64, cudaHostAllocDefault) == cudaSuccess;
+    if (!ok) { flod_destroy(c); return FLOD_E_CUDA; }      // releases whatever was created
+    memset(c->sub_n_host, 0, 64);
     *out = c;
     return FLOD_OK;
 }
@@ -349,6 +363,15 @@ int check_frame_args(flod_ctx *ctx, const flod_camera *cam, const float *out_rgb
     if (cam->width > ctx->ws_w || cam->height > ctx->ws_h)
         return fail(ctx, FLOD_E_INVALID_ARG, "render: camera larger than the workspace was sized for");
     for (int i = 0; i < 9; ++i) if (!isfinite(cam->R[i])) return fail(ctx, FLOD_E_INVALID_ARG, "render: non-finite R");
+    // R must be a rotation: k_geometry's covariance-free off-screen bound |row of J R|^2 <= pre_c1 / z^2 and the
+    // meaning of depth both rest on it
+    for (int i = 0; i < 3; ++i)
+        for (int j = i; j < 3; ++j) {
+            double d = 0.0;
+            for (int k = 0; k < 3; ++k) d += (double)cam->R[3 * i + k] * (double)cam->R[3 * j + k];
+            if (fabs(d - (i == j ? 1.0 : 0.0)) > 1e-4)
+                return fail(ctx, FLOD_E_INVALID_ARG, "render: R is not orthonormal (max |R R^T - I| > 1e-4)");
+        }
     for (int i = 0; i < 3; ++i) if (!isfinite(cam->t[i]) || !isfinite(cam->bg[i])) return fail(ctx, FLOD_E_INVALID_ARG, "render: non-finite t / bg");
     if (!isfinite(cam->cx) || !isfinite(cam->cy)) return fail(ctx, FLOD_E_INVALID_ARG, "render: non-finite principal point");
     return FLOD_OK;
@@ -442,6 +465,29 @@ int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, flo
     return enqueue_frame(ctx, ctx->scene, p, out_rgb_dev, (cudaStream_t)stream);
 }
 
+}  // extern "C"
+
+namespace {
+
+// after a frame rendered into ws.image[i] on `s`: copy the image and the frame's overflow word out on `cs`
+int enqueue_copy_out(flod_ctx *ctx, int i, const flod_camera *cam, float *out_rgb_host, cudaStream_t s, cudaStream_t cs)
+{
+    CUDA_TRY(ctx, cudaEventRecord(ctx->ev_rendered[i], s));
+    CUDA_TRY(ctx, cudaStreamWaitEvent(cs, ctx->ev_rendered[i], 0));
+    CUDA_TRY(ctx, cudaMemcpyAsync(out_rgb_host, ctx->ws.image[i], (size_t)3 * cam->width * cam->height * sizeof(float),
+                                  cudaMemcpyDeviceToHost, cs));
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->sub_n_host + 1 + i, ctx->ws.ovf_slots + i, sizeof(unsigned int), cudaMemcpyDeviceToHost, cs));
+    CUDA_TRY(ctx, cudaEventRecord(ctx->ev_copied[i], cs));
+    ctx->copy_pending[i] = true;
+    ctx->last_copy_stream = cs;
+    ctx->img_turn = i ^ 1;
+    return FLOD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
 int flod_render_to_host_async(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, float *out_rgb_host,
                               void *stream, void *copy_stream)
 {
@@ -452,25 +498,26 @@ int flod_render_to_host_async(flod_ctx *ctx, const flod_camera *cam, flod_level_
     const int i = ctx->img_turn;
     // image[i] may still be on its way out (frame k - 2): the kernels of this frame wait for that copy only
     if (ctx->copy_pending[i]) CUDA_TRY(ctx, cudaStreamWaitEvent(s, ctx->ev_copied[i], 0));
-    int rc = flod_render(ctx, cam, mode, gamma, ctx->ws.image[i], stream);
+    ctx->ws.ovf_out = ctx->ws.ovf_slots + i;               // the tile scan reports this frame's overflow word here
+    const int rc = flod_render(ctx, cam, mode, gamma, ctx->ws.image[i], stream);
+    ctx->ws.ovf_out = ctx->ws.ovf_slots + 2;
     if (rc != FLOD_OK) return rc;
-    CUDA_TRY(ctx, cudaEventRecord(ctx->ev_rendered[i], s));
-    CUDA_TRY(ctx, cudaStreamWaitEvent(cs, ctx->ev_rendered[i], 0));
-    CUDA_TRY(ctx, cudaMemcpyAsync(out_rgb_host, ctx->ws.image[i], (size_t)3 * cam->width * cam->height * sizeof(float),
-                                  cudaMemcpyDeviceToHost, cs));
-    CUDA_TRY(ctx, cudaEventRecord(ctx->ev_copied[i], cs));
-    ctx->copy_pending[i] = true;
-    ctx->last_copy_stream = cs;
-    ctx->img_turn = i ^ 1;
-    return FLOD_OK;
+    return enqueue_copy_out(ctx, i, cam, out_rgb_host, s, cs);
 }
 
 int flod_wait_host(flod_ctx *ctx)
 {
     if (!ctx) return FLOD_E_INVALID_ARG;
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    unsigned int ovf = 0;
     for (int i = 0; i < 2; ++i)
-        if (ctx->copy_pending[i]) { CUDA_TRY(ctx, cudaEventSynchronize(ctx->ev_copied[i])); ctx->copy_pending[i] = false; }
+        if (ctx->copy_pending[i]) {
+            CUDA_TRY(ctx, cudaEventSynchronize(ctx->ev_copied[i]));
+            ctx->copy_pending[i] = false;
+            ovf |= ctx->sub_n_host[1 + i];
+            ctx->sub_n_host[1 + i] = 0;
+        }
+    if (ovf) return fail(ctx, FLOD_E_CAPACITY, overflow_text(ovf));
     return FLOD_OK;
 }
 
@@ -641,7 +688,7 @@ int flod_get_stats(flod_ctx *ctx, flod_stats *out)
         for (int i = 0; i < FLOD_N_STAGES; ++i) cudaEventElapsedTime(&out->ms_stage[i], ctx->ev[i], ctx->ev[i + 1]);
         cudaEventElapsedTime(&out->ms_total, ctx->ev[0], ctx->ev[FLOD_N_STAGES]);
     }
-    if (h.overflow) return fail(ctx, FLOD_E_CAPACITY, "frame needed more pairs than max_pairs; grow the workspace and re-render");
+    if (h.overflow) return fail(ctx, FLOD_E_CAPACITY, overflow_text(h.overflow));
     return FLOD_OK;
 }
 

@@ -13,18 +13,12 @@ namespace flod {
 
 constexpr int kTile = FLOD_TILE;
 constexpr int kPreBlock = 256;            // duplication: visible Gaussians per block step
-#ifndef FLOD_GEO_THREADS
-#define FLOD_GEO_THREADS 128
-#endif
-constexpr int kGeoThreads = FLOD_GEO_THREADS;   // geometry: threads per block, kGeoPer consecutive Gaussians per thread
+constexpr int kGeoThreads = 128;   // geometry: threads per block, kGeoPer consecutive Gaussians per thread
 constexpr int kGeoPer = 1024 / kGeoThreads;     // a block scans 1024 Gaussians = one segment
 static_assert(kGeoPer % 4 == 0 && kGeoPer * kGeoThreads == 1024, "whole quads per thread, 1024 per block");
 constexpr int kGeoBlock = kGeoThreads * kGeoPer;
 constexpr int kSortCap = 4096;            // per-tile sort: lists up to this many keys are scattered into shared memory
-#ifndef FLOD_CTR_STRIDE
-#define FLOD_CTR_STRIDE 64
-#endif
-constexpr int kCtrStride = FLOD_CTR_STRIDE;            // ints between two per-tile atomic counters: one counter per 256 B, so that the
+constexpr int kCtrStride = 64;            // ints between two per-tile atomic counters: one counter per 256 B, so that the
                                           // L2 slices share the atomic traffic (a dense 16 KB grid sits on a few slices)
 
 // Scene planes in the caller's arena (SoA, one plane per attribute, gid order = levels concatenated).
@@ -92,6 +86,8 @@ struct WorkspaceDev {
     unsigned long long *pairs;            // [max_pairs] (depth bits << 32) | position, grouped by tile, unsorted
     unsigned long long *pairs_tmp;        // [max_pairs] scatter target of the per-tile sort for lists longer than kSortCap
     uint32_t *vals;                       // [max_pairs] positions, grouped by tile, sorted by (depth, gid)
+    unsigned int *ovf_slots;              // [3] overflow word of the frame rendered into image[0], image[1], and of any other frame
+    unsigned int *ovf_out;                // where THIS frame's tile scan reports (set on the host before the launches)
     float *image[2];                      // 2 x [3][H][W] for flod_render_to_host(_async): double-buffered so that the copy
                                           // of frame k overlaps the kernels of frame k + 1
 };
@@ -171,6 +167,7 @@ int launch_subset_build(const Context &c, const SnapshotDev &dst, const SubsetPa
 int launch_colour(const Context &c, const FrameParams &p, cudaStream_t s);      // a4, and a5 + a8 (tile scan) in block 0
 int launch_duplicate(const Context &c, const FrameParams &p, cudaStream_t s);   // a6
 int init_duplicate();                                                            // once per device: shared-memory opt-in
+int init_tile_sort();                                                            // once per device: shared-memory opt-in
 int launch_tile_sort(const Context &c, const FrameParams &p, cudaStream_t s);   // a7
 int launch_blend(const Context &c, const FrameParams &p, float *out_rgb, cudaStream_t s);   // a9
 

@@ -1,7 +1,7 @@
 // Steps a1-a4 of the hot path:
 //   k_geometry  a1 level selection (Eq. 6-7), a2 cull + view transform, a3 EWA projection, conic,
-//               tile rect.  Phase 1: a thread owns four consecutive Gaussians (16-byte loads from the mean
-//               planes), selects, transforms, culls and applies a conservative off-screen test; the block lists the
+//               tile rect.  Phase 1: a thread owns eight consecutive Gaussians (two 16-byte loads per mean
+//               plane), selects, transforms, culls and applies a conservative off-screen test; the block lists the
 //               survivors.  Phase 2: one survivor per thread, all lanes busy, runs the projection; a visible Gaussian
 //               writes its records at the front of the block's segment of the per-frame arrays, in gid order (no
 //               inter-block scan: see WorkspaceDev), and adds its rect to a 2-D difference grid of the tile counts
@@ -73,11 +73,8 @@ struct GeoSmem {
     unsigned long long pairs;
 };
 
-#ifndef FLOD_GEO_MINBLOCKS
-#define FLOD_GEO_MINBLOCKS 1
-#endif
 template <bool DEBUG>
-__global__ void __launch_bounds__(kGeoThreads, FLOD_GEO_MINBLOCKS)
+__global__ void __launch_bounds__(kGeoThreads)
 k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ FrameParams p)
 {
     __shared__ GeoSmem S;
@@ -89,7 +86,7 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
     const long long g_end = p.first_gid + p.n_scan;
     const float *R = p.R;
 
-    // ================= phase 1: a thread owns four consecutive Gaussians (16-byte loads from the mean and rho2 planes)
+    // ================= phase 1: a thread owns kGeoPer = 8 consecutive Gaussians (two 16-byte loads per mean / rho2 plane)
     // a1 level selection, a2 view transform and z cull (canonical fp32), then a conservative off-screen test that
     // needs no covariance.  What survives is a CANDIDATE; the candidates of the block are listed in gid order.
     unsigned int m_sel = 0, m_front = 0, m_cand = 0;
@@ -280,13 +277,11 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
                 ws.dbg[c] = d;
             }
             // a5, first half: +1 over the rect in the 2-D difference grid of the per-tile pair counts
-#ifndef FLOD_X_NO_GEO_ATOMICS
             const int gw = p.TX + 1;
             atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx0) * kCtrStride, 1);
             atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx1) * kCtrStride, -1);
             atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx0) * kCtrStride, -1);
             atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx1) * kCtrStride, 1);
-#endif
         }
     }
     // ---- block totals
@@ -304,9 +299,6 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
     }
 }
 
-#ifndef FLOD_COLOUR_UNROLL
-#define FLOD_COLOUR_UNROLL 2
-#endif
 // ---- a4: colour of every visible Gaussian.  rgb = max(0, 0.5 + sum_k Y_k(dir) sh_k)  (R16)
 // LANES threads share one Gaussian.  LANES = 4 needs the degree-3 row layout written by the upload: the row is 12
 // float4; float4 number (4 i + j), i = 0..2, holds floats [4 i, 4 i + 4) of the 12 floats (k, channel) of the
@@ -323,7 +315,7 @@ k_colour(const SceneDev sc, const WorkspaceDev ws, int TX, int TY, unsigned int 
     const unsigned int n_here = ws.seg_count[seg];
     // U Gaussians per lane group and step: the U direction records are loaded first, then the U SH rows, then the
     // arithmetic -- two dependent round trips to memory per step instead of per Gaussian
-    constexpr int U = FLOD_COLOUR_UNROLL;
+    constexpr int U = 2;
     for (unsigned int j0 = 0; j0 < n_here; j0 += U * per_block) {
         bool ok[U];
         unsigned int ci[U];

@@ -87,7 +87,9 @@ __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, 
     too_long = __syncthreads_or((int)too_long);
     if (tid == 0) {
         ws.hdr->n_pairs_clamped = (unsigned int)min(total, (unsigned long long)max_pairs);
-        ws.hdr->overflow = (total > max_pairs || too_long) ? 1u : 0u;
+        const unsigned int ovf = (total > max_pairs ? 1u : 0u) | (too_long ? 2u : 0u);
+        ws.hdr->overflow = ovf;
+        *ws.ovf_out = ovf;                                     // read back with the image by flod_render_to_host*
     }
 }
 

@@ -19,12 +19,8 @@ constexpr int kSortThreads = 256;
 constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kSortBinsLog = 11;
 constexpr int kSortBins = 1 << kSortBinsLog;
-#ifndef FLOD_SORT_KEYS_PER_BIN_LOG
-#define FLOD_SORT_KEYS_PER_BIN_LOG 1
-#endif
-#ifndef FLOD_SORT_SLICE_LOG
-#define FLOD_SORT_SLICE_LOG 10
-#endif
+constexpr int kSortKeysPerBinLog = 1;                     // about two keys per bin
+constexpr int kSortSliceLog = 10;                         // depth slices of long lists: 512-1024 keys
 constexpr int kCoarseBinsLog = 8;
 constexpr int kCoarseBins = 1 << kCoarseBinsLog;
 constexpr unsigned int kRankMax = 64;                     // bins up to this size are finished by per-key rank counting
@@ -57,10 +53,7 @@ __device__ __forceinline__ unsigned int block_min_u32(SortSmem &S, unsigned int 
     return v;
 }
 
-#ifndef FLOD_SORT_UNROLL
-#define FLOD_SORT_UNROLL 6
-#endif
-constexpr int kSortU = FLOD_SORT_UNROLL;                  // keys a thread holds in registers / loads in flight per step
+constexpr int kSortU = 6;                  // keys a thread holds in registers / loads in flight per step
 
 // f(key) for src[from .. n) strided over the block, kSortU independent loads in flight per thread and step.
 template <class F>
@@ -78,7 +71,7 @@ __device__ __forceinline__ void for_keys(const u64 *src, unsigned int from, unsi
 // Distributes src[0, n) into dst[0, n) by bin (src and dst must not overlap).  On return ends[b] is the exclusive end
 // of bin b in dst (its start is ends[b-1], 0 for b = 0), and all writes are visible to the block.
 __device__ BinMap bin_pass(const u64 *src, u64 *dst, unsigned int n, unsigned int *ends, SortSmem &S, int tid,
-                           int per_bin_log = FLOD_SORT_KEYS_PER_BIN_LOG, int min_bins_log = 6, int max_bins_log = kSortBinsLog)
+                           int per_bin_log = kSortKeysPerBinLog, int min_bins_log = 6, int max_bins_log = kSortBinsLog)
 {
     const int lane = tid & 31, warp = tid >> 5;
     // the first kSortU * kSortThreads keys (the whole list of an average tile) stay in registers over the three passes
@@ -233,7 +226,7 @@ k_tile_sort(const WorkspaceDev ws, int n_tiles)
     // per key, the slices cost one more scatter.  A slice that is still longer than kSortCap (a cluster of nearly
     // equal depths) goes through global memory.
     u64 *tmp = ws.pairs_tmp + rg.x;
-    const BinMap mc = bin_pass(pairs, tmp, L, S.cends, S, tid, FLOD_SORT_SLICE_LOG, 1, kCoarseBinsLog);
+    const BinMap mc = bin_pass(pairs, tmp, L, S.cends, S, tid, kSortSliceLog, 1, kCoarseBinsLog);
     for (unsigned int b = 0; b < mc.nb; ++b) {
         const unsigned int lo = b ? S.cends[b - 1] : 0u, n2 = S.cends[b] - lo;
         if (n2 == 0) continue;
@@ -250,14 +243,16 @@ k_tile_sort(const WorkspaceDev ws, int n_tiles)
     }
 }
 
+// Once per device (flod_create, after cudaSetDevice): SortSmem exceeds the 48 KB default of dynamic shared memory, and
+// the opt-in is a per-device attribute of the function.
+int init_tile_sort()
+{
+    return cudaFuncSetAttribute(k_tile_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)) == cudaSuccess ? 0 : -1;
+}
+
 int launch_tile_sort(const Context &c, const FrameParams &p, cudaStream_t s)
 {
     if (p.n_pre_blocks <= 0) return 0;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(k_tile_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
-        attr_set = true;
-    }
     k_tile_sort<<<p.n_tiles, kSortThreads, sizeof(SortSmem), s>>>(c.ws, p.n_tiles);
     return 1;
 }

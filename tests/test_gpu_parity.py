@@ -35,15 +35,16 @@ def make_renderer(pkg, levels, sh_degree, width, height, max_pairs=1 << 20, flag
     return r
 
 
-def check_image(gpu, fr, tol=1e-3):
-    """north_star tolerance with the envelope rule; returns (max abs diff, number of marginal pixels)."""
-    ref = fr.composite()
+def check_image(gpu, fr, tol=1e-3, brute=False):
+    """north_star tolerance with the envelope rule; returns (max abs diff, number of marginal pixels).
+    brute=True compares with per-pixel compositing over ALL depth-sorted Gaussians (no tiles, no rects)."""
+    ref = fr.composite(brute=brute)
     d = np.abs(gpu.astype(np.float64) - ref)
     bad = d > tol
     n_marginal = 0
     if bad.any():
-        lo = fr.composite(skip_thr=SKIP_THR * (1 - DELTA))
-        hi = fr.composite(skip_thr=SKIP_THR * (1 + DELTA))
+        lo = fr.composite(skip_thr=SKIP_THR * (1 - DELTA), brute=brute)
+        hi = fr.composite(skip_thr=SKIP_THR * (1 + DELTA), brute=brute)
         mn = np.minimum(np.minimum(ref, lo), hi) - tol
         mx = np.maximum(np.maximum(ref, lo), hi) + tol
         marginal = (np.abs(lo - ref) > 1e-5) | (np.abs(hi - ref) > 1e-5)
@@ -139,11 +140,9 @@ def test_determinism(config0):
 def test_brute_force_parity_on_tiny_input(config0):
     """north_star: GPU image against per-pixel compositing over ALL depth-sorted Gaussians (no tiles)."""
     sc, cam, osc, r = config0
-    img = r.render(cam, 1, 2, 1.0).cpu().numpy()
-    fr = osc.frame(cam, 1, 2, 1.0)
-    brute = fr.composite(brute=True)
-    d = np.abs(img - brute)
-    assert np.quantile(d, 0.999) <= 1e-3 and d.max() <= 5e-3
+    for (ls, le) in ((1, 2), (2, 2)):
+        img = r.render(cam, ls, le, 1.0).cpu().numpy()
+        check_image(img, osc.frame(cam, ls, le, 1.0), brute=True)
 
 
 # ------------------------------------------------------------------------- edge cases, small scenes
@@ -258,6 +257,56 @@ def test_needle_gaussians_stay_within_tolerance(pkg):
     r.close()
 
 
+def test_anisotropic_camera_off_centre_principal_point(pkg):
+    """R4 and every fy / cy / lim_y term (O2-O4, Eq. 7): fx != fy, cx != W/2, cy != H/2.  With fx == fy and a centred
+    principal point a swap of the two would go unnoticed on both sides."""
+    rng = np.random.default_rng(61)
+    lv = _rand_levels(rng, (1500, 3000, 6000), (0.08, 0.02, 0.0), extent=2.5, sh_degree=2)
+    osc = OracleScene(lv, 2)
+    r = make_renderer(pkg, lv, 2, 208, 136, max_pairs=1 << 22)
+    for (fx, fy, cx, cy) in ((190.0, 127.0, 81.25, 90.5), (95.0, 240.0, 150.0, 20.0)):
+        cam = camera(width=208, height=136, f=fx, fy=fy, cx=cx, cy=cy, bg=(0.2, 0.1, 0.3))
+        check_frame(r, osc, cam, 3, 3, 1.0)
+        _, _, fr = check_frame(r, osc, cam, 1, 3, 1.5)
+        per_level = [int(fr.mask[a:b].sum()) for a, b in ((0, 1500), (1500, 4500), (4500, 10500))]
+        assert all(n > 0 for n in per_level)
+        check_frame(r, osc, cam, 2, 3, 0.7, ref_pos=[0.4, -0.3, 0.2])
+    r.close()
+
+
+def test_non_orthonormal_camera_rotation_is_rejected(pkg):
+    """R is a rotation.  The covariance-free off-screen bound of k_geometry assumes it; a scaled or sheared R
+    is an argument error, not a silently different image."""
+    lv = level(1, 0.0, [[0, 0, 1.0]], 0.1)
+    r = make_renderer(pkg, [lv], 0, 64, 64)
+    for R in (np.eye(3) * 1.01, np.array([[1, 0.01, 0], [0, 1, 0], [0, 0, 1.0]])):
+        with pytest.raises(pkg.FlodError) as e:
+            r.render(camera(width=64, height=64, R=R), 1, 1, 1.0)
+        assert e.value.code == -1
+    r.render(camera(width=64, height=64), 1, 1, 1.0)
+    r.close()
+
+
+def test_two_contexts_in_one_process_are_independent(pkg):
+    """include/flod.h: "contexts are independent".  Two contexts with different scenes and workspaces, frames
+    interleaved; the per-device kernel attributes (shared-memory opt-ins) are set by every flod_create."""
+    rng = np.random.default_rng(5)
+    lva = _rand_levels(rng, (2000, 5000), (0.05, 0.0))
+    lvb = _rand_levels(rng, (700,), (0.0,), sh_degree=1)
+    cam = camera(width=96, height=80, f=90.0)
+    ra = make_renderer(pkg, lva, 0, 96, 80)
+    rb = make_renderer(pkg, lvb, 1, 96, 80)
+    osa, osb = OracleScene(lva, 0), OracleScene(lvb, 1)
+    a0 = ra.render(cam, 1, 2, 1.0).cpu().numpy()
+    b0 = rb.render(cam, 1, 1, 1.0).cpu().numpy()
+    for _ in range(2):
+        check_frame(ra, osa, cam, 1, 2, 1.0)
+        check_frame(rb, osb, cam, 1, 1, 1.0)
+    assert np.array_equal(a0, ra.render(cam, 1, 2, 1.0).cpu().numpy())
+    assert np.array_equal(b0, rb.render(cam, 1, 1, 1.0).cpu().numpy())
+    ra.close(); rb.close()
+
+
 def test_paper_rho4_ladder(pkg):
     """R7: the paper's tau = 0.2, rho = 4 ladder through Eq. 7, selective {1..5}."""
     rng = np.random.default_rng(40)
@@ -297,9 +346,22 @@ def test_errors_and_capacity(pkg):
     st = r.get_stats(raise_on_overflow=False)
     need = OracleScene(lv, 0).frame(cam, 2, 2, 1.0).counts["n_pairs"]
     assert st["overflow"] == 1 and st["n_pairs"] == need > 256
+    # the host-buffer calls block on the frame anyway, so they report the overflow themselves
+    with pytest.raises(pkg.FlodError) as e:
+        r.render_to_host(cam, 2, 2, 1.0)
+    assert e.value.code == -5
+    import torch
+    side = torch.cuda.Stream(device=r.device)
+    buf = torch.zeros((3, 64, 64), dtype=torch.float32).pin_memory()
+    r.render_to_host_async(cam, 2, 2, 1.0, buf, side)
+    with pytest.raises(pkg.FlodError) as e:
+        r.wait_host()
+    assert e.value.code == -5
+    r.wait_host()                            # the flag was consumed: nothing pending any more
     r.set_workspace(64, 64, need)            # grow to exactly what was reported and re-render
     r.set_options(pkg.FLOD_OPT_DEBUG)
     check_frame(r, OracleScene(lv, 0), cam, 2, 2, 1.0)
+    assert np.array_equal(r.render_to_host(cam, 2, 2, 1.0).numpy(), r.render(cam, 2, 2, 1.0).cpu().numpy())
     r.close()
 
 
