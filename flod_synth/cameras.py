@@ -85,3 +85,14 @@ def make_poses(config: int, width: int | None = None, height: int | None = None,
             cams.append(pinhole(R, t, W, H, eye=eye))
         return cams
     raise ValueError(f"no pose recipe for config {config}")
+
+
+def poses_checksum(cams) -> str:
+    """sha256 over the fp32 fields of a pose list (R, t, fx, fy, cx, cy, width, height, z_near)."""
+    import hashlib
+    h = hashlib.sha256()
+    for c in cams:
+        h.update(np.ascontiguousarray(c.R, dtype=np.float32).tobytes()); h.update(np.ascontiguousarray(c.t, dtype=np.float32).tobytes())
+        h.update(np.array([c.fx, c.fy, c.cx, c.cy, c.z_near], dtype=np.float32).tobytes())
+        h.update(np.array([c.width, c.height], dtype=np.int32).tobytes())
+    return h.hexdigest()

@@ -187,3 +187,16 @@ def make_random_scene(seed: int, n_per_level=(200, 300), s_min=(0.05, 0.0), sh_d
             opacity_logit=rng.normal(0.0, 1.5, n).astype(np.float32),
             sh=np.ascontiguousarray(sh, dtype=np.float32)))
     return scene
+
+
+def scene_checksum(scene: Scene) -> str:
+    """sha256 over every level's id, s_min and arrays (bytes, in field order): names the exact inputs a seed produced,
+    so that a numpy / platform change that alters a "seeded" scene is noticed (tests/golden/scene_checksums.json)."""
+    import hashlib
+    h = hashlib.sha256()
+    h.update(np.int32(scene.sh_degree).tobytes())
+    for lv in scene.levels:
+        h.update(np.int32(lv.level).tobytes()); h.update(np.float32(lv.s_min).tobytes())
+        for a in (lv.mean, lv.log_scale, lv.quat, lv.opacity_logit, lv.sh):
+            h.update(np.ascontiguousarray(a, dtype=np.float32).tobytes())
+    return h.hexdigest()

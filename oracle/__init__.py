@@ -53,6 +53,8 @@ def lib():
             f.argtypes = [C.c_void_p]
         L.orc_frame_create.restype = C.c_void_p
         L.orc_frame_create.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_float, C.c_void_p]
+        L.orc_frame_create_ex.restype = C.c_void_p
+        L.orc_frame_create_ex.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_float, C.c_void_p, C.c_int]
         L.orc_frame_destroy.argtypes = [C.c_void_p]
         for name in ("mask", "state", "mu2d", "depth", "cov2d", "conic", "rect", "n_tiles", "rgb",
                      "tile_start", "centre"):
@@ -189,21 +191,24 @@ class OracleScene:
     def dead(self):
         return _view(lib().orc_scene_dead(self._h), (self.n_total,), np.uint8)
 
-    def frame(self, cam, l_start, l_end, gamma, ref_pos=None):
-        return OracleFrame(self, cam, l_start, l_end, gamma, ref_pos)
+    def frame(self, cam, l_start, l_end, gamma, ref_pos=None, geometry_only=False, fp64=False):
+        return OracleFrame(self, cam, l_start, l_end, gamma, ref_pos, geometry_only, fp64)
 
 
 class OracleFrame:
     """Steps O1-O6 for one camera and level mode; `composite` is O7.  Levels are level ids."""
 
-    def __init__(self, scene, cam, l_start, l_end, gamma, ref_pos=None):
+    def __init__(self, scene, cam, l_start, l_end, gamma, ref_pos=None, geometry_only=False, fp64=False):
+        """geometry_only: steps O1-O4 and the per-tile counts of O6 only (no colours, no stored lists, no image).
+        fp64: variant O64 -- every step in fp64 with no intermediate rounding (a report, never a parity target)."""
         self.scene = scene
         self.W, self.H = cam.width, cam.height
         cs = _camera_struct(cam)
         ref = None if ref_pos is None else _f32(ref_pos)
         base = scene.level_ids[0] - 1
-        self._h = lib().orc_frame_create(scene._h, C.addressof(cs), l_start - base, l_end - base,
-                                         float(np.float32(gamma)), None if ref is None else ref.ctypes.data)
+        self._h = lib().orc_frame_create_ex(scene._h, C.addressof(cs), l_start - base, l_end - base,
+                                            float(np.float32(gamma)), None if ref is None else ref.ctypes.data,
+                                            (0 if geometry_only else 3) | (4 if fp64 else 0))
         if not self._h:
             raise ValueError("orc_frame_create failed (bad level range or gamma)")
         self.TX, self.TY = lib().orc_frame_tx(self._h), lib().orc_frame_ty(self._h)

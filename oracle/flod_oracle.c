@@ -64,6 +64,7 @@ typedef struct {
     float *kappa;     /* [n] 2 ln(255 o) */
     uint8_t *dead;    /* [n] o < 1/255 */
     float *sh;        /* [n][K][3] */
+    float *raw_ls, *raw_q, *raw_logit;   /* [n][3], [n][4], [n]: the uploaded attributes (O64 activates from them) */
 } orc_scene;
 
 /* ---------------------------------------------------------------- small pins: Eq. 3, 4, 7 --- */
@@ -127,10 +128,16 @@ orc_scene *orc_scene_create(int n_levels, const orc_level_desc *lv, int sh_degre
     sc->kappa = (float *)malloc(sizeof(float) * na);
     sc->dead = (uint8_t *)malloc(na);
     sc->sh = (float *)malloc(sizeof(float) * 3 * sc->K * na);
+    sc->raw_ls = (float *)malloc(sizeof(float) * 3 * na);
+    sc->raw_q = (float *)malloc(sizeof(float) * 4 * na);
+    sc->raw_logit = (float *)malloc(sizeof(float) * na);
     for (int l = 0; l < n_levels; ++l) {
         int64_t base = sc->offset[l];
         memcpy(sc->mean + 3 * base, lv[l].mean, sizeof(float) * 3 * lv[l].n);
         memcpy(sc->sh + 3 * sc->K * base, lv[l].sh, sizeof(float) * 3 * sc->K * lv[l].n);
+        memcpy(sc->raw_ls + 3 * base, lv[l].log_scale, sizeof(float) * 3 * lv[l].n);
+        memcpy(sc->raw_q + 4 * base, lv[l].quat, sizeof(float) * 4 * lv[l].n);
+        memcpy(sc->raw_logit + base, lv[l].opacity_logit, sizeof(float) * lv[l].n);
 #pragma omp parallel for schedule(static)
         for (int64_t i = 0; i < lv[l].n; ++i)
             orc_activate_one(lv[l].log_scale + 3 * i, lv[l].quat + 4 * i, lv[l].opacity_logit[i],
@@ -144,6 +151,7 @@ void orc_scene_destroy(orc_scene *sc)
 {
     if (!sc) return;
     free(sc->mean); free(sc->cov); free(sc->opacity); free(sc->kappa); free(sc->dead); free(sc->sh);
+    free(sc->raw_ls); free(sc->raw_q); free(sc->raw_logit);
     free(sc);
 }
 
@@ -228,7 +236,12 @@ typedef struct {
     uint32_t *tile_start;        /* [T_n + 1] */
     uint32_t *bf_list;           /* [n_bf] all gaussians with state >= ST_EMPTY_RECT, (depth,gid) order */
     int bf_sorted;               /* bf_list is ordered on first brute-force use */
+    int what;                    /* ORC_WITH_* : which of the optional products were built */
+    /* variant O64 (ORC_FP64): the same steps with every operation in fp64 and nothing rounded to fp32 on the way */
+    double *mu2d64, *depth64, *conic64, *opacity64;
 } orc_frame;
+
+enum { ORC_WITH_COLOUR = 1, ORC_WITH_PAIRS = 2, ORC_FP64 = 4 };
 
 /* Eq. 7 with the two boundary overrides, squared and rounded once to fp32.
  * Bands are half-open [d_proj^(l), d_proj^(l-1)) (DESIGN R1).  f = fx (DESIGN R4). */
@@ -313,6 +326,84 @@ static int project_one(const orc_frame *fr, int64_t g)
     return nt ? ST_VISIBLE : ST_EMPTY_RECT;
 }
 
+/* ---- variant O64 (SURVEY 8(c) "Oracle variants"): steps O0-O4 with every operation in fp64 on the fp32 inputs and
+ * no intermediate rounding -- the mathematical result the canonical-fp32 sequence approximates.  NOT a parity target:
+ * it exists to report how many masks / rects differ between the two and how far the images are apart.  The fp32
+ * copies it leaves in mu2d / depth / conic / rect are for reporting; compositing reads the fp64 arrays. */
+static int project_one_f64(const orc_frame *fr, int64_t g, const double centre[3], double limx, double limy)
+{
+    const orc_scene *sc = fr->sc;
+    const orc_camera *cm = &fr->cam;
+    const float *R = cm->R, *t = cm->t;
+    const float *m = sc->mean + 3 * g;
+    /* O0 in fp64 (Eq. 1), unrounded */
+    const float *ls = sc->raw_ls + 3 * g, *q = sc->raw_q + 4 * g;
+    double s0 = exp((double)ls[0]), s1 = exp((double)ls[1]), s2 = exp((double)ls[2]);
+    double w = q[0], x = q[1], y = q[2], z = q[3];
+    double nrm = sqrt(((w * w + x * x) + y * y) + z * z);
+    w /= nrm; x /= nrm; y /= nrm; z /= nrm;
+    double Rg[3][3] = {
+        { 1.0 - 2.0 * (y * y + z * z), 2.0 * (x * y - w * z), 2.0 * (x * z + w * y) },
+        { 2.0 * (x * y + w * z), 1.0 - 2.0 * (x * x + z * z), 2.0 * (y * z - w * x) },
+        { 2.0 * (x * z - w * y), 2.0 * (y * z + w * x), 1.0 - 2.0 * (x * x + y * y) } };
+    double v[3] = { s0 * s0, s1 * s1, s2 * s2 }, S[3][3];
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j)
+            S[i][j] = (Rg[i][0] * v[0] * Rg[j][0] + Rg[i][1] * v[1] * Rg[j][1]) + Rg[i][2] * v[2] * Rg[j][2];
+    double o = 1.0 / (1.0 + exp(-(double)sc->raw_logit[g]));
+    /* O2 */
+    double px = ((double)R[0] * m[0] + (double)R[1] * m[1] + (double)R[2] * m[2]) + t[0];
+    double py = ((double)R[3] * m[0] + (double)R[4] * m[1] + (double)R[5] * m[2]) + t[1];
+    double pz = ((double)R[6] * m[0] + (double)R[7] * m[1] + (double)R[8] * m[2]) + t[2];
+    if (pz <= (double)cm->z_near) return ST_CULL_NEAR;
+    if (o < 1.0 / 255.0) return ST_CULL_DEAD;
+    double ix = px / pz, iy = py / pz;
+    double mx = (double)cm->fx * ix + cm->cx, my = (double)cm->fy * iy + cm->cy;
+    /* O3 */
+    double u = fmin(fmax(ix, -limx), limx), vv = fmin(fmax(iy, -limy), limy);
+    double J[2][3] = { { cm->fx / pz, 0.0, -((double)cm->fx * u) / pz }, { 0.0, cm->fy / pz, -((double)cm->fy * vv) / pz } };
+    double M[2][3];
+    for (int i = 0; i < 2; ++i)
+        for (int k = 0; k < 3; ++k) M[i][k] = J[i][0] * R[k] + J[i][1] * R[3 + k] + J[i][2] * R[6 + k];
+    double c2[2][2];
+    for (int i = 0; i < 2; ++i)
+        for (int j = 0; j < 2; ++j) {
+            double acc = 0.0;
+            for (int k = 0; k < 3; ++k)
+                for (int l = 0; l < 3; ++l) acc += M[i][k] * S[k][l] * M[j][l];
+            c2[i][j] = acc;
+        }
+    double a = c2[0][0] + 0.3, b = c2[0][1], c = c2[1][1] + 0.3;
+    double det = a * c - b * b;
+    fr->mu2d64[2 * g] = mx; fr->mu2d64[2 * g + 1] = my; fr->depth64[g] = pz; fr->opacity64[g] = o;
+    fr->mu2d[2 * g] = (float)mx; fr->mu2d[2 * g + 1] = (float)my; fr->depth[g] = (float)pz;
+    fr->cov2d[3 * g] = (float)a; fr->cov2d[3 * g + 1] = (float)b; fr->cov2d[3 * g + 2] = (float)c;
+    if (!(det > 0.0)) return ST_CULL_DET;
+    fr->conic64[3 * g] = c / det; fr->conic64[3 * g + 1] = -(b / det); fr->conic64[3 * g + 2] = a / det;
+    for (int k = 0; k < 3; ++k) fr->conic[3 * g + k] = (float)fr->conic64[3 * g + k];
+    /* O4: the exact box of the alpha = 1/255 contour (no pad: the pad of the fp32 sequence covers ITS rounding) */
+    double kap = 2.0 * log(255.0 * o);
+    double hx = sqrt(kap * a), hy = sqrt(kap * c);
+    double TXd = fr->TX, TYd = fr->TY;
+    int32_t tx0 = (int32_t)fmin(fmax(floor((mx - hx) / 16.0), 0.0), TXd), tx1 = (int32_t)fmin(fmax(floor((mx + hx) / 16.0) + 1.0, 0.0), TXd);
+    int32_t ty0 = (int32_t)fmin(fmax(floor((my - hy) / 16.0), 0.0), TYd), ty1 = (int32_t)fmin(fmax(floor((my + hy) / 16.0) + 1.0, 0.0), TYd);
+    fr->rect[4 * g] = tx0; fr->rect[4 * g + 1] = ty0; fr->rect[4 * g + 2] = tx1; fr->rect[4 * g + 3] = ty1;
+    uint32_t nt = (uint32_t)((tx1 - tx0) * (ty1 - ty0));
+    fr->n_tiles[g] = nt;
+    return nt ? ST_VISIBLE : ST_EMPTY_RECT;
+}
+
+static const orc_frame *g_sort_frame;   /* qsort has no context argument; frames are built serially */
+static int cmp_pair64(const void *pa, const void *pb)
+{
+    const orc_pair *a = (const orc_pair *)pa, *b = (const orc_pair *)pb;
+    if (a->tile != b->tile) return a->tile < b->tile ? -1 : 1;
+    double da = g_sort_frame->depth64[a->gid], db = g_sort_frame->depth64[b->gid];
+    if (da != db) return da < db ? -1 : 1;
+    if (a->gid != b->gid) return a->gid < b->gid ? -1 : 1;
+    return 0;
+}
+
 static int cmp_pair(const void *pa, const void *pb)
 {
     const orc_pair *a = (const orc_pair *)pa, *b = (const orc_pair *)pb;
@@ -322,10 +413,14 @@ static int cmp_pair(const void *pa, const void *pb)
     return 0;
 }
 
-static const orc_frame *g_sort_frame;   /* qsort has no context argument; frames are built serially */
 static int cmp_bf(const void *pa, const void *pb)
 {
     uint32_t a = *(const uint32_t *)pa, b = *(const uint32_t *)pb;
+    if (g_sort_frame->what & ORC_FP64) {
+        double da = g_sort_frame->depth64[a], db = g_sort_frame->depth64[b];
+        if (da != db) return da < db ? -1 : 1;
+        return a < b ? -1 : (a > b ? 1 : 0);
+    }
     float da = g_sort_frame->depth[a], db = g_sort_frame->depth[b];
     if (da != db) return da < db ? -1 : 1;
     return a < b ? -1 : (a > b ? 1 : 0);
@@ -336,16 +431,19 @@ void orc_frame_destroy(orc_frame *fr)
     if (!fr) return;
     free(fr->mask); free(fr->state); free(fr->mu2d); free(fr->depth); free(fr->cov2d); free(fr->conic);
     free(fr->rect); free(fr->n_tiles); free(fr->rgb); free(fr->pairs); free(fr->tile_start); free(fr->bf_list);
+    free(fr->mu2d64); free(fr->depth64); free(fr->conic64); free(fr->opacity64);
     free(fr);
 }
 
-/* Steps O1-O6 for one camera and mode.  ref_pos NULL = camera centre (DESIGN R2). */
-orc_frame *orc_frame_create(const orc_scene *sc, const orc_camera *cam, int l_start, int l_end,
-                            float gamma, const float *ref_pos)
+/* Steps O1-O6 for one camera and mode.  ref_pos NULL = camera centre (DESIGN R2).  `what` (ORC_WITH_*) only leaves
+ * products out: without ORC_WITH_COLOUR step O5 is skipped, without ORC_WITH_PAIRS the lists of O6 are counted
+ * (tile_start is complete) but not stored -- masks, states, geometry and per-tile counts never depend on it. */
+orc_frame *orc_frame_create_ex(const orc_scene *sc, const orc_camera *cam, int l_start, int l_end,
+                               float gamma, const float *ref_pos, int what)
 {
     if (!sc || !cam || l_start < 1 || l_end > sc->L || l_start > l_end || !(gamma > 0.0f)) return NULL;
     orc_frame *fr = (orc_frame *)calloc(1, sizeof(orc_frame));
-    fr->sc = sc; fr->cam = *cam; fr->l_start = l_start; fr->l_end = l_end; fr->gamma = gamma;
+    fr->sc = sc; fr->cam = *cam; fr->l_start = l_start; fr->l_end = l_end; fr->gamma = gamma; fr->what = what;
     fr->TX = (cam->width + ORC_TILE - 1) / ORC_TILE;
     fr->TY = (cam->height + ORC_TILE - 1) / ORC_TILE;
     const float *R = cam->R, *t = cam->t;
@@ -368,6 +466,16 @@ orc_frame *orc_frame_create(const orc_scene *sc, const orc_camera *cam, int l_st
     fr->rect = (int32_t *)calloc(4 * na, sizeof(int32_t));
     fr->n_tiles = (uint32_t *)calloc(na, sizeof(uint32_t));
     fr->rgb = (double *)calloc(3 * na, sizeof(double));
+    const int f64 = (what & ORC_FP64) != 0;
+    double centre64[3], limx64 = 1.3 * (double)cam->width / (2.0 * (double)cam->fx), limy64 = 1.3 * (double)cam->height / (2.0 * (double)cam->fy);
+    for (int i = 0; i < 3; ++i)
+        centre64[i] = -(((double)R[i] * (double)t[0] + (double)R[3 + i] * (double)t[1]) + (double)R[6 + i] * (double)t[2]);
+    if (f64) {
+        fr->mu2d64 = (double *)calloc(2 * na, sizeof(double));
+        fr->depth64 = (double *)calloc(na, sizeof(double));
+        fr->conic64 = (double *)calloc(3 * na, sizeof(double));
+        fr->opacity64 = (double *)calloc(na, sizeof(double));
+    }
 
     int64_t n_sel = 0, n_front = 0, n_vis = 0, n_pairs = 0, n_bf = 0;
     for (int l = l_start; l <= l_end; ++l) {
@@ -376,14 +484,23 @@ orc_frame *orc_frame_create(const orc_scene *sc, const orc_camera *cam, int l_st
         fr->n_scan += e - b;
 #pragma omp parallel for schedule(static) reduction(+ : n_sel, n_front, n_vis, n_pairs, n_bf)
         for (int64_t g = b; g < e; ++g) {
-            if (!select_one(sc->mean + 3 * g, fr->ref, lo2, hi2)) continue;
+            if (f64) {      /* O1 in fp64: unrounded thresholds d_proj^2, unrounded camera centre (or the given reference) */
+                double dl = (l == l_end) ? 0.0 : (double)sc->s_min[l - 1] * (double)cam->fx / (double)gamma;
+                double dh = (l == l_start) ? INFINITY : (double)sc->s_min[l - 2] * (double)cam->fx / (double)gamma;
+                double d2 = 0.0;
+                for (int i = 0; i < 3; ++i) {
+                    double d = (double)sc->mean[3 * g + i] - (ref_pos ? (double)ref_pos[i] : centre64[i]);
+                    d2 += d * d;
+                }
+                if (!(d2 >= dl * dl && d2 < dh * dh)) continue;
+            } else if (!select_one(sc->mean + 3 * g, fr->ref, lo2, hi2)) continue;
             fr->mask[g] = 1; n_sel++;
-            int st = project_one(fr, g);
+            int st = f64 ? project_one_f64(fr, g, centre64, limx64, limy64) : project_one(fr, g);
             fr->state[g] = (uint8_t)st;
             if (st != ST_CULL_NEAR) n_front++;
             if (st >= ST_EMPTY_RECT) {
                 n_bf++;
-                orc_sh_color(sc->sh_degree, sc->mean + 3 * g, fr->centre,
+                if (what & ORC_WITH_COLOUR) orc_sh_color(sc->sh_degree, sc->mean + 3 * g, fr->centre,
                              sc->sh + 3 * (int64_t)sc->K * g, fr->rgb + 3 * g);
             }
             if (st == ST_VISIBLE) { n_vis++; n_pairs += fr->n_tiles[g]; }
@@ -408,6 +525,7 @@ orc_frame *orc_frame_create(const orc_scene *sc, const orc_camera *cam, int l_st
             for (int tx = r[0]; tx < r[2]; ++tx) fr->tile_start[ty * fr->TX + tx + 1]++;
     }
     for (int tI = 0; tI < T_n; ++tI) fr->tile_start[tI + 1] += fr->tile_start[tI];
+    if (!(what & ORC_WITH_PAIRS)) return fr;
     uint32_t *fill = (uint32_t *)malloc(sizeof(uint32_t) * (size_t)(T_n > 0 ? T_n : 1));
     memcpy(fill, fr->tile_start, sizeof(uint32_t) * (size_t)T_n);
     for (int64_t g = 0; g < n; ++g) {
@@ -421,10 +539,18 @@ orc_frame *orc_frame_create(const orc_scene *sc, const orc_camera *cam, int l_st
             }
     }
     free(fill);
+    g_sort_frame = fr;
 #pragma omp parallel for schedule(dynamic, 8)
     for (int tI = 0; tI < T_n; ++tI)
-        qsort(fr->pairs + fr->tile_start[tI], (size_t)(fr->tile_start[tI + 1] - fr->tile_start[tI]), sizeof(orc_pair), cmp_pair);
+        qsort(fr->pairs + fr->tile_start[tI], (size_t)(fr->tile_start[tI + 1] - fr->tile_start[tI]), sizeof(orc_pair),
+              f64 ? cmp_pair64 : cmp_pair);
     return fr;
+}
+
+orc_frame *orc_frame_create(const orc_scene *sc, const orc_camera *cam, int l_start, int l_end,
+                            float gamma, const float *ref_pos)
+{
+    return orc_frame_create_ex(sc, cam, l_start, l_end, gamma, ref_pos, ORC_WITH_COLOUR | ORC_WITH_PAIRS);
 }
 
 /* accessors */
@@ -462,11 +588,17 @@ typedef struct { double T, C[3]; uint32_t E, B; int stopped; } pix_state;
 static inline int blend_one(const orc_frame *fr, uint32_t g, double pxc, double pyc,
                             double skip_thr, double stop_thr, pix_state *ps)
 {
-    double dx = (double)fr->mu2d[2 * g] - pxc, dy = (double)fr->mu2d[2 * g + 1] - pyc;
-    double A = fr->conic[3 * g], B = fr->conic[3 * g + 1], C = fr->conic[3 * g + 2];
+    double dx, dy, A, B, C, o;
+    if (fr->what & ORC_FP64) {
+        dx = fr->mu2d64[2 * g] - pxc; dy = fr->mu2d64[2 * g + 1] - pyc;
+        A = fr->conic64[3 * g]; B = fr->conic64[3 * g + 1]; C = fr->conic64[3 * g + 2]; o = fr->opacity64[g];
+    } else {
+        dx = (double)fr->mu2d[2 * g] - pxc; dy = (double)fr->mu2d[2 * g + 1] - pyc;
+        A = fr->conic[3 * g]; B = fr->conic[3 * g + 1]; C = fr->conic[3 * g + 2]; o = (double)fr->sc->opacity[g];
+    }
     double q = 0.5 * (A * dx * dx + C * dy * dy) + B * dx * dy;
     if (q < 0.0) q = 0.0;
-    double alpha = (double)fr->sc->opacity[g] * exp(-q);
+    double alpha = o * exp(-q);
     if (alpha > 0.99) alpha = 0.99;
     ps->E++;
     if (alpha < skip_thr) return 0;
@@ -491,6 +623,10 @@ void orc_frame_composite(const orc_frame *fr, double skip_thr, double stop_thr, 
 {
     int W = fr->cam.width, H = fr->cam.height;
     int T_n = fr->TX * fr->TY;
+    if ((fr->what & (ORC_WITH_COLOUR | ORC_WITH_PAIRS)) != (ORC_WITH_COLOUR | ORC_WITH_PAIRS)) {
+        for (int64_t i = 0; i < (int64_t)3 * W * H; ++i) out_rgb[i] = NAN;     /* a geometry-only frame has no image */
+        return;
+    }
     if (brute && !fr->bf_sorted) {            /* global (depth, gid) order, built on first use */
         orc_frame *mf = (orc_frame *)fr;
         g_sort_frame = fr;

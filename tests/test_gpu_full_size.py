@@ -20,6 +20,8 @@ def full(request):
     build.build()
     import paper_2408_12894_b200 as pkg
     scene = fs.make_scene(1)
+    from test_gpu_config34 import _report_checksum
+    _report_checksum(1, scene)
     cams = fs.make_poses(1)
     osc = OracleScene(scene.levels, scene.sh_degree)
     r = pkg.Renderer(0)
@@ -30,10 +32,11 @@ def full(request):
     r.close()
 
 
-def _geometry_exact(r, osc, cam, ls, le, gamma):
-    img = r.render(cam, ls, le, gamma).cpu().numpy()
+def _geometry_exact(r, osc, cam, ls, le, gamma, geometry_only=False):
+    img = r.render(cam, ls, le, gamma)
+    img = None if geometry_only else img.cpu().numpy()
     st = r.get_stats()
-    fr = osc.frame(cam, ls, le, gamma)
+    fr = osc.frame(cam, ls, le, gamma, geometry_only=geometry_only)
     c = fr.counts
     assert (st["n_scan"], st["n_sel"], st["n_front"], st["n_vis"], st["n_pairs"]) == (
         c["n_scan"], c["n_sel"], c["n_front"], c["n_vis"], c["n_pairs"])
@@ -81,15 +84,29 @@ def test_config1_max_level_other_poses(full, pose):
 def test_config2_selective_masks_and_counts_exact(full, gamma):
     """BASELINE.json config 2: selective {3,4,5}, gamma in {1,2,4}: masks and per-tile pair counts exactly."""
     scene, cams, osc, r = full
-    # FLOD_FULL_SWEEP=1: all 200 poses (SURVEY 8(d) config 2; ~3 minutes per gamma, so not the default)
-    poses = range(len(cams)) if os.environ.get("FLOD_FULL_SWEEP") else (0, 50, 150)
-    for pose in poses:
+    for pose in (0, 50, 150):
         img, fr, st = _geometry_exact(r, osc, cams[pose], 3, 5, gamma)
         if pose == 50:
             check_image(img, fr)
     off = scene.offsets
     per_level = [int(fr.mask[off[l]:off[l + 1]].sum()) for l in range(5)]
     assert per_level[0] == per_level[1] == 0 and sum(per_level[2:]) == st["n_sel"]
+
+
+@pytest.mark.parametrize("gamma", [1.0, 2.0, 4.0])
+def test_config2_sweep_all_poses_masks_and_counts_exact(full, gamma):
+    """BASELINE.json configs[2]'s contract: "the level-selection masks and per-tile pair counts are checked against the
+    oracle exactly" on the 200 poses x gamma in {1,2,4}.  Geometry only on both sides (no image download, no stored
+    lists in the oracle): masks, the five frame counters and the per-tile pair counts of every pose.
+    FLOD_SWEEP_STRIDE=k checks every k-th pose only."""
+    scene, cams, osc, r = full
+    stride = int(os.environ.get("FLOD_SWEEP_STRIDE", "1"))
+    n_sel = n_pairs = 0
+    for pose in range(0, len(cams), stride):
+        _, fr, st = _geometry_exact(r, osc, cams[pose], 3, 5, gamma, geometry_only=True)
+        n_sel += st["n_sel"]; n_pairs += st["n_pairs"]
+    n = len(range(0, len(cams), stride))
+    print(f"config2 gamma {gamma}: {n} poses, 0 mismatches; mean N_sel {n_sel / n:.0f}, mean P {n_pairs / n:.0f}")
 
 
 def test_single_levels_sweep(full):

@@ -706,3 +706,26 @@ def test_sh_basis_equals_library_spherical_harmonics():
                 y = complex(sph_harm_y(l, abs(m), theta, phi))
                 want.append(math.sqrt(2) * y.imag if m < 0 else (y.real if m == 0 else math.sqrt(2) * y.real))
         np.testing.assert_allclose(oracle.sh_basis(3, d), want, atol=1e-12)
+
+
+# ------------------------------------------------------------------------ variant O64
+
+def test_fp32_pipeline_sits_on_the_fp64_result():
+    """O32 (canonical fp32 geometry, the parity target) against O64 (every step in fp64, nothing rounded on the way) on
+    config 0: same masks and cull states, O64's exact rect never sticks out of O32's padded one (the pad covers the fp32
+    rounding: R13's conservativeness does not rest on fp32 luck), images within 1e-5 -- two orders below north_star's
+    1e-3, so the tolerance is spent on the kernel's fp32 compositing, not on the geometry's precision."""
+    import flod_synth as fs
+    sc = fs.make_scene(0)
+    cam = fs.make_poses(0)[0]
+    osc = OracleScene(sc.levels, sc.sh_degree)
+    for (ls, le) in ((2, 2), (1, 2)):
+        a, b = osc.frame(cam, ls, le, 1.0), osc.frame(cam, ls, le, 1.0, fp64=True)
+        assert np.array_equal(a.mask, b.mask) and np.array_equal(a.state, b.state)
+        vis = a.state == oracle.ST_VISIBLE
+        ra, rb = a.rect[vis], b.rect[vis]
+        assert (rb[:, :2] >= ra[:, :2]).all() and (rb[:, 2:] <= ra[:, 2:]).all()
+        assert (ra != rb).any(axis=1).mean() < 0.02            # the pad costs under 2 % of the rects one more tile row/column
+        np.testing.assert_allclose(a.mu2d[vis], b.mu2d[vis], rtol=1e-5, atol=1e-4)
+        np.testing.assert_allclose(a.conic[vis], b.conic[vis], rtol=2e-4, atol=1e-7)
+        assert np.abs(a.composite() - b.composite()).max() < 1e-5
