@@ -191,16 +191,21 @@ class OracleScene:
     def dead(self):
         return _view(lib().orc_scene_dead(self._h), (self.n_total,), np.uint8)
 
-    def frame(self, cam, l_start, l_end, gamma, ref_pos=None, geometry_only=False, fp64=False):
-        return OracleFrame(self, cam, l_start, l_end, gamma, ref_pos, geometry_only, fp64)
+    def frame(self, cam, l_start, l_end, gamma, ref_pos=None, geometry_only=False, fp64=False, pair_rule=1):
+        return OracleFrame(self, cam, l_start, l_end, gamma, ref_pos, geometry_only, fp64, pair_rule)
 
 
 class OracleFrame:
     """Steps O1-O6 for one camera and level mode; `composite` is O7.  Levels are level ids."""
 
-    def __init__(self, scene, cam, l_start, l_end, gamma, ref_pos=None, geometry_only=False, fp64=False):
+    def __init__(self, scene, cam, l_start, l_end, gamma, ref_pos=None, geometry_only=False, fp64=False, pair_rule=1):
         """geometry_only: steps O1-O4 and the per-tile counts of O6 only (no colours, no stored lists, no image).
-        fp64: variant O64 -- every step in fp64 with no intermediate rounding (a report, never a parity target)."""
+        fp64: variant O64 -- every step in fp64 with no intermediate rounding (a report, never a parity target).
+        pair_rule: which tiles a visible Gaussian is listed in (DESIGN R13 / R26): 1 = every tile of its rect,
+        2 = the tiles of its rect that hold a pixel centre of the padded alpha = 1/255 ellipse."""
+        if pair_rule not in (1, 2) or (fp64 and pair_rule != 1):
+            raise ValueError("pair_rule is 1 (box) or 2 (ellipse); O64 uses rule 1")
+        self.pair_rule = pair_rule
         self.scene = scene
         self.W, self.H = cam.width, cam.height
         cs = _camera_struct(cam)
@@ -208,7 +213,7 @@ class OracleFrame:
         base = scene.level_ids[0] - 1
         self._h = lib().orc_frame_create_ex(scene._h, C.addressof(cs), l_start - base, l_end - base,
                                             float(np.float32(gamma)), None if ref is None else ref.ctypes.data,
-                                            (0 if geometry_only else 3) | (4 if fp64 else 0))
+                                            (0 if geometry_only else 3) | (4 if fp64 else 0) | (8 if pair_rule == 2 else 0))
         if not self._h:
             raise ValueError("orc_frame_create failed (bad level range or gamma)")
         self.TX, self.TY = lib().orc_frame_tx(self._h), lib().orc_frame_ty(self._h)

@@ -241,7 +241,7 @@ typedef struct {
     double *mu2d64, *depth64, *conic64, *opacity64;
 } orc_frame;
 
-enum { ORC_WITH_COLOUR = 1, ORC_WITH_PAIRS = 2, ORC_FP64 = 4 };
+enum { ORC_WITH_COLOUR = 1, ORC_WITH_PAIRS = 2, ORC_FP64 = 4, ORC_RULE_ELLIPSE = 8 };
 
 /* Eq. 7 with the two boundary overrides, squared and rounded once to fp32.
  * Bands are half-open [d_proj^(l), d_proj^(l-1)) (DESIGN R1).  f = fx (DESIGN R4). */
@@ -404,6 +404,56 @@ static int cmp_pair64(const void *pa, const void *pb)
     return 0;
 }
 
+/* ---- O6, pair rule 2 "ellipse" (DESIGN R26).  Pair rule 1 "box" lists a visible Gaussian in EVERY tile of
+ * its rect (O4).  Rule 2 lists it, inside that rect, only in the tiles that hold a pixel centre of the (padded) contour
+ * alpha = 1/255 of Eq. 2, i.e. of the ellipse  A dx^2 + 2 B dx dy + C dy^2 <= K  around mu', with (A, B, C)
+ * the ROUNDED fp32 conic that O7 evaluates and K = kappa (1 + 2^-9).  The pixel centres of tile row ty are the band
+ * y in [16 ty + .5, 16 ty + 15.5]; the ellipse cut by a band is convex, so the tiles of that row are one span
+ * [ta, tb]: for a fixed dy the ellipse is dx in [sl dy - w(dy), sl dy + w(dy)], sl = -B/A,
+ * w(dy) = sqrt(K/A - (D/A) dy^2), D = C - B^2/A; its right end is concave in dy with its maximum at the ellipse's
+ * rightmost point dy = dyt, so over the band it is largest at clamp(dyt, band) (likewise the left end at
+ * clamp(-dyt, band)).  A tile column holds pixel centres x in [16 tx + .5, 16 tx + 15.5].
+ * Arithmetic: canonical fp64 -- every operation below is one IEEE binary64 operation in the written order (the
+ * difference C - B^2/A cancels badly in fp32 for needle-shaped footprints), inputs are the fp32 values of O2-O4.
+ * Pads: 2^-9 on K and 2^-6 px on the ends, far above the rounding of this sequence and of O7's exponent.
+ * Returns the number of tiles of row ty (0: none) and the span in *ta, *tb (inclusive). */
+static int ellipse_row_span(float mx, float my, float cA, float cB, float cC, float kappa,
+                            int tx0, int tx1, int ty, int *ta_out, int *tb_out)
+{
+    const double dA = (double)cA, dB = (double)cB, dC = (double)cC;
+    const double K = (double)kappa * 1.001953125;
+    const double rA = 1.0 / dA;
+    const double sl = -(dB * rA);
+    const double D = dC - (dB * dB) * rA;
+    const double Dp = dA - (dB * dB) / dC;
+    *ta_out = tx0; *tb_out = tx1 - 1;
+    if (!(dA > 0.0) || !(dC > 0.0) || !(D > 0.0) || !(Dp > 0.0)) return tx1 - tx0;   /* not an ellipse after rounding: the box rule */
+    const double KA = K * rA, DA = D * rA;
+    const double dxm = sqrt(K / Dp);
+    const double dyt = -((dB / dC) * dxm);
+    const double y0 = ((double)(16 * ty) + 0.5) - (double)my, y1 = y0 + 15.0;
+    const double dn = fmin(fmax(0.0, y0), y1);
+    if (DA * (dn * dn) > KA) return 0;                       /* the band misses the ellipse */
+    const double dh = fmin(fmax(dyt, y0), y1), dl = fmin(fmax(-dyt, y0), y1);
+    const double wh = sqrt(fmax(0.0, KA - DA * (dh * dh))), wl = sqrt(fmax(0.0, KA - DA * (dl * dl)));
+    const double xh = ((double)mx + (sl * dh + wh)) + 0.015625;
+    const double xl = ((double)mx + (sl * dl - wl)) - 0.015625;
+    const double ta = fmax(ceil((xl - 15.5) * 0.0625), (double)tx0);
+    const double tb = fmin(floor((xh - 0.5) * 0.0625), (double)(tx1 - 1));
+    if (!(tb >= ta)) return 0;
+    *ta_out = (int)ta; *tb_out = (int)tb;
+    return (int)tb - (int)ta + 1;
+}
+
+/* the tiles of row ty of Gaussian g's rect under the frame's pair rule */
+static inline int row_span(const orc_frame *fr, int64_t g, int ty, int *ta, int *tb)
+{
+    const int32_t *r = fr->rect + 4 * g;
+    if (!(fr->what & ORC_RULE_ELLIPSE)) { *ta = r[0]; *tb = r[2] - 1; return r[2] - r[0]; }
+    return ellipse_row_span(fr->mu2d[2 * g], fr->mu2d[2 * g + 1], fr->conic[3 * g], fr->conic[3 * g + 1], fr->conic[3 * g + 2],
+                            fr->sc->kappa[g], r[0], r[2], ty, ta, tb);
+}
+
 static int cmp_pair(const void *pa, const void *pb)
 {
     const orc_pair *a = (const orc_pair *)pa, *b = (const orc_pair *)pb;
@@ -521,22 +571,31 @@ orc_frame *orc_frame_create_ex(const orc_scene *sc, const orc_camera *cam, int l
         if (fr->state[g] >= ST_EMPTY_RECT) fr->bf_list[q++] = (uint32_t)g;
         if (fr->state[g] != ST_VISIBLE) continue;
         const int32_t *r = fr->rect + 4 * g;
-        for (int ty = r[1]; ty < r[3]; ++ty)
-            for (int tx = r[0]; tx < r[2]; ++tx) fr->tile_start[ty * fr->TX + tx + 1]++;
+        uint32_t np = 0;
+        for (int ty = r[1]; ty < r[3]; ++ty) {
+            int ta, tb;
+            if (!row_span(fr, g, ty, &ta, &tb)) continue;
+            for (int tx = ta; tx <= tb; ++tx) { fr->tile_start[ty * fr->TX + tx + 1]++; ++np; }
+        }
+        fr->n_tiles[g] = np;                /* pairs of g (= its rect's area under pair rule 1) */
     }
     for (int tI = 0; tI < T_n; ++tI) fr->tile_start[tI + 1] += fr->tile_start[tI];
+    fr->n_pairs = n_pairs = fr->tile_start[T_n];
     if (!(what & ORC_WITH_PAIRS)) return fr;
     uint32_t *fill = (uint32_t *)malloc(sizeof(uint32_t) * (size_t)(T_n > 0 ? T_n : 1));
     memcpy(fill, fr->tile_start, sizeof(uint32_t) * (size_t)T_n);
     for (int64_t g = 0; g < n; ++g) {
         if (fr->state[g] != ST_VISIBLE) continue;
         const int32_t *r = fr->rect + 4 * g;
-        for (int ty = r[1]; ty < r[3]; ++ty)
-            for (int tx = r[0]; tx < r[2]; ++tx) {
+        for (int ty = r[1]; ty < r[3]; ++ty) {
+            int ta, tb;
+            if (!row_span(fr, g, ty, &ta, &tb)) continue;
+            for (int tx = ta; tx <= tb; ++tx) {
                 uint32_t tile = (uint32_t)(ty * fr->TX + tx);
                 orc_pair *pp = fr->pairs + fill[tile]++;
                 pp->tile = tile; pp->depth = fr->depth[g]; pp->gid = (uint32_t)g;
             }
+        }
     }
     free(fill);
     g_sort_frame = fr;

@@ -509,6 +509,106 @@ def test_tiled_equals_brute_force_bit_exactly():
         assert (tE <= bE).all()
 
 
+# ------------------------------------------------------------------------ pair rule 2 "ellipse" (R26)
+
+def _needle_and_blob_scene(rng, n):
+    """Footprints of every shape: blobs, large discs, needles at the dilation floor in every orientation, high and
+    barely-alive opacities (kappa from 0.05 to 11)."""
+    pos = np.stack([rng.uniform(-2, 2, n), rng.uniform(-1.5, 1.5, n), rng.uniform(0.4, 7.0, n)], axis=1)
+    scale = np.exp(rng.uniform(-4.5, -0.5, (n, 3)))
+    thin = rng.random(n) < 0.4
+    scale[thin, 1:] = 1e-4
+    scale[thin, 0] = np.exp(rng.uniform(-1.5, 1.0, thin.sum()))
+    logit = np.where(rng.random(n) < 0.2, rng.uniform(-5.5, -5.0, n), rng.normal(0, 2.5, n))
+    return [level(1, 0.0, pos, scale, quat=rng.normal(size=(n, 4)), logit=logit, rgb=rng.uniform(0, 1, (n, 3)))]
+
+
+def test_ellipse_pair_rule_tiled_equals_brute_force_bit_exactly():
+    """R26 keeps what R13 had to deliver (S:171 / S:177): with pair rule 2 the tiled image still equals per-pixel
+    compositing over ALL Gaussians bit for bit -- no pixel with alpha >= 1/255 lies in a tile that was dropped."""
+    rng = np.random.default_rng(2026)
+    for k in range(30):
+        n = int(rng.integers(1, 500))
+        lv = _needle_and_blob_scene(rng, n) if k % 3 else _random_scene(rng, n)
+        cam = camera(width=int(rng.integers(17, 150)), height=int(rng.integers(17, 110)), f=float(rng.uniform(40, 260)),
+                     fy=float(rng.uniform(40, 260)), cx=float(rng.uniform(10, 90)), cy=float(rng.uniform(10, 60)),
+                     bg=tuple(rng.uniform(0, 1, 3)))
+        sc = OracleScene(lv, 0)
+        f1, f2 = sc.frame(cam, 1, 1, 1.0), sc.frame(cam, 1, 1, 1.0, pair_rule=2)
+        t_img, tE, tB, tT = f2.composite(stats=True)
+        b_img, bE, bB, bT = f2.composite(brute=True, stats=True)
+        assert np.array_equal(t_img, b_img) and np.array_equal(tB, bB) and np.array_equal(tT, bT)
+        assert np.array_equal(t_img, f1.composite())
+        # rule 2 only ever drops tiles of rule 1's rect; everything else of the frame is the same
+        assert (f2.tile_counts <= f1.tile_counts).all() and (f2.n_tiles <= f1.n_tiles).all()
+        assert np.array_equal(f1.rect, f2.rect) and np.array_equal(f1.state, f2.state) and f1.counts["n_vis"] == f2.counts["n_vis"]
+        assert (tE <= f1.composite(stats=True)[1]).all()
+
+
+def test_ellipse_pair_rule_lists_exactly_the_tiles_the_contour_reaches():
+    """R26 against the definition, tile by tile (numpy, fp64, from the oracle's mu', conic and opacity): a tile is
+    listed if one of its pixel centres has alpha >= 1/255 (conservative) and only if the contour grown by the pads
+    reaches the box of its pixel centres (tight: the minimum of the quadratic form over that box, found by dense
+    sampling of its border, is within the padded level)."""
+    rng = np.random.default_rng(909)
+    cam = camera(width=208, height=136, f=150.0, fy=210.0, cx=99.0, cy=70.5)
+    lv = _needle_and_blob_scene(rng, 260)
+    sc = OracleScene(lv, 0)
+    fr = sc.frame(cam, 1, 1, 1.0, pair_rule=2)
+    tile, _, gid = fr.sorted_pairs()
+    listed = {}
+    for t, g in zip(tile, gid):
+        listed.setdefault(int(g), set()).add(int(t))
+    jj, ii = np.mgrid[0:fr.TY * 16, 0:fr.TX * 16]
+    n_loose = n_listed = 0
+    for g in np.nonzero(fr.state == oracle.ST_VISIBLE)[0]:
+        A, B, C = fr.conic[g].astype(np.float64)
+        mx, my = fr.mu2d[g].astype(np.float64)
+        o = float(sc.opacity[g])
+        dx, dy = mx - (ii + 0.5), my - (jj + 0.5)
+        q = np.maximum(0.0, 0.5 * (A * dx * dx + C * dy * dy) + B * dx * dy)
+        hit = np.minimum(0.99, o * np.exp(-q)) >= SKIP_THR
+        r = fr.rect[g]
+        must = {int(ty * fr.TX + tx) for ty in range(r[1], r[3]) for tx in range(r[0], r[2])
+                if hit[16 * ty:16 * ty + 16, 16 * tx:16 * tx + 16].any()}
+        got = listed.get(int(g), set())
+        assert must <= got, f"gaussian {g}: tiles {sorted(must - got)} hold a blended pixel but are not listed"
+        assert got <= {int(ty * fr.TX + tx) for ty in range(r[1], r[3]) for tx in range(r[0], r[2])}
+        # tightness: min of the form over the pixel-centre box of every listed tile (dense border + centre clamp)
+        K0 = 2.0 * math.log(o / SKIP_THR)
+        K = K0 * (1 + 2.0 ** -8) + 2.0 * math.sqrt(K0 * (A + C)) * 2.0 ** -5       # the pads: 2^-9 on K, 2^-6 px along x (|grad| <= 2 sqrt(K lambda_max))
+        for t in got:
+            ty, tx = divmod(t, fr.TX)
+            xs = np.linspace(16 * tx + 0.5, 16 * tx + 15.5, 241); ys = np.linspace(16 * ty + 0.5, 16 * ty + 15.5, 241)
+            bx = np.concatenate([xs, xs, np.full(241, xs[0]), np.full(241, xs[-1]), [min(max(mx, xs[0]), xs[-1])]])
+            by = np.concatenate([np.full(241, ys[0]), np.full(241, ys[-1]), ys, ys, [min(max(my, ys[0]), ys[-1])]])
+            qq = A * (mx - bx) ** 2 + C * (my - by) ** 2 + 2 * B * (mx - bx) * (my - by)
+            n_listed += 1
+            n_loose += int(qq.min() > K)
+    assert n_listed > 1500 and n_loose == 0, (n_loose, n_listed)
+
+
+def test_ellipse_pair_rule_closed_form_disc():
+    """One isotropic Gaussian on the optical axis: the contour is the circle r = sigma' sqrt(2 ln(255 o)) around
+    (cx, cy); the listed tiles are exactly those whose pixel-centre box lies within r of the centre (tiles at the
+    corners of the rect are dropped: the count approaches pi/4 of the rect for large discs)."""
+    f, s, d, o = 300.0, 0.25, 2.0, 0.9
+    cam = camera(width=400, height=400, f=f)
+    sc = OracleScene([level(1, 0.0, [[0, 0, d]], s, opacity=o)], 0)
+    f1, f2 = sc.frame(cam, 1, 1, 1.0), sc.frame(cam, 1, 1, 1.0, pair_rule=2)
+    o32 = float(sc.opacity[0])
+    rad = math.sqrt(((f * s / d) ** 2 + 0.3) * 2 * math.log(255 * o32))
+    want = np.zeros(f2.TX * f2.TY, np.uint32)
+    for ty in range(f2.TY):
+        for tx in range(f2.TX):
+            nx = min(max(200.0, 16 * tx + 0.5), 16 * tx + 15.5); ny = min(max(200.0, 16 * ty + 0.5), 16 * ty + 15.5)
+            dist = math.hypot(nx - 200.0, ny - 200.0)
+            assert abs(dist - rad) > 0.05          # no tile sits on the decision edge in this construction
+            want[ty * f2.TX + tx] = dist <= rad
+    assert np.array_equal(f2.tile_counts, want)
+    assert 0.7 < want.sum() / f1.counts["n_pairs"] < 0.86 and f1.counts["n_pairs"] > 250
+
+
 def test_brute_force_in_numpy_on_tiny_input():
     """Independent restatement of P:104-111 in vectorised numpy: every pixel, every Gaussian, global depth order,
     from the oracle's projected (mu', conic) and colours.  Different code, same definition."""
