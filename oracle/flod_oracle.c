@@ -406,40 +406,51 @@ static int cmp_pair64(const void *pa, const void *pb)
 
 /* ---- O6, pair rule 2 "ellipse" (DESIGN R26).  Pair rule 1 "box" lists a visible Gaussian in EVERY tile of
  * its rect (O4).  Rule 2 lists it, inside that rect, only in the tiles that hold a pixel centre of the (padded) contour
- * alpha = 1/255 of Eq. 2, i.e. of the ellipse  A dx^2 + 2 B dx dy + C dy^2 <= K  around mu', with (A, B, C)
- * the ROUNDED fp32 conic that O7 evaluates and K = kappa (1 + 2^-9).  The pixel centres of tile row ty are the band
- * y in [16 ty + .5, 16 ty + 15.5]; the ellipse cut by a band is convex, so the tiles of that row are one span
- * [ta, tb]: for a fixed dy the ellipse is dx in [sl dy - w(dy), sl dy + w(dy)], sl = -B/A,
- * w(dy) = sqrt(K/A - (D/A) dy^2), D = C - B^2/A; its right end is concave in dy with its maximum at the ellipse's
- * rightmost point dy = dyt, so over the band it is largest at clamp(dyt, band) (likewise the left end at
- * clamp(-dyt, band)).  A tile column holds pixel centres x in [16 tx + .5, 16 tx + 15.5].
- * Arithmetic: canonical fp64 -- every operation below is one IEEE binary64 operation in the written order (the
- * difference C - B^2/A cancels badly in fp32 for needle-shaped footprints), inputs are the fp32 values of O2-O4.
- * Pads: 2^-9 on K and 2^-6 px on the ends, far above the rounding of this sequence and of O7's exponent.
+ * alpha = 1/255 of Eq. 2.  With the exponent of Eq. 2 in its factorised form (DESIGN R25),
+ *     log2 alpha = log2 o - a w^2 - d dy^2,   w = dx + k dy,   k = B/A,  a = A log2(e)/2,  d = (C - B^2/A) log2(e)/2,
+ * the contour is  a w^2 + d dy^2 = E = log2 o + log2 255.  The pixel centres of tile row ty are the band
+ * y in [16 ty + .5, 16 ty + 15.5]; the ellipse cut by a band is convex, so the listed tiles of a row are ONE span
+ * [ta, tb].  For a fixed dy = y - mu'y the ellipse is x - mu'x in [sl dy - s(dy), sl dy + s(dy)], sl = -k,
+ * s(dy)^2 = KA - DA dy^2, KA = E/a, DA = d/a; the right end is concave in dy with its maximum at the ellipse's rightmost
+ * point dy = dyt = -k sqrt(KA / (DA (DA + k^2))), so over the band it is largest at clamp(dyt, band) (the left end
+ * smallest at clamp(-dyt, band)).  A tile column holds pixel centres x in [16 tx + .5, 16 tx + 15.5].
+ * Arithmetic: k, a, d are derived from the ROUNDED fp32 conic (A, B, C) that O7 evaluates, in fp64 (C - B^2/A cancels
+ * for thin diagonal footprints), each rounded once to fp32; everything after that is canonical fp32, like O1-O4:
+ * one IEEE binary32 operation per written operation.  In this parametrisation nothing cancels except s^2 near the
+ * ellipse's tips, where an error e in s^2 moves s by up to sqrt(e): the ends are padded by 2^-8 sqrt(KA) + 2^-6 pixels
+ * plus 2^-20 of the magnitudes that were added, E by 2^-9 E + 2^-16.
  * Returns the number of tiles of row ty (0: none) and the span in *ta, *tb (inclusive). */
-static int ellipse_row_span(float mx, float my, float cA, float cB, float cC, float kappa,
+static int ellipse_row_span(float mx, float my, float cA, float cB, float cC, float opacity,
                             int tx0, int tx1, int ty, int *ta_out, int *tb_out)
 {
+    const double LOG2E = 1.4426950408889634;
     const double dA = (double)cA, dB = (double)cB, dC = (double)cC;
-    const double K = (double)kappa * 1.001953125;
     const double rA = 1.0 / dA;
-    const double sl = -(dB * rA);
-    const double D = dC - (dB * dB) * rA;
-    const double Dp = dA - (dB * dB) / dC;
+    const float k = (float)(dB * rA);
+    const float a = -(float)((-0.5 * LOG2E) * dA);
+    const float d = -fminf((float)((-0.5 * LOG2E) * (dC - (dB * dB) * rA)), 0.0f);
+    const float l2o = (float)log2((double)opacity);
     *ta_out = tx0; *tb_out = tx1 - 1;
-    if (!(dA > 0.0) || !(dC > 0.0) || !(D > 0.0) || !(Dp > 0.0)) return tx1 - tx0;   /* not an ellipse after rounding: the box rule */
-    const double KA = K * rA, DA = D * rA;
-    const double dxm = sqrt(K / Dp);
-    const double dyt = -((dB / dC) * dxm);
-    const double y0 = ((double)(16 * ty) + 0.5) - (double)my, y1 = y0 + 15.0;
-    const double dn = fmin(fmax(0.0, y0), y1);
-    if (DA * (dn * dn) > KA) return 0;                       /* the band misses the ellipse */
-    const double dh = fmin(fmax(dyt, y0), y1), dl = fmin(fmax(-dyt, y0), y1);
-    const double wh = sqrt(fmax(0.0, KA - DA * (dh * dh))), wl = sqrt(fmax(0.0, KA - DA * (dl * dl)));
-    const double xh = ((double)mx + (sl * dh + wh)) + 0.015625;
-    const double xl = ((double)mx + (sl * dl - wl)) - 0.015625;
-    const double ta = fmax(ceil((xl - 15.5) * 0.0625), (double)tx0);
-    const double tb = fmin(floor((xh - 0.5) * 0.0625), (double)(tx1 - 1));
+    if (!(a > 0.0f)) return tx1 - tx0;                       /* not an ellipse after rounding: the box rule */
+    const float E = (l2o + 7.994353436858858f) * 1.001953125f + 0.0000152587890625f;
+    const float sl = -k;
+    const float KA = E / a;
+    const float DA = d / a;
+    float dyt;
+    if (DA > 0.0f) dyt = -(k * sqrtf(KA / (DA * (DA + k * k))));
+    else dyt = k < 0.0f ? INFINITY : (k > 0.0f ? -INFINITY : 0.0f);      /* a strip: the ends are linear in dy */
+    const float pad = sqrtf(KA) * 0.00390625f + 0.015625f;
+    const float y0 = ((float)(16 * ty) + 0.5f) - my, y1 = y0 + 15.0f;
+    const float dn = fminf(fmaxf(0.0f, y0), y1);
+    if (DA * (dn * dn) > KA * 1.001953125f) return 0;        /* the band misses the ellipse */
+    const float dh = fminf(fmaxf(dyt, y0), y1), dl = fminf(fmaxf(-dyt, y0), y1);
+    const float sh = sqrtf(fmaxf(0.0f, KA - DA * (dh * dh))), sq = sqrtf(fmaxf(0.0f, KA - DA * (dl * dl)));
+    const float ch = sl * dh, cl = sl * dl;
+    const float padr = pad + ((fabsf(mx) + fabsf(ch)) + fabsf(cl)) * 9.5367431640625e-7f;
+    const float xh = (mx + (ch + sh)) + padr;
+    const float xl = (mx + (cl - sq)) - padr;
+    const float ta = fmaxf(ceilf((xl - 15.5f) * 0.0625f), (float)tx0);
+    const float tb = fminf(floorf((xh - 0.5f) * 0.0625f), (float)(tx1 - 1));
     if (!(tb >= ta)) return 0;
     *ta_out = (int)ta; *tb_out = (int)tb;
     return (int)tb - (int)ta + 1;
@@ -451,7 +462,7 @@ static inline int row_span(const orc_frame *fr, int64_t g, int ty, int *ta, int 
     const int32_t *r = fr->rect + 4 * g;
     if (!(fr->what & ORC_RULE_ELLIPSE)) { *ta = r[0]; *tb = r[2] - 1; return r[2] - r[0]; }
     return ellipse_row_span(fr->mu2d[2 * g], fr->mu2d[2 * g + 1], fr->conic[3 * g], fr->conic[3 * g + 1], fr->conic[3 * g + 2],
-                            fr->sc->kappa[g], r[0], r[2], ty, ta, tb);
+                            fr->sc->opacity[g], r[0], r[2], ty, ta, tb);
 }
 
 static int cmp_pair(const void *pa, const void *pb)

@@ -549,7 +549,7 @@ def test_ellipse_pair_rule_lists_exactly_the_tiles_the_contour_reaches():
     """R26 against the definition, tile by tile (numpy, fp64, from the oracle's mu', conic and opacity): a tile is
     listed if one of its pixel centres has alpha >= 1/255 (conservative) and only if the contour grown by the pads
     reaches the box of its pixel centres (tight: the minimum of the quadratic form over that box, found by dense
-    sampling of its border, is within the padded level)."""
+    sampling of its border, is within the padded level) -- needles included."""
     rng = np.random.default_rng(909)
     cam = camera(width=208, height=136, f=150.0, fy=210.0, cx=99.0, cy=70.5)
     lv = _needle_and_blob_scene(rng, 260)
@@ -574,9 +574,12 @@ def test_ellipse_pair_rule_lists_exactly_the_tiles_the_contour_reaches():
         got = listed.get(int(g), set())
         assert must <= got, f"gaussian {g}: tiles {sorted(must - got)} hold a blended pixel but are not listed"
         assert got <= {int(ty * fr.TX + tx) for ty in range(r[1], r[3]) for tx in range(r[0], r[2])}
-        # tightness: min of the form over the pixel-centre box of every listed tile (dense border + centre clamp)
+        # tightness: min of the form over the pixel-centre box of every listed tile (dense border + centre clamp) is within
+        # the padded level: E (1 + 2^-9) + 2^-16, ends moved by 2^-8 sqrt(K/A) + 2^-6 px + 2^-20 of the summed magnitudes
+        # (|grad Q| <= 2 sqrt(K lambda_max))
         K0 = 2.0 * math.log(o / SKIP_THR)
-        K = K0 * (1 + 2.0 ** -8) + 2.0 * math.sqrt(K0 * (A + C)) * 2.0 ** -5       # the pads: 2^-9 on K, 2^-6 px along x (|grad| <= 2 sqrt(K lambda_max))
+        pad = math.sqrt(K0 / A) / 256 + 2.0 ** -6 + 2.0 ** -19 * (abs(mx) + 2 * abs(B / A) * (abs(my) + 16 * fr.TY))
+        K = K0 * (1 + 2.0 ** -8) + 2.0 ** -14 + 2.0 * math.sqrt(K0 * (A + C)) * 2 * pad + (A + C) * (2 * pad) ** 2
         for t in got:
             ty, tx = divmod(t, fr.TX)
             xs = np.linspace(16 * tx + 0.5, 16 * tx + 15.5, 241); ys = np.linspace(16 * ty + 0.5, 16 * ty + 15.5, 241)
