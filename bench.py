@@ -47,6 +47,9 @@ def parse_args():
     ap.add_argument("--subset-period", type=int, default=0,
                     help="selective modes only: render from a materialised G_sel (flod_render_subset) that is rebuilt "
                          "every N frames on a second stream and swapped in when ready (P:699-711); 0 = Eq. 6 per frame")
+    ap.add_argument("--pair-rule", type=int, default=2, choices=[1, 2],
+                    help="which tiles a Gaussian is listed in: 1 = every tile of its rect (R13), 2 = the tiles the alpha = 1/255 "
+                         "ellipse reaches (R26, the library's default); same image, fewer pairs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--count-scale", type=float, default=1.0, help="shrink the scene (debugging only; reported)")
     return ap.parse_args()
@@ -160,9 +163,9 @@ class ClockSampler:
 
 # ----------------------------------------------------------------------------------------- reference arm
 
-def oracle_frame_seconds(osc, cam, ls, le, gamma):
+def oracle_frame_seconds(osc, cam, ls, le, gamma, pair_rule=2):
     t0 = time.perf_counter()
-    fr = osc.frame(cam, ls, le, gamma)
+    fr = osc.frame(cam, ls, le, gamma, pair_rule=pair_rule)
     img = fr.composite()
     return time.perf_counter() - t0, fr, img
 
@@ -194,7 +197,7 @@ def run_reference(args):
     K = args.steps if args.steps is not None else 5
     W = args.warmup if args.warmup is not None else 1
     osc = oracle.OracleScene(scene.levels, scene.sh_degree)
-    t_full, _, _ = oracle_frame_seconds(osc, cams[0], ls, le, args.gamma)      # un-timed probe of one full frame
+    t_full, _, _ = oracle_frame_seconds(osc, cams[0], ls, le, args.gamma, args.pair_rule)      # un-timed probe of one full frame
     budget = 150.0 / max(K + W, 1)
     frac = 1.0 if t_full <= budget else max(1.0 / 64.0, budget / t_full)
     use = []
@@ -202,11 +205,11 @@ def run_reference(args):
         cam = cams[k % len(cams)]
         use.append(crop_camera(cam, frac) if frac < 1.0 else (cam, 1.0))
     for k in range(W):
-        oracle_frame_seconds(osc, use[k][0], ls, le, args.gamma)
+        oracle_frame_seconds(osc, use[k][0], ls, le, args.gamma, args.pair_rule)
     t0 = time.perf_counter()
     done = 0.0
     for k in range(W, W + K):
-        oracle_frame_seconds(osc, use[k][0], ls, le, args.gamma)
+        oracle_frame_seconds(osc, use[k][0], ls, le, args.gamma, args.pair_rule)
         done += use[k][1]
     dt = time.perf_counter() - t0
     value = done / dt
@@ -245,7 +248,7 @@ def workload_config(args, scene, cam, mode, ls, le):
                     f"{'max-level' if mode == 'max' else mode} render (levels {ls}..{le}"
                     + (f", gamma {args.gamma} px" if ls != le else "") + ")",
         "levels": [ls, le], "gamma": args.gamma, "n_gaussians": scene.n_total, "width": cam.width, "height": cam.height,
-        "count_scale": args.count_scale,
+        "count_scale": args.count_scale, "pair_rule": args.pair_rule,
         "selection": (f"materialised G_sel, asynchronous rebuild every {args.subset_period} frames at the current camera "
                       "centre, swapped in when ready (value and stages; e2e uses the per-frame predicate)" if args.subset_period > 0 and ls != le else "Eq. 6 evaluated per frame"),
         "l2": "inputs larger than L2 (scanned level planes + SH exceed 126 MB), no flush between frames",
@@ -289,6 +292,7 @@ def run_ours(args):
     cs = [camera_struct(c) for c in cams]
     cam0 = cams[0]
     r = pkg.Renderer(local_rank)
+    r.set_pair_rule(args.pair_rule)
     scene_bytes = r.upload_levels(scene.levels, scene.sh_degree)
     max_pairs = 32 << 20
     ws_bytes = r.set_workspace(cam0.width, cam0.height, max_pairs)
@@ -450,7 +454,7 @@ def run_ours(args):
     if not args.no_cpu_baseline and world == 1:
         import oracle
         osc = oracle.OracleScene(scene.levels, scene.sh_degree)
-        dt, fr, _ = oracle_frame_seconds(osc, cams[0], ls, le, args.gamma)
+        dt, fr, _ = oracle_frame_seconds(osc, cams[0], ls, le, args.gamma, args.pair_rule)
         line["cpu_baseline"] = {"value": 1.0 / dt, "unit": "frames/s", "cores": oracle.num_threads(), "kind": "oracle",
                                 "sample": "1 full frame (pose 0): selection + projection + pair sort + tiled compositing"}
     print(json.dumps(line), flush=True)

@@ -35,7 +35,7 @@ extern "C" {
 #define FLOD_API
 #endif
 
-#define FLOD_ABI_VERSION 4
+#define FLOD_ABI_VERSION 5
 #define FLOD_MAX_LEVELS 16
 #define FLOD_TILE 16                 /* tiles are 16x16 pixels */
 #define FLOD_N_STAGES 5              /* 0 geometry (a1-a3), 1 colour (a4) with the tile scan (a5, a8) in one of its blocks,
@@ -147,6 +147,16 @@ FLOD_API int flod_set_workspace(flod_ctx *ctx, void *workspace_dev, size_t bytes
 FLOD_API int flod_set_selection_reference(flod_ctx *ctx, const float ref_pos[3]);
 
 FLOD_API int flod_set_options(flod_ctx *ctx, unsigned flags);
+
+/* Which tiles a visible Gaussian is listed in (R13, R26).  Both rules are conservative -- every pixel with
+ * alpha >= 1/255 lies in a listed tile -- so the image is the same; per-tile pair counts, n_pairs and
+ * the sorted pair sequence are those of the chosen rule.
+ *   FLOD_PAIR_RULE_BOX      every tile of the rect (the padded box of the alpha = 1/255 contour);
+ *   FLOD_PAIR_RULE_ELLIPSE  (default) the tiles of the rect that hold a pixel centre of the padded alpha = 1/255 ellipse
+ *                           of Eq. 2: one span of tiles per tile row, computed in fp64 from the rounded
+ *                           conic; 20-30 % fewer pairs. */
+enum { FLOD_PAIR_RULE_BOX = 1, FLOD_PAIR_RULE_ELLIPSE = 2 };
+FLOD_API int flod_set_pair_rule(flod_ctx *ctx, int rule);
 
 /* Steps a1-a9 for one frame, asynchronous on `stream` (a cudaStream_t passed as void*).
  * out_rgb_dev: [3][height][width] planar fp32.  Errors detected on the host are returned here; a capacity

@@ -18,6 +18,7 @@ HEADER = os.path.join(HERE, "..", "include", "flod.h")
 
 FLOD_OPT_DEBUG, FLOD_OPT_PROFILE, FLOD_OPT_COUNT, FLOD_OPT_SMALL_WINDOWS = 1, 2, 4, 8
 FLOD_DBG_MASK, FLOD_DBG_TILE_COUNTS, FLOD_DBG_PROJECTED, FLOD_DBG_SORTED_PAIRS, FLOD_DBG_ACTIVATED = range(5)
+PAIR_RULE_BOX, PAIR_RULE_ELLIPSE = 1, 2
 FLOD_N_STAGES = 5
 STAGE_NAMES = ("geometry", "colour", "duplicate", "tile_sort", "blend")
 ERRORS = {-1: "FLOD_E_INVALID_ARG", -2: "FLOD_E_LEVEL_RANGE", -3: "FLOD_E_NOT_UPLOADED",
@@ -88,6 +89,7 @@ def load_library():
     L.flod_set_workspace.argtypes = [vp, vp, sz, C.c_int, C.c_int, i64]
     L.flod_set_selection_reference.argtypes = [vp, C.POINTER(C.c_float)]
     L.flod_set_options.argtypes = [vp, C.c_uint]
+    L.flod_set_pair_rule.argtypes = [vp, C.c_int]
     L.flod_render.argtypes = [vp, C.POINTER(CameraStruct), LevelMode, C.c_float, vp, vp]
     L.flod_render_to_host.argtypes = [vp, C.POINTER(CameraStruct), LevelMode, C.c_float, vp, vp]
     L.flod_render_to_host_async.argtypes = [vp, C.POINTER(CameraStruct), LevelMode, C.c_float, vp, vp, vp]
@@ -146,6 +148,7 @@ class Renderer:
         self.workspace = None
         self.n_total = 0
         self.ws_dims = None
+        self.pair_rule = PAIR_RULE_ELLIPSE          # the library's default (include/flod.h)
 
     def close(self):
         if getattr(self, "_h", None):
@@ -198,6 +201,10 @@ class Renderer:
         else:
             arr = (C.c_float * 3)(*[float(np.float32(v)) for v in ref_pos])
             self._check(self.lib.flod_set_selection_reference(self._h, arr))
+
+    def set_pair_rule(self, rule: int):
+        self._check(self.lib.flod_set_pair_rule(self._h, rule))
+        self.pair_rule = rule
 
     def set_options(self, flags: int):
         self._check(self.lib.flod_set_options(self._h, flags))

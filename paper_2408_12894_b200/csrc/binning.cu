@@ -31,6 +31,7 @@ __device__ __forceinline__ bool dup_large_rects(const WorkspaceDev &ws)
     return ws.hdr->n_pairs > (unsigned long long)kDupLargeArea * ws.hdr->n_vis32;
 }
 
+template <bool ELLIPSE>
 __global__ void __launch_bounds__(kPreBlock)
 k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs)
 {
@@ -95,18 +96,32 @@ k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs)
         const unsigned int gy = (ty0 >> 1) + k / gw, gx = gx0 + k % gw;
         const unsigned int x = 2u * gx, y = 2u * gy;
         const bool cx0 = x >= tx0, cx1 = x + 1u < tx1, cy0 = y >= ty0, cy1 = y + 1u < ty1;   // x < tx1 and y < ty1 always hold
-        const float4 add = make_float4(cx0 && cy0 ? 1.0f : 0.0f, cx1 && cy0 ? 1.0f : 0.0f,
-                                       cx0 && cy1 ? 1.0f : 0.0f, cx1 && cy1 ? 1.0f : 0.0f);
+        bool h00 = cx0 && cy0, h10 = cx1 && cy0, h01 = cx0 && cy1, h11 = cx1 && cy1;            // tile (x + i, y + j) is listed
+        if (ELLIPSE) {
+            // R26: inside the rect, a tile is listed if it lies in its row's span (span.cuh: the canonical fp32 sequence
+            // k_geometry counted with, so count and emit agree by construction)
+            const float4 fa = ws.gA[p0 + r];
+            const float2 fb = *reinterpret_cast<const float2 *>(ws.gB + p0 + r);
+            const SpanCoef sp = span_coefficients(fa.x, fa.y, fa.z, fa.w, fb.x, fb.y);
+            int ta = 1, tb = 0;
+            if (cy0 && span_of_row(sp, (int)tx0, (int)tx1, (int)y, &ta, &tb) == 0) { ta = 1; tb = 0; }
+            h00 = h00 && (int)x >= ta && (int)x <= tb; h10 = h10 && (int)x + 1 >= ta && (int)x + 1 <= tb;
+            ta = 1; tb = 0;
+            if (cy1 && span_of_row(sp, (int)tx0, (int)tx1, (int)y + 1, &ta, &tb) == 0) { ta = 1; tb = 0; }
+            h01 = h01 && (int)x >= ta && (int)x <= tb; h11 = h11 && (int)x + 1 >= ta && (int)x + 1 <= tb;
+            if (!(h00 || h10 || h01 || h11)) continue;
+        }
+        const float4 add = make_float4(h00 ? 1.0f : 0.0f, h10 ? 1.0f : 0.0f, h01 ? 1.0f : 0.0f, h11 ? 1.0f : 0.0f);
         // the four range starts are fetched BEFORE the atomic, so that their L2 round trips overlap its latency
         const unsigned int t00 = y * (unsigned int)TX + x;
-        const unsigned int s00 = cx0 && cy0 ? ws.ranges[t00].x : 0u, s10 = cx1 && cy0 ? ws.ranges[t00 + 1].x : 0u;
-        const unsigned int s01 = cx0 && cy1 ? ws.ranges[t00 + TX].x : 0u, s11 = cx1 && cy1 ? ws.ranges[t00 + TX + 1].x : 0u;
+        const unsigned int s00 = h00 ? ws.ranges[t00].x : 0u, s10 = h10 ? ws.ranges[t00 + 1].x : 0u;
+        const unsigned int s01 = h01 ? ws.ranges[t00 + TX].x : 0u, s11 = h11 ? ws.ranges[t00 + TX + 1].x : 0u;
         const unsigned long long key = ((unsigned long long)s_depth[r] << 32) | (p0 + r);
         const float4 old = atomicAdd(reinterpret_cast<float4 *>(ws.cursor4 + (size_t)(gy * (unsigned int)GX + gx) * kCtrStride), add);
-        if (cx0 && cy0) { const unsigned int pos = s00 + (unsigned int)old.x; if (pos < max_pairs) ws.pairs[pos] = key; }
-        if (cx1 && cy0) { const unsigned int pos = s10 + (unsigned int)old.y; if (pos < max_pairs) ws.pairs[pos] = key; }
-        if (cx0 && cy1) { const unsigned int pos = s01 + (unsigned int)old.z; if (pos < max_pairs) ws.pairs[pos] = key; }
-        if (cx1 && cy1) { const unsigned int pos = s11 + (unsigned int)old.w; if (pos < max_pairs) ws.pairs[pos] = key; }
+        if (h00) { const unsigned int pos = s00 + (unsigned int)old.x; if (pos < max_pairs) ws.pairs[pos] = key; }
+        if (h10) { const unsigned int pos = s10 + (unsigned int)old.y; if (pos < max_pairs) ws.pairs[pos] = key; }
+        if (h01) { const unsigned int pos = s01 + (unsigned int)old.z; if (pos < max_pairs) ws.pairs[pos] = key; }
+        if (h11) { const unsigned int pos = s11 + (unsigned int)old.w; if (pos < max_pairs) ws.pairs[pos] = key; }
     }
 }
 
@@ -139,10 +154,10 @@ __device__ __forceinline__ void dup_pair(unsigned int *s_cnt, unsigned int t, un
     }
 }
 
-template <bool kEmit>
+template <bool kEmit, bool ELLIPSE>
 __device__ __forceinline__ void dup_pass(const WorkspaceDev &ws, unsigned int *s_cnt, unsigned int *s_pref, unsigned int *s_segn,
-                                         unsigned int *s_wtot, unsigned int TX, unsigned int n_segs, unsigned int win0,
-                                         unsigned int win_n, unsigned int max_pairs)
+                                         unsigned int *s_wtot, unsigned int (*s_row)[32][2], unsigned int TX, unsigned int n_segs,
+                                         unsigned int win0, unsigned int win_n, unsigned int max_pairs)
 {
     const unsigned int tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     // every block walks ALL segments, kDupSegRound at a time, and takes every (32 gridDim)-th unit of the round: a coarse
@@ -173,47 +188,87 @@ __device__ __forceinline__ void dup_pass(const WorkspaceDev &ws, unsigned int *s
         __syncthreads();
         const unsigned int n_units = s_pref[nr];
         for (unsigned int v = warp * gridDim.x + blockIdx.x; v < n_units; v += kDupSWarps * gridDim.x) {
-            {
-                unsigned int lo = 0, hi = nr - 1u;          // the segment k with s_pref[k] <= v < s_pref[k + 1]
-                while (lo < hi) {
-                    const unsigned int mid = (lo + hi + 1u) >> 1;
-                    if (s_pref[mid] <= v) lo = mid; else hi = mid - 1u;
+            unsigned int lo = 0, hi = nr - 1u;          // the segment k with s_pref[k] <= v < s_pref[k + 1]
+            while (lo < hi) {
+                const unsigned int mid = (lo + hi + 1u) >> 1;
+                if (s_pref[mid] <= v) lo = mid; else hi = mid - 1u;
+            }
+            const unsigned int k = lo, c = v - s_pref[lo];
+            const unsigned int seg = k0 + k;
+            const unsigned int j = (c << 5) + lane;
+            const unsigned int p = seg * kGeoBlock + j;
+            unsigned int xy0 = 0, w = 0, h = 0, area = 0, depth = 0;
+            SpanCoef sp{};
+            if (j < s_segn[k]) {
+                const ushort4 rc = ws.rect[p];
+                xy0 = (unsigned int)rc.x | ((unsigned int)rc.y << 16);
+                w = (unsigned int)rc.z - rc.x; h = (unsigned int)rc.w - rc.y;
+                area = w * h;
+                if (kEmit) depth = ws.depth[p];
+                if (ELLIPSE) {
+                    const float4 fa = ws.gA[p];
+                    const float2 fb = *reinterpret_cast<const float2 *>(ws.gB + p);
+                    sp = span_coefficients(fa.x, fa.y, fa.z, fa.w, fb.x, fb.y);
                 }
-                const unsigned int k = lo, c = v - s_pref[lo];
-                const unsigned int seg = k0 + k;
-                const unsigned int j = (c << 5) + lane;
-                const unsigned int p = seg * kGeoBlock + j;
-                unsigned int xy0 = 0, w = 0, area = 0, depth = 0;
-                if (j < s_segn[k]) {
-                    const ushort4 rc = ws.rect[p];
-                    xy0 = (unsigned int)rc.x | ((unsigned int)rc.y << 16);
-                    w = (unsigned int)rc.z - rc.x;
-                    area = w * ((unsigned int)rc.w - rc.y);
-                    if (kEmit) depth = ws.depth[p];
+            }
+            if (area <= kDupInline) {                   // small rects: every lane walks its own
+                const unsigned long long key = ((unsigned long long)depth << 32) | p;
+                const unsigned int tx0 = xy0 & 0xffffu, ty0 = xy0 >> 16;
+                for (unsigned int dy = 0; dy < h; ++dy) {
+                    int ta = (int)tx0, tb = (int)(tx0 + w) - 1;
+                    if (ELLIPSE && span_of_row(sp, (int)tx0, (int)(tx0 + w), (int)(ty0 + dy), &ta, &tb) == 0) continue;
+                    for (int tx = ta; tx <= tb; ++tx)
+                        dup_pair<kEmit>(s_cnt, (ty0 + dy) * TX + (unsigned int)tx, win0, win_n, key, ws.pairs, max_pairs);
                 }
-                if (area <= kDupInline) {                   // small rects: every lane walks its own
-                    const unsigned long long key = ((unsigned long long)depth << 32) | p;
-                    unsigned int t = (xy0 >> 16) * TX + (xy0 & 0xffffu), x = 0;
-                    for (unsigned int i = 0; i < area; ++i) {
-                        dup_pair<kEmit>(s_cnt, t, win0, win_n, key, ws.pairs, max_pairs);
-                        ++t;
-                        if (++x == w) { x = 0; t += TX - w; }
-                    }
-                }
-                unsigned int big = __ballot_sync(0xffffffffu, area > kDupInline);
-                while (big) {                               // large rects: the whole warp expands one at a time
-                    const int r = __ffs((int)big) - 1;
-                    big &= big - 1u;
-                    const unsigned int rxy = __shfl_sync(0xffffffffu, xy0, r), rw = __shfl_sync(0xffffffffu, w, r);
-                    const unsigned int ra = __shfl_sync(0xffffffffu, area, r), rd = __shfl_sync(0xffffffffu, depth, r);
-                    const unsigned long long key = ((unsigned long long)rd << 32) | (p - lane + (unsigned int)r);
-                    const unsigned int t0 = (rxy >> 16) * TX + (rxy & 0xffffu);
+            }
+            unsigned int big = __ballot_sync(0xffffffffu, area > kDupInline);
+            while (big) {                               // large rects: the whole warp expands one at a time
+                const int r = __ffs((int)big) - 1;
+                big &= big - 1u;
+                const unsigned int rxy = __shfl_sync(0xffffffffu, xy0, r), rw = __shfl_sync(0xffffffffu, w, r);
+                const unsigned int ra = __shfl_sync(0xffffffffu, area, r), rd = __shfl_sync(0xffffffffu, depth, r);
+                const unsigned long long key = ((unsigned long long)rd << 32) | (p - lane + (unsigned int)r);
+                const unsigned int tx0 = rxy & 0xffffu, ty0 = rxy >> 16, t0 = ty0 * TX + tx0;
+                if (!ELLIPSE) {
                     // q / rw by multiplication: exact for q < 2^16 (inv = ceil(2^32 / rw), rw < 2^16)
                     const unsigned int inv = rw > 1u ? 0xffffffffu / rw + 1u : 0u;
                     const bool fast = ra <= 65536u && rw > 1u;
                     for (unsigned int q = lane; q < ra; q += 32u) {
                         const unsigned int dy = fast ? __umulhi(q, inv) : q / rw;
                         dup_pair<kEmit>(s_cnt, t0 + dy * TX + (q - dy * rw), win0, win_n, key, ws.pairs, max_pairs);
+                    }
+                } else {
+                    // R26: 32 tile rows at a time, one row's span per lane; the listed tiles of the chunk are then dealt to
+                    // the lanes through an exclusive scan of the span lengths
+                    SpanCoef rs;
+                    rs.sl = __shfl_sync(0xffffffffu, sp.sl, r); rs.KA = __shfl_sync(0xffffffffu, sp.KA, r);
+                    rs.DA = __shfl_sync(0xffffffffu, sp.DA, r); rs.dyt = __shfl_sync(0xffffffffu, sp.dyt, r);
+                    rs.pad = __shfl_sync(0xffffffffu, sp.pad, r); rs.mx = __shfl_sync(0xffffffffu, sp.mx, r);
+                    rs.my = __shfl_sync(0xffffffffu, sp.my, r); rs.box = __shfl_sync(0xffffffffu, (int)sp.box, r) != 0;
+                    const unsigned int rh = ra / rw;
+                    for (unsigned int r0 = 0; r0 < rh; r0 += 32u) {
+                        int ta = 1, tb = 0;
+                        if (r0 + lane < rh && span_of_row(rs, (int)tx0, (int)(tx0 + rw), (int)(ty0 + r0 + lane), &ta, &tb) == 0) { ta = 1; tb = 0; }
+                        const unsigned int n = tb >= ta ? (unsigned int)(tb - ta + 1) : 0u;
+                        unsigned int incl = n;
+#pragma unroll
+                        for (int o = 1; o < 32; o <<= 1) {
+                            const unsigned int t = __shfl_up_sync(0xffffffffu, incl, o);
+                            if (lane >= o) incl += t;
+                        }
+                        const unsigned int total = __shfl_sync(0xffffffffu, incl, 31);
+                        __syncwarp();
+                        s_row[warp][lane][0] = incl - n;                        // index of the row's first listed tile in the chunk
+                        s_row[warp][lane][1] = (ty0 + r0 + lane) * TX + (unsigned int)ta;
+                        __syncwarp();
+                        for (unsigned int q = lane; q < total; q += 32u) {
+                            unsigned int a = 0, b = 31;                         // last row whose first index is <= q
+                            while (a < b) {
+                                const unsigned int mid = (a + b + 1u) >> 1;
+                                if (s_row[warp][mid][0] <= q) a = mid; else b = mid - 1u;
+                            }
+                            dup_pair<kEmit>(s_cnt, s_row[warp][a][1] + (q - s_row[warp][a][0]), win0, win_n, key, ws.pairs, max_pairs);
+                        }
                     }
                 }
             }
@@ -222,6 +277,7 @@ __device__ __forceinline__ void dup_pass(const WorkspaceDev &ws, unsigned int *s
     }
 }
 
+template <bool ELLIPSE>
 __global__ void __launch_bounds__(kDupSThreads, 1)
 k_duplicate_shared(const WorkspaceDev ws, unsigned int TX, unsigned int T_n, unsigned int n_segs, unsigned int win_cap,
                    unsigned int max_pairs)
@@ -230,36 +286,44 @@ k_duplicate_shared(const WorkspaceDev ws, unsigned int TX, unsigned int T_n, uns
     __shared__ unsigned int s_pref[kDupSegRound + 1];
     __shared__ unsigned int s_segn[kDupSegRound];
     __shared__ unsigned int s_wtot[kDupSegRound / 32];
+    __shared__ unsigned int s_row[kDupSWarps][32][2];   // per warp: (index of the first listed tile, its tile id) of 32 tile rows
     if (!dup_large_rects(ws)) return;
     const unsigned int tid = threadIdx.x;
     for (unsigned int win0 = 0; win0 < T_n; win0 += win_cap) {
         const unsigned int win_n = min(win_cap, T_n - win0);
         for (unsigned int r = tid; r < win_n; r += kDupSThreads) s_cnt[r] = 0;
         __syncthreads();
-        dup_pass<false>(ws, s_cnt, s_pref, s_segn, s_wtot, TX, n_segs, win0, win_n, max_pairs);
+        dup_pass<false, ELLIPSE>(ws, s_cnt, s_pref, s_segn, s_wtot, s_row, TX, n_segs, win0, win_n, max_pairs);
         for (unsigned int r = tid; r < win_n; r += kDupSThreads) {      // (dup_pass ends with a barrier)
             const unsigned int c = s_cnt[r];
             if (c) s_cnt[r] = ws.ranges[win0 + r].x + atomicAdd(&ws.cursor[win0 + r], c);
         }
         __syncthreads();
-        dup_pass<true>(ws, s_cnt, s_pref, s_segn, s_wtot, TX, n_segs, win0, win_n, max_pairs);
+        dup_pass<true, ELLIPSE>(ws, s_cnt, s_pref, s_segn, s_wtot, s_row, TX, n_segs, win0, win_n, max_pairs);
     }
 }
 
 int init_duplicate()
 {
-    return cudaFuncSetAttribute(k_duplicate_shared, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                kDupWinCap * (int)sizeof(unsigned int)) == cudaSuccess ? 0 : -1;
+    const int bytes = kDupWinCap * (int)sizeof(unsigned int);
+    return cudaFuncSetAttribute(k_duplicate_shared<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess &&
+           cudaFuncSetAttribute(k_duplicate_shared<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess ? 0 : -1;
 }
 
 int launch_duplicate(const Context &c, const FrameParams &p, cudaStream_t s)
 {
     if (p.n_pre_blocks <= 0) return 0;
-    k_duplicate<<<p.n_pre_blocks, kPreBlock, 0, s>>>(c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs);
     const unsigned int T_n = (unsigned int)p.n_tiles;
     const unsigned int win_cap = (c.flags & FLOD_OPT_SMALL_WINDOWS) ? 1024u : min(T_n, (unsigned int)kDupWinCap);
-    k_duplicate_shared<<<c.sm_count, kDupSThreads, win_cap * sizeof(unsigned int), s>>>(
-        c.ws, (unsigned int)p.TX, T_n, (unsigned int)p.n_pre_blocks, win_cap, p.max_pairs);
+    if (p.pair_rule == FLOD_PAIR_RULE_BOX) {
+        k_duplicate<false><<<p.n_pre_blocks, kPreBlock, 0, s>>>(c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs);
+        k_duplicate_shared<false><<<c.sm_count, kDupSThreads, win_cap * sizeof(unsigned int), s>>>(
+            c.ws, (unsigned int)p.TX, T_n, (unsigned int)p.n_pre_blocks, win_cap, p.max_pairs);
+    } else {
+        k_duplicate<true><<<p.n_pre_blocks, kPreBlock, 0, s>>>(c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs);
+        k_duplicate_shared<true><<<c.sm_count, kDupSThreads, win_cap * sizeof(unsigned int), s>>>(
+            c.ws, (unsigned int)p.TX, T_n, (unsigned int)p.n_pre_blocks, win_cap, p.max_pairs);
+    }
     return 2;
 }
 

@@ -341,6 +341,14 @@ int flod_set_options(flod_ctx *ctx, unsigned flags)
     return FLOD_OK;
 }
 
+int flod_set_pair_rule(flod_ctx *ctx, int rule)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    if (rule != FLOD_PAIR_RULE_BOX && rule != FLOD_PAIR_RULE_ELLIPSE) return fail(ctx, FLOD_E_INVALID_ARG, "pair rule is 1 (box) or 2 (ellipse)");
+    ctx->pair_rule = rule;
+    return FLOD_OK;
+}
+
 int flod_launches_per_frame(const flod_ctx *ctx)
 {
     if (!ctx || !ctx->has_ws) return 0;
@@ -416,6 +424,7 @@ int enqueue_frame(flod_ctx *ctx, const SceneDev &sc, FrameParams &p, float *out_
 {
     const int64_t n_scan = p.n_scan;
     p.max_pairs = (unsigned int)ctx->max_pairs;
+    p.pair_rule = ctx->pair_rule;
     p.quad_gid = p.first_gid & ~3ll;
     p.n_pre_blocks = (int)((p.first_gid - p.quad_gid + n_scan + kGeoBlock - 1) / kGeoBlock);
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));

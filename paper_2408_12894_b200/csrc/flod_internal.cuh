@@ -8,6 +8,7 @@
 #include <string>
 
 #include "../../include/flod.h"
+#include "span.cuh"
 
 namespace flod {
 
@@ -111,6 +112,7 @@ struct FrameParams {
     unsigned int max_pairs;
     int n_pre_blocks;                     // blocks of k_geometry
     int n_tiles;                          // TX * TY
+    int pair_rule;                        // FLOD_PAIR_RULE_BOX / FLOD_PAIR_RULE_ELLIPSE
 };
 
 struct Context {
@@ -132,6 +134,7 @@ struct Context {
     int64_t max_pairs = 0;
     // options / state
     unsigned flags = 0;
+    int pair_rule = FLOD_PAIR_RULE_ELLIPSE;
     bool has_ref = false;
     float ref[3] = {0, 0, 0};
     cudaStream_t last_stream = nullptr;

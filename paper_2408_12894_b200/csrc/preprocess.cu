@@ -73,7 +73,7 @@ struct GeoSmem {
     unsigned long long pairs;
 };
 
-template <bool DEBUG>
+template <bool DEBUG, bool ELLIPSE>
 __global__ void __launch_bounds__(kGeoThreads)
 k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ FrameParams p)
 {
@@ -185,13 +185,13 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
     for (unsigned int s0 = 0, step = 0; s0 < n_cand; s0 += kGeoThreads, ++step) {
         const unsigned int s = s0 + tid;
         bool vis = false;
-        float mx2 = 0.f, my2 = 0.f, z = 0.f, cA = 0.f, cB = 0.f, cC = 0.f, l2o = 0.f, wxk = 0.f, wyk = 0.f, wzk = 0.f;
+        float mx2 = 0.f, my2 = 0.f, z = 0.f, cA = 0.f, cB = 0.f, cC = 0.f, l2o = 0.f, wxk = 0.f, wyk = 0.f, wzk = 0.f, kap = 0.f;
         int tx0 = 0, tx1 = 0, ty0 = 0, ty1 = 0;
         long long g = 0;
         if (s < n_cand) {
             g = gb + S.cand[s];
             wxk = __ldg(sc.mx + g); wyk = __ldg(sc.my + g); wzk = __ldg(sc.mz + g);
-            const float kap = __ldg(sc.kappa + g);
+            kap = __ldg(sc.kappa + g);
             const float Sxx = __ldg(sc.cov[0] + g), Sxy = __ldg(sc.cov[1] + g), Sxz = __ldg(sc.cov[2] + g);
             const float Syy = __ldg(sc.cov[3] + g), Syz = __ldg(sc.cov[4] + g), Szz = __ldg(sc.cov[5] + g);
             l2o = __ldg(sc.l2o + g);
@@ -251,16 +251,17 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
         }
         n_vis_before += step_total;
         if (vis) {
-            my_pairs += (unsigned int)((tx1 - tx0) * (ty1 - ty0));
-            // DESIGN R25: factorised exponent from the ROUNDED conic, derived in fp64, rounded once
-            const double LOG2E = 1.4426950408889634;
+            // DESIGN R25: factorised exponent from the ROUNDED conic, derived in fp64, rounded once.  Canonical (every
+            // operation one IEEE binary64 operation, written order): pair rule 2 (R26, span.cuh) takes the contour from
+            // these values, and the oracle restates the derivation.
+            const double HL2E = -0.5 * 1.4426950408889634;
             const double dA = (double)cA, dB = (double)cB, dC = (double)cC;
-            const double rA = 1.0 / dA;
-            const float kk = (float)(dB * rA);
-            const float a2 = (float)(-0.5 * LOG2E * dA);               // stored negated: e = log2 o + a2 w^2 + d2 dy^2
+            const double rA = __ddiv_rn(1.0, dA);
+            const float kk = (float)__dmul_rn(dB, rA);
+            const float a2 = (float)__dmul_rn(HL2E, dA);                 // stored negated: e = log2 o + a2 w^2 + d2 dy^2
             // <= 0 so that q >= 0 holds by construction in k_blend (the oracle clamps q at 0; a conic left indefinite by
             // rounding differs from its clamp by less than R25's evaluation error)
-            const float d2 = fminf((float)(-0.5 * LOG2E * (dC - dB * dB * rA)), 0.0f);
+            const float d2 = fminf((float)__dmul_rn(HL2E, __dsub_rn(dC, __dmul_rn(__dmul_rn(dB, dB), rA))), 0.0f);
             const size_t c = (size_t)seg_base + pos;
             ws.gA[c] = make_float4(mx2, my2, kk, a2);
             reinterpret_cast<float2 *>(ws.gB)[2 * c] = make_float2(d2, l2o);          // (r, g) by k_colour
@@ -276,12 +277,27 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
                 d.rect[0] = tx0; d.rect[1] = ty0; d.rect[2] = tx1; d.rect[3] = ty1;
                 ws.dbg[c] = d;
             }
-            // a5, first half: +1 over the rect in the 2-D difference grid of the per-tile pair counts
+            // a5, first half: the difference grid of the per-tile pair counts
             const int gw = p.TX + 1;
-            atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx0) * kCtrStride, 1);
-            atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx1) * kCtrStride, -1);
-            atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx0) * kCtrStride, -1);
-            atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx1) * kCtrStride, 1);
+            if (!ELLIPSE) {
+                // +1 over the rect in a 2-D difference grid: four atomics whatever the rect's area
+                my_pairs += (unsigned int)((tx1 - tx0) * (ty1 - ty0));
+                atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx0) * kCtrStride, 1);
+                atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx1) * kCtrStride, -1);
+                atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx0) * kCtrStride, -1);
+                atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx1) * kCtrStride, 1);
+            } else {
+                // R26: one span of listed tiles per tile row (span.cuh), +1 / -1 at its ends in a row-wise difference grid
+                const SpanCoef sp = span_coefficients(mx2, my2, kk, a2, d2, l2o);
+                for (int ty = ty0; ty < ty1; ++ty) {
+                    int ta, tb;
+                    const int n = span_of_row(sp, tx0, tx1, ty, &ta, &tb);
+                    if (n == 0) continue;
+                    my_pairs += (unsigned int)n;
+                    atomicAdd(ws.tile_diff + (size_t)(ty * gw + ta) * kCtrStride, 1);
+                    atomicAdd(ws.tile_diff + (size_t)(ty * gw + tb + 1) * kCtrStride, -1);
+                }
+            }
         }
     }
     // ---- block totals
@@ -305,10 +321,10 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
 // coefficients k = 4 j .. 4 j + 3, so one load instruction of the 4 lanes reads 64 contiguous bytes.
 template <int DEG, int LANES, bool DEBUG>
 __global__ void __launch_bounds__(256)
-k_colour(const SceneDev sc, const WorkspaceDev ws, int TX, int TY, unsigned int max_pairs)
+k_colour(const SceneDev sc, const WorkspaceDev ws, int TX, int TY, unsigned int max_pairs, int pair_rule)
 {
     constexpr int K = (DEG + 1) * (DEG + 1);
-    if (blockIdx.x == 0) { tile_scan_block(ws, TX, TY, max_pairs); return; }
+    if (blockIdx.x == 0) { tile_scan_block(ws, TX, TY, max_pairs, pair_rule != FLOD_PAIR_RULE_BOX); return; }
     const unsigned int sub = threadIdx.x % LANES;
     const unsigned int per_block = 256 / LANES;
     const unsigned int seg = blockIdx.x - 1;             // one block per segment of k_geometry
@@ -396,16 +412,22 @@ k_colour(const SceneDev sc, const WorkspaceDev ws, int TX, int TY, unsigned int 
 int launch_geometry(const Context &c, const SceneDev &sc, const FrameParams &p, cudaStream_t s)
 {
     if (p.n_pre_blocks <= 0) return 0;
-    if (c.flags & FLOD_OPT_DEBUG) k_geometry<true><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(sc, c.ws, p);
-    else k_geometry<false><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(sc, c.ws, p);
+    const bool ell = p.pair_rule != FLOD_PAIR_RULE_BOX;
+    if (c.flags & FLOD_OPT_DEBUG) {
+        if (ell) k_geometry<true, true><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(sc, c.ws, p);
+        else k_geometry<true, false><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(sc, c.ws, p);
+    } else {
+        if (ell) k_geometry<false, true><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(sc, c.ws, p);
+        else k_geometry<false, false><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(sc, c.ws, p);
+    }
     return 1;
 }
 
 template <int DEG, int LANES>
 static void launch_colour_t(const Context &c, const FrameParams &p, int grid, cudaStream_t s)
 {
-    if (c.flags & FLOD_OPT_DEBUG) k_colour<DEG, LANES, true><<<grid, 256, 0, s>>>(c.scene, c.ws, p.TX, p.TY, p.max_pairs);
-    else k_colour<DEG, LANES, false><<<grid, 256, 0, s>>>(c.scene, c.ws, p.TX, p.TY, p.max_pairs);
+    if (c.flags & FLOD_OPT_DEBUG) k_colour<DEG, LANES, true><<<grid, 256, 0, s>>>(c.scene, c.ws, p.TX, p.TY, p.max_pairs, p.pair_rule);
+    else k_colour<DEG, LANES, false><<<grid, 256, 0, s>>>(c.scene, c.ws, p.TX, p.TY, p.max_pairs, p.pair_rule);
 }
 
 int launch_colour(const Context &c, const FrameParams &p, cudaStream_t s)

@@ -10,7 +10,9 @@
 
 namespace flod {
 
-__device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, int TY, unsigned int max_pairs)
+// rowwise: the grid holds one +1 / -1 pair per (Gaussian, tile row) (pair rule 2), so the prefix along x alone gives the
+// counts; otherwise +1 -1 -1 +1 at the corners of every rect (pair rule 1) and the prefix runs along x, then y.
+__device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, int TY, unsigned int max_pairs, bool rowwise)
 {
     __shared__ unsigned long long s_wtot[32];
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
@@ -36,7 +38,7 @@ __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, 
     }
     __syncthreads();
     // ---- prefix along y: a thread owns a column, eight independent loads in flight per step
-    for (int x = tid; x < gw; x += nthr) {
+    for (int x = tid; x < gw && !rowwise; x += nthr) {
         int run = 0;
         for (int y0 = 0; y0 < gh; y0 += 8) {
             int v[8];

@@ -60,6 +60,14 @@ def test_config3_single_level(config3, l):
             print(f"config3 level {l} pose {pose}: P={fr.counts['n_pairs']} n_vis={fr.counts['n_vis']} "
                   f"max list={int(fr.tile_counts.max())} max|gpu-oracle|={res[0]:.2e} marginal={res[1]}")
     assert fr.counts["n_scan"] == scene.levels[l - 1].n
+    if l == 3:      # the box rule (R13) on the heaviest frame of the config
+        import paper_2408_12894_b200 as pkg
+        r.set_pair_rule(pkg.PAIR_RULE_BOX)
+        try:
+            _, _, fr1 = check_frame(r, osc, cams[61], l, l, 1.0, image=False)
+        finally:
+            r.set_pair_rule(pkg.PAIR_RULE_ELLIPSE)
+        print(f"config3 level 3 pose 61: P box rule {fr1.counts['n_pairs']}, ellipse rule {fr.counts['n_pairs']}")
 
 
 @pytest.fixture(scope="module")
@@ -102,7 +110,7 @@ def test_config4_materialised_subset_on_the_walk(config4):
     for pose, ref in ((100, None), (110, c100)):
         img = r.render_subset(cams[pose]).cpu().numpy()
         st = r.get_stats()
-        fr = osc.frame(cams[pose], 3, 5, 1.0, ref_pos=ref, geometry_only=True)
+        fr = osc.frame(cams[pose], 3, 5, 1.0, ref_pos=ref, geometry_only=True, pair_rule=r.pair_rule)
         c = fr.counts
         assert n_sel == c["n_sel"] == st["n_sel"] and (st["n_front"], st["n_vis"], st["n_pairs"]) == (c["n_front"], c["n_vis"], c["n_pairs"])
         assert np.array_equal(r.debug_mask(), fr.mask)

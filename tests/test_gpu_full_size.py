@@ -36,7 +36,7 @@ def _geometry_exact(r, osc, cam, ls, le, gamma, geometry_only=False):
     img = r.render(cam, ls, le, gamma)
     img = None if geometry_only else img.cpu().numpy()
     st = r.get_stats()
-    fr = osc.frame(cam, ls, le, gamma, geometry_only=geometry_only)
+    fr = osc.frame(cam, ls, le, gamma, geometry_only=geometry_only, pair_rule=r.pair_rule)
     c = fr.counts
     assert (st["n_scan"], st["n_sel"], st["n_front"], st["n_vis"], st["n_pairs"]) == (
         c["n_scan"], c["n_sel"], c["n_front"], c["n_vis"], c["n_pairs"])
@@ -53,8 +53,18 @@ def test_activation_bit_exact_full_scene(full):
     assert np.array_equal(act[~dead, 7], osc.kappa[~dead]) and (act[dead, 7] == -1.0).all()
 
 
-def test_config1_max_level_pose0_everything(full):
-    """Level 5, pose 0: every checked intermediate and the full image."""
+@pytest.mark.parametrize("rule", [2, 1])
+def test_config1_max_level_pose0_everything(full, rule):
+    """Level 5, pose 0: every checked intermediate and the full image, under both pair rules (R13 box, R26 ellipse)."""
+    scene, cams, osc, r = full
+    r.set_pair_rule(rule)
+    try:
+        _config1_pose0(full)
+    finally:
+        r.set_pair_rule(2)
+
+
+def _config1_pose0(full):
     scene, cams, osc, r = full
     img, fr, st = _geometry_exact(r, osc, cams[0], 5, 5, 1.0)
     assert st["n_pairs"] > 3_000_000 and fr.TX * fr.TY == 4056
@@ -70,7 +80,7 @@ def test_config1_max_level_pose0_everything(full):
     assert np.array_equal(pr["mu2d"], fr.mu2d[vis]) and np.array_equal(pr["conic"], fr.conic[vis])
     assert np.abs(pr["rgb"].astype(np.float64) - fr.rgb[vis]).max() <= 1e-5
     dmax, n_marginal = check_image(img, fr)
-    print(f"config1 L5 pose0: max|gpu-oracle|={dmax:.2e}, marginal pixels={n_marginal}")
+    print(f"config1 L5 pose0 pair rule {r.pair_rule}: P={st['n_pairs']} max|gpu-oracle|={dmax:.2e}, marginal pixels={n_marginal}")
 
 
 @pytest.mark.parametrize("pose", [67, 133])
@@ -138,7 +148,7 @@ def test_materialised_subset_equals_fused_selection(full):
     for pose, ref in ((50, None), (55, c50)):
         img = r.render_subset(cams[pose]).cpu().numpy()
         st = r.get_stats()
-        fr = osc.frame(cams[pose], 3, 5, 2.0, ref_pos=ref)
+        fr = osc.frame(cams[pose], 3, 5, 2.0, ref_pos=ref, pair_rule=r.pair_rule)
         c = fr.counts
         assert n_sel == c["n_sel"] == st["n_sel"] == st["n_scan"]
         assert (st["n_front"], st["n_vis"], st["n_pairs"]) == (c["n_front"], c["n_vis"], c["n_pairs"])
@@ -189,7 +199,7 @@ def test_coarse_level_duplication_shared_counters_and_windows(full):
     sequence must be the oracle's either way."""
     import paper_2408_12894_b200 as pkg
     scene, cams, osc, r = full
-    fr = osc.frame(cams[3], 1, 1, 1.0)
+    fr = osc.frame(cams[3], 1, 1, 1.0, pair_rule=r.pair_rule)
     assert fr.counts["n_pairs"] > 128 * fr.counts["n_vis"]          # the large-rect kernel's condition
     tile, depth, gid = fr.sorted_pairs()
     for flags in (pkg.FLOD_OPT_DEBUG, pkg.FLOD_OPT_DEBUG | pkg.FLOD_OPT_SMALL_WINDOWS):

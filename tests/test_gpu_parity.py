@@ -59,7 +59,7 @@ def check_frame(r, osc, cam, l_start, l_end, gamma, ref_pos=None, image=True):
     r.set_selection_reference(ref_pos)
     img = r.render(cam, l_start, l_end, gamma).cpu().numpy()
     st = r.get_stats()
-    fr = osc.frame(cam, l_start, l_end, gamma, ref_pos)
+    fr = osc.frame(cam, l_start, l_end, gamma, ref_pos, pair_rule=r.pair_rule)
     c = fr.counts
     assert (st["n_scan"], st["n_sel"], st["n_front"], st["n_vis"], st["n_pairs"]) == (
         c["n_scan"], c["n_sel"], c["n_front"], c["n_vis"], c["n_pairs"])
@@ -110,6 +110,27 @@ def test_config0_max_level(config0):
     assert fr.counts["n_pairs"] > 10000 and dmax <= 1e-3 + 4e-3
 
 
+def test_config0_both_pair_rules(pkg, config0):
+    """R13 / R26: the box rule and the ellipse rule give their own per-tile counts and pair sequences --
+    each exactly the oracle's for that rule -- and the same image bit for bit (a dropped tile holds no pixel with
+    alpha >= 1/255, so no blended term changes)."""
+    sc, cam, osc, r = config0
+    imgs, pairs = {}, {}
+    try:
+        for rule in (pkg.PAIR_RULE_BOX, pkg.PAIR_RULE_ELLIPSE):
+            r.set_pair_rule(rule)
+            for (ls, le) in ((2, 2), (1, 2)):
+                _, img, fr = check_frame(r, osc, cam, ls, le, 1.0)
+                imgs[rule, ls] = img
+                pairs[rule, ls] = fr.counts["n_pairs"]
+    finally:
+        r.set_pair_rule(pkg.PAIR_RULE_ELLIPSE)
+    for ls in (2, 1):
+        assert np.array_equal(imgs[1, ls], imgs[2, ls]) and pairs[2, ls] < 0.95 * pairs[1, ls]
+    with pytest.raises(pkg.FlodError):
+        r.set_pair_rule(3)
+
+
 def test_config0_selective(config0):
     """BASELINE.json config 0: selective render with levels {1,2}, gamma = 1 px."""
     sc, cam, osc, r = config0
@@ -142,7 +163,7 @@ def test_brute_force_parity_on_tiny_input(config0):
     sc, cam, osc, r = config0
     for (ls, le) in ((1, 2), (2, 2)):
         img = r.render(cam, ls, le, 1.0).cpu().numpy()
-        check_image(img, osc.frame(cam, ls, le, 1.0), brute=True)
+        check_image(img, osc.frame(cam, ls, le, 1.0, pair_rule=r.pair_rule), brute=True)
 
 
 # ------------------------------------------------------------------------- edge cases, small scenes
@@ -178,9 +199,11 @@ def test_random_scenes(pkg, seed, counts, wh, deg):
     osc = OracleScene(lv, deg)
     r = make_renderer(pkg, lv, deg, wh[0], wh[1], max_pairs=1 << 21)
     L = len(counts)
-    check_frame(r, osc, cam, L, L, 1.0)
-    check_frame(r, osc, cam, 1, L, 2.0)
-    check_frame(r, osc, cam, 1, 1, 1.0)
+    for rule in (pkg.PAIR_RULE_ELLIPSE, pkg.PAIR_RULE_BOX):
+        r.set_pair_rule(rule)
+        check_frame(r, osc, cam, L, L, 1.0)
+        check_frame(r, osc, cam, 1, L, 2.0)
+        check_frame(r, osc, cam, 1, 1, 1.0)
     r.close()
 
 
@@ -212,8 +235,10 @@ def test_screen_filling_and_degenerate_gaussians(pkg):
                opacity=[0.3, 0.9, 0.8, 0.99, 0.6, 0.5], rgb=[[1, 0, 0], [0, 1, 0], [0, 0, 1], [1, 1, 0], [0, 1, 1], [1, 0, 1]])
     r = make_renderer(pkg, [lv], 0, 96, 64)
     osc = OracleScene([lv], 0)
-    (dmax, _), img, fr = check_frame(r, osc, cam, 1, 1, 1.0)
-    assert fr.n_tiles.max() == fr.TX * fr.TY
+    for rule in (pkg.PAIR_RULE_BOX, pkg.PAIR_RULE_ELLIPSE):
+        r.set_pair_rule(rule)
+        (dmax, _), img, fr = check_frame(r, osc, cam, 1, 1, 1.0)
+        assert fr.n_tiles.max() == fr.TX * fr.TY
     r.close()
 
 
@@ -254,6 +279,10 @@ def test_needle_gaussians_stay_within_tolerance(pkg):
     r = make_renderer(pkg, [lv], 0, 640, 400)
     osc = OracleScene([lv], 0)
     (dmax, nm), img, fr = check_frame(r, osc, cam, 1, 1, 1.0)
+    r.set_pair_rule(pkg.PAIR_RULE_BOX)
+    _, img1, fr1 = check_frame(r, osc, cam, 1, 1, 1.0)
+    # (thin diagonal needles keep the box rule -- their determinant cancels in fp32, R26 -- the others are cut down)
+    assert np.array_equal(img, img1) and fr.counts["n_pairs"] <= fr1.counts["n_pairs"]
     r.close()
 
 
@@ -344,7 +373,7 @@ def test_errors_and_capacity(pkg):
         r.get_stats()
     assert e.value.code == -5
     st = r.get_stats(raise_on_overflow=False)
-    need = OracleScene(lv, 0).frame(cam, 2, 2, 1.0).counts["n_pairs"]
+    need = OracleScene(lv, 0).frame(cam, 2, 2, 1.0, pair_rule=r.pair_rule).counts["n_pairs"]
     assert st["overflow"] == 1 and st["n_pairs"] == need > 256
     # the host-buffer calls block on the frame anyway, so they report the overflow themselves
     with pytest.raises(pkg.FlodError) as e:
@@ -430,7 +459,7 @@ def test_instrumented_counts_match_oracle(pkg, config0):
     r = make_renderer(pkg, sc.levels, sc.sh_degree, cam.width, cam.height, flags=pkg.FLOD_OPT_COUNT | pkg.FLOD_OPT_PROFILE)
     r.render(cam, 2, 2, 1.0)
     st = r.get_stats()
-    _, E, B, _ = osc.frame(cam, 2, 2, 1.0).composite(stats=True)
+    _, E, B, _ = osc.frame(cam, 2, 2, 1.0, pair_rule=r.pair_rule).composite(stats=True)
     assert abs(st["blends"] - int(B.sum())) <= max(20, 1e-3 * B.sum())
     assert abs(st["evals"] - int(E.sum())) <= max(20, 1e-3 * E.sum())
     assert st["ms_total"] > 0 and all(m >= 0 for m in st["ms_stage"])
@@ -472,7 +501,7 @@ def test_subset_small_scenes_errors_and_empty_selection(pkg):
         n_sel = r.subset_swap()
         img = r.render_subset(cam).cpu().numpy()
         st = r.get_stats()
-        fr = osc.frame(cam, 1, 3, gamma, ref_pos=ref)
+        fr = osc.frame(cam, 1, 3, gamma, ref_pos=ref, pair_rule=r.pair_rule)
         c = fr.counts
         assert n_sel == c["n_sel"] and (st["n_front"], st["n_vis"], st["n_pairs"]) == (c["n_front"], c["n_vis"], c["n_pairs"])
         assert np.array_equal(r.debug_mask(), fr.mask)
@@ -511,6 +540,7 @@ def test_random_scenes_every_kernel_path(pkg, seed):
     r = make_renderer(pkg, lv, deg, W, H, max_pairs=1 << 23)
     if seed % 4 == 0:
         r.set_options(pkg.FLOD_OPT_DEBUG | pkg.FLOD_OPT_SMALL_WINDOWS)
+    r.set_pair_rule(pkg.PAIR_RULE_BOX if seed % 5 == 0 else pkg.PAIR_RULE_ELLIPSE)
     check_frame(r, osc, cam, L, L, 1.0)
     check_frame(r, osc, cam, 1, L, float(rng.uniform(0.5, 4)))
     ref = rng.uniform(-2, 2, 3).astype(np.float32); gamma = float(rng.uniform(0.5, 4))
@@ -520,5 +550,5 @@ def test_random_scenes_every_kernel_path(pkg, seed):
     b = r.render(cam, 1, L, gamma).cpu().numpy()
     r.set_selection_reference(None)
     assert np.array_equal(a, b)
-    check_image(a, osc.frame(cam, 1, L, gamma, ref_pos=ref))
+    check_image(a, osc.frame(cam, 1, L, gamma, ref_pos=ref, pair_rule=r.pair_rule))
     r.close()
