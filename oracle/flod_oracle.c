@@ -434,8 +434,9 @@ static int ellipse_row_span(float mx, float my, float cA, float cB, float cC, fl
     if (!(a > 0.0f)) return tx1 - tx0;                       /* not an ellipse after rounding: the box rule */
     const float E = (l2o + 7.994353436858858f) * 1.001953125f + 0.0000152587890625f;
     const float sl = -k;
-    const float KA = E / a;
-    const float DA = d / a;
+    const float ra = 1.0f / a;
+    const float KA = E * ra;
+    const float DA = d * ra;
     float dyt;
     if (DA > 0.0f) dyt = -(k * sqrtf(KA / (DA * (DA + k * k))));
     else dyt = k < 0.0f ? INFINITY : (k > 0.0f ? -INFINITY : 0.0f);      /* a strip: the ends are linear in dy */

@@ -286,17 +286,30 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
                 atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx1) * kCtrStride, -1);
                 atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx0) * kCtrStride, -1);
                 atomicAdd(ws.tile_diff + (size_t)(ty1 * gw + tx1) * kCtrStride, 1);
-            } else {
-                // R26: one span of listed tiles per tile row (span.cuh), +1 / -1 at its ends in a row-wise difference grid
-                const SpanCoef sp = span_coefficients(mx2, my2, kk, a2, d2, l2o);
-                for (int ty = ty0; ty < ty1; ++ty) {
-                    int ta, tb;
-                    const int n = span_of_row(sp, tx0, tx1, ty, &ta, &tb);
-                    if (n == 0) continue;
-                    my_pairs += (unsigned int)n;
-                    atomicAdd(ws.tile_diff + (size_t)(ty * gw + ta) * kCtrStride, 1);
-                    atomicAdd(ws.tile_diff + (size_t)(ty * gw + tb + 1) * kCtrStride, -1);
-                }
+            }
+            // (R26, pair rule 2: phase 3 counts the listed tiles)
+        }
+    }
+    // ================= phase 3 (pair rule 2, DESIGN R26): one VISIBLE Gaussian per thread -- the block's visible ones sit
+    // densely at the front of its segment, so all lanes are busy here, unlike in phase 2 where the lanes of culled
+    // candidates idle.  The span of listed tiles of every tile row of the rect (span.cuh: canonical fp32 from the blend
+    // features just written) is counted with +1 / -1 at its ends in a row-wise difference grid.
+    if (ELLIPSE) {
+        __syncthreads();                                   // the records of phase 2 are visible to the whole block
+        const int gw = p.TX + 1;
+        for (unsigned int j = tid; j < n_vis_before; j += kGeoThreads) {
+            const size_t c = (size_t)seg_base + j;
+            const float4 fa = ws.gA[c];
+            const float2 fb = *reinterpret_cast<const float2 *>(ws.gB + c);
+            const ushort4 rc = ws.rect[c];
+            const SpanCoef sp = span_coefficients(fa.x, fa.y, fa.z, fa.w, fb.x, fb.y);
+            for (int ty = rc.y; ty < (int)rc.w; ++ty) {
+                int ta, tb;
+                const int n = span_of_row(sp, (int)rc.x, (int)rc.z, ty, &ta, &tb);
+                if (n == 0) continue;
+                my_pairs += (unsigned int)n;
+                atomicAdd(ws.tile_diff + (size_t)(ty * gw + ta) * kCtrStride, 1);
+                atomicAdd(ws.tile_diff + (size_t)(ty * gw + tb + 1) * kCtrStride, -1);
             }
         }
     }

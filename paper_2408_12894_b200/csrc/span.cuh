@@ -27,8 +27,9 @@ __device__ __forceinline__ SpanCoef span_coefficients(float mx, float my, float 
     c.box = !(a > 0.0f);                                  // not an ellipse after rounding: every tile of the rect
     const float E = __fadd_rn(__fmul_rn(__fadd_rn(l2o, 7.994353436858858f), 1.001953125f), 0.0000152587890625f);
     c.sl = -k;
-    c.KA = __fdiv_rn(E, a);
-    c.DA = __fdiv_rn(d, a);
+    const float ra = __fdiv_rn(1.0f, a);
+    c.KA = __fmul_rn(E, ra);
+    c.DA = __fmul_rn(d, ra);
     if (c.DA > 0.0f) c.dyt = -__fmul_rn(k, __fsqrt_rn(__fdiv_rn(c.KA, __fmul_rn(c.DA, __fadd_rn(c.DA, __fmul_rn(k, k))))));
     else c.dyt = k < 0.0f ? __int_as_float(0x7f800000) : (k > 0.0f ? __int_as_float(0xff800000) : 0.0f);   // a strip
     c.pad = __fadd_rn(__fmul_rn(__fsqrt_rn(c.KA), 0.00390625f), 0.015625f);
