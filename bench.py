@@ -50,6 +50,10 @@ def parse_args():
     ap.add_argument("--pair-rule", type=int, default=2, choices=[1, 2],
                     help="which tiles a Gaussian is listed in: 1 = every tile of its rect (R13), 2 = the tiles the alpha = 1/255 "
                          "ellipse reaches (R26, the library's default); same image, fewer pairs")
+    ap.add_argument("--shard", default="poses", choices=["poses", "rows"],
+                    help="N > 1: poses = replicas, every rank renders its own poses, no collective (weak scaling); rows = "
+                         "every rank renders its strip of tile rows of the SAME pose and one all-gather per frame assembles "
+                         "the image on every rank (strong scaling; meant for --config 4 --size 1920x1080)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--count-scale", type=float, default=1.0, help="shrink the scene (debugging only; reported)")
     return ap.parse_args()
@@ -252,7 +256,8 @@ def workload_config(args, scene, cam, mode, ls, le):
         "selection": (f"materialised G_sel, asynchronous rebuild every {args.subset_period} frames at the current camera "
                       "centre, swapped in when ready (value and stages; e2e uses the per-frame predicate)" if args.subset_period > 0 and ls != le else "Eq. 6 evaluated per frame"),
         "l2": "inputs larger than L2 (scanned level planes + SH exceed 126 MB), no flush between frames",
-        "parallelism": f"replicas x{args.gpus} (poses sharded, no collective)",
+        "parallelism": (f"replicas x{args.gpus} (poses sharded, no collective)" if args.shard == "poses" else
+                        f"tile rows x{args.gpus} (every rank renders a strip of each frame, one all-gather of strips per frame)"),
     }
 
 
@@ -275,7 +280,11 @@ def run_ours(args):
     dist = None
     if world > 1:
         import torch.distributed as dist
+        os.environ.setdefault("NCCL_DEBUG", "INFO")           # the communicator's log (transport, NVLS) goes to stderr
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if args.gpus != world:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE is {world}")
+    rows_mode = args.shard == "rows"                          # (with one rank: the whole image as one strip, no collective)
 
     def barrier():
         torch.cuda.synchronize()
@@ -299,7 +308,12 @@ def run_ours(args):
     out = torch.empty((3, cam0.height, cam0.width), dtype=torch.float32, device=r.device)
     host = torch.empty((3, cam0.height, cam0.width), dtype=torch.float32, pin_memory=True)
     from paper_2408_12894_b200.shard import max_over_ranks, pose_index
-    my_pose = lambda k: cs[pose_index(k, rank, world, len(cs))]       # poses sharded over ranks
+    # poses sharded over ranks (replicas), or every rank on the same pose (tile-row sharding)
+    my_pose = (lambda k: cs[k % len(cs)]) if rows_mode else (lambda k: cs[pose_index(k, rank, world, len(cs))])
+    rsf = None
+    if rows_mode:
+        from paper_2408_12894_b200.shard import RowShardedFrame
+        rsf = RowShardedFrame(cam0.width, cam0.height, rank, world, r.device, dist)
 
     use_subset = args.subset_period > 0 and ls != le
     sub = {"pending": False}
@@ -315,6 +329,8 @@ def run_ours(args):
         r.subset_swap()
 
     def render_frame(k, out_t):
+        if rows_mode:      # this rank's strip, then the all-gather of strips: the image lands in rsf.image on every rank
+            return rsf.render(lambda tyb, tye, o: r.render_rows(my_pose(k), ls, le, args.gamma, tyb, tye, o))
         if not use_subset:
             return r.render(my_pose(k), ls, le, args.gamma, out_t)
         if sub["pending"] and r.subset_ready():
@@ -352,13 +368,19 @@ def run_ours(args):
     # overlaps the kernels of frame k + 1; two pinned buffers alternate), closed by flod_wait_host
     copy_stream = torch.cuda.Stream(device=r.device)
     hosts = [host, torch.empty_like(host).pin_memory()]
+    def e2e_frame(k):
+        if rows_mode:      # strip -> all-gather -> the assembled image to pinned host memory, every frame
+            hosts[k & 1].copy_(render_frame(k, None), non_blocking=True)
+        else:
+            r.render_to_host_async(my_pose(k), ls, le, args.gamma, hosts[k & 1], copy_stream)
+
     for k in range(W):
-        r.render_to_host_async(my_pose(k), ls, le, args.gamma, hosts[k & 1], copy_stream)
+        e2e_frame(k)
     r.wait_host()
     barrier()
     t0 = time.perf_counter()
     for k in range(K):
-        r.render_to_host_async(my_pose(k), ls, le, args.gamma, hosts[k & 1], copy_stream)
+        e2e_frame(k)
     r.wait_host()
     torch.cuda.synchronize()
     ms_e2e = 1e3 * (time.perf_counter() - t0)
@@ -380,6 +402,16 @@ def run_ours(args):
     stage_ms /= n_diag
     for key in agg:
         agg[key] /= n_diag
+    strip = None
+    if rows_mode:          # what this rank's strip costs (rank 0's is reported)
+        sm = np.zeros(len(STAGE_NAMES)); sp = 0
+        for k in range(n_diag):
+            r.render_rows(my_pose(k), ls, le, args.gamma, rsf.tyb, rsf.tye, rsf.piece[:, :rsf.strip_rows()].contiguous())
+            st = r.get_stats()
+            sm += np.array(st["ms_stage"]); sp += st["n_pairs"]
+        strip = {"tile_rows": [rsf.tyb, rsf.tye], "n_pairs": sp / n_diag,
+                 "stage_ns": {n: float(v) * 1e6 / n_diag for n, v in zip(STAGE_NAMES, sm)},
+                 "allgather_bytes_per_frame": rsf.bytes_gathered_per_frame()}
     r.set_options(pkg.FLOD_OPT_COUNT)
     E = B = 0
     for k in range(n_diag):
@@ -436,11 +468,12 @@ def run_ours(args):
                  "peak_source": f"{peak_src} MEASURED_PEAKS.json" if dominant != "blend"
                  else f"{sm_count} SMs x 128 FP32 lanes x 2 x {sm_max_mhz:.0f} MHz (DESIGN §6.3)"})
 
-    fps = world * K / (ms * 1e-3)
-    fps_e2e = world * K / (ms_e2e * 1e-3)
+    frames = K if rows_mode else world * K                # rows: all ranks worked on the same K frames
+    fps = frames / (ms * 1e-3)
+    fps_e2e = frames / (ms_e2e * 1e-3)
     line = {
         "metric": "frames/sec", "value": fps, "unit": "frames/s", "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong" if rows_mode else "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic", "config": workload_config(args, scene, cam0, mode, ls, le),
         "blended_pairs_per_sec": B * fps, "tile_pairs_per_sec": P * fps,
         "e2e": {"value": fps_e2e, "unit": "frames/s", "h2d_bytes_per_step": 88,
@@ -451,6 +484,8 @@ def run_ours(args):
         "peak_device_bytes": int(peak_mem), "scene_bytes": int(scene_bytes), "workspace_bytes": int(ws_bytes),
         "target": {"fps": 300, "met": bool(fps >= 300)},
     }
+    if strip is not None:
+        line["strip_rank0"] = strip
     if not args.no_cpu_baseline and world == 1:
         import oracle
         osc = oracle.OracleScene(scene.levels, scene.sh_degree)
@@ -462,8 +497,22 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` on its own: start the N ranks (one process per GPU, NCCL) the way the driver does."""
+    import socket
+    sock = socket.socket()
+    sock.bind(("127.0.0.1", 0))
+    port = sock.getsockname()[1]
+    sock.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
+        respawn_under_torchrun(args)
     if args.impl == "reference":
         run_reference(args)
     else:

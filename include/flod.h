@@ -35,7 +35,7 @@ extern "C" {
 #define FLOD_API
 #endif
 
-#define FLOD_ABI_VERSION 5
+#define FLOD_ABI_VERSION 6
 #define FLOD_MAX_LEVELS 16
 #define FLOD_TILE 16                 /* tiles are 16x16 pixels */
 #define FLOD_N_STAGES 5              /* 0 geometry (a1-a3), 1 colour (a4) with the tile scan (a5, a8) in one of its blocks,
@@ -165,6 +165,15 @@ FLOD_API int flod_set_pair_rule(flod_ctx *ctx, int rule);
  * cam->R must be a rotation (max |R R^T - I| <= 1e-4), else FLOD_E_INVALID_ARG. */
 FLOD_API int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma,
                 float *out_rgb_dev, void *stream);
+
+/* One horizontal STRIP of a frame: the tile rows [ty_begin, ty_end) (0 <= ty_begin <= ty_end <= ceil(height / 16)), i.e. the
+ * image rows [16 ty_begin, min(height, 16 ty_end)), written to out_strip_dev as [3][rows][width] planar fp32.  The unit of
+ * screen-space sharding over GPUs: each rank culls the Gaussians to its strip (rects are clipped to
+ * it), lists, orders and blends only its own tiles; the strips of all ranks, stacked, are the image flod_render writes,
+ * bit for bit (a tile's list, its order and its arithmetic do not depend on the other tiles).  flod_get_stats then
+ * counts what the strip needed (n_vis, n_pairs of the strip). */
+FLOD_API int flod_render_rows(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma,
+                     int ty_begin, int ty_end, float *out_strip_dev, void *stream);
 
 /* Same, end to end with HOST buffers: renders into an image of the workspace and copies it to out_rgb_host
  * ([3][height][width] fp32, ideally pinned) on `stream`, then waits for the copy.  The frame's overflow word travels

@@ -91,6 +91,7 @@ def load_library():
     L.flod_set_options.argtypes = [vp, C.c_uint]
     L.flod_set_pair_rule.argtypes = [vp, C.c_int]
     L.flod_render.argtypes = [vp, C.POINTER(CameraStruct), LevelMode, C.c_float, vp, vp]
+    L.flod_render_rows.argtypes = [vp, C.POINTER(CameraStruct), LevelMode, C.c_float, C.c_int, C.c_int, vp, vp]
     L.flod_render_to_host.argtypes = [vp, C.POINTER(CameraStruct), LevelMode, C.c_float, vp, vp]
     L.flod_render_to_host_async.argtypes = [vp, C.POINTER(CameraStruct), LevelMode, C.c_float, vp, vp, vp]
     L.flod_wait_host.argtypes = [vp]
@@ -216,6 +217,17 @@ class Renderer:
             out = self._torch.empty((3, cs.height, cs.width), dtype=self._torch.float32, device=self.device)
         self._check(self.lib.flod_render(self._h, C.byref(cs), LevelMode(l_start, l_end), float(gamma),
                                          C.c_void_p(out.data_ptr()), self._stream()))
+        return out
+
+    # ---- flod_render_rows: the strip of tile rows [ty_begin, ty_end) into a [3][rows][W] buffer
+    def render_rows(self, cam, l_start: int, l_end: int, gamma: float, ty_begin: int, ty_end: int, out=None):
+        cs = cam if isinstance(cam, CameraStruct) else camera_struct(cam)
+        rows = max(0, min(cs.height, 16 * ty_end) - 16 * ty_begin)
+        if out is None:
+            out = self._torch.empty((3, rows, cs.width), dtype=self._torch.float32, device=self.device)
+        ptr = out.data_ptr() if out.numel() else self.arena.data_ptr()      # (an empty strip writes nothing; any non-null pointer)
+        self._check(self.lib.flod_render_rows(self._h, C.byref(cs), LevelMode(l_start, l_end), float(gamma),
+                                              int(ty_begin), int(ty_end), C.c_void_p(ptr), self._stream()))
         return out
 
     # ---- flod_render_to_host: host buffer in, host buffer out

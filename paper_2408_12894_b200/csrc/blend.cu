@@ -62,7 +62,7 @@ constexpr int kBlendMinBlocks = 8;                   // 64 registers per thread
 template <bool COUNT>
 __global__ void __launch_bounds__(kBlendThreads, kBlendMinBlocks)
 k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, int n_tiles,
-        float bg0, float bg1, float bg2)
+        float bg0, float bg1, float bg2, int tile0, int out_row0, int out_rows)
 {
     // staging, 36 bytes per Gaussian of the batch: A = (mu'x, mu'y, k, a2), B = (d2, log2 o, r, g), c = b
     __shared__ float4 s_A[2][kBatch], s_B[2][kBatch];           // double-buffered
@@ -71,7 +71,7 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
     __shared__ float4 s_buf[kBlendWarps][kWarpBuf * 3];
     __shared__ unsigned short s_idx[kBlendWarps][kWarpBuf];    // batch index of the survivor (counting variant only)
 
-    const int tile = blockIdx.x;
+    const int tile = tile0 + blockIdx.x;                // the grid covers the frame's strip of tile rows
     if (tile >= n_tiles || ws.hdr->overflow) return;   // an overflowed frame is undefined: its lists were not sorted
     const int tx = tile % TX, ty = tile / TX;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -215,13 +215,13 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
     }
     const bool done0 = T.x < 1e-4f, done1 = T.y < 1e-4f;
     const float T0 = T.x, T1 = T.y, r0 = cr.x, r1 = cr.y, g0 = cg.x, g1 = cg.y, b0 = cb2.x, b1 = cb2.y;
-    const size_t plane = (size_t)W * H;
+    const size_t plane = (size_t)W * out_rows;          // out holds image rows [out_row0, out_row0 + out_rows) of every plane
     if (in0) {
-        const size_t o = (size_t)py0 * W + px;
+        const size_t o = (size_t)(py0 - out_row0) * W + px;
         out[o] = fmaf(T0, bg0, r0); out[plane + o] = fmaf(T0, bg1, g0); out[2 * plane + o] = fmaf(T0, bg2, b0);
     }
     if (in1) {
-        const size_t o = (size_t)py1 * W + px;
+        const size_t o = (size_t)(py1 - out_row0) * W + px;
         out[o] = fmaf(T1, bg0, r1); out[plane + o] = fmaf(T1, bg1, g1); out[2 * plane + o] = fmaf(T1, bg2, b1);
     }
     if (COUNT) {
@@ -242,13 +242,14 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
 
 int launch_blend(const Context &c, const FrameParams &p, float *out_rgb, cudaStream_t s)
 {
-    const int n_tiles = p.TX * p.TY;
+    const int tile0 = p.ty_begin * p.TX, n_tiles = p.ty_end * p.TX, grid = n_tiles - tile0;
+    if (grid <= 0) return 0;
     if (c.flags & FLOD_OPT_COUNT)
-        k_blend<true><<<n_tiles, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
-                                                        p.bg[0], p.bg[1], p.bg[2]);
+        k_blend<true><<<grid, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
+                                                     p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows);
     else
-        k_blend<false><<<n_tiles, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
-                                                         p.bg[0], p.bg[1], p.bg[2]);
+        k_blend<false><<<grid, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
+                                                      p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows);
     return 1;
 }
 

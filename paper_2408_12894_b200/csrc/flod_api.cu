@@ -402,6 +402,7 @@ void camera_params(FrameParams &p, const flod_camera *cam)
         p.pre_c1 = (float)(fm * fm * (1.0 + lm * lm) * 1.0001);
     }
     p.n_tiles = p.TX * p.TY;
+    p.ty_begin = 0; p.ty_end = p.TY; p.out_row0 = 0; p.out_rows = p.H;      // the whole image unless flod_render_rows says otherwise
 }
 
 // Eq. 7 thresholds of the level positions i0..i1 (squared, fp64 -> fp32 once): lo2[k], hi2[k], level_end[k]
@@ -455,7 +456,13 @@ int enqueue_frame(flod_ctx *ctx, const SceneDev &sc, FrameParams &p, float *out_
 
 extern "C" {
 
-int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, float *out_rgb_dev, void *stream)
+}  // extern "C"
+
+namespace {
+
+// flod_render / flod_render_rows: ty_end < 0 = the whole image into a [3][H][W] buffer
+int render_impl(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, int ty_begin, int ty_end,
+                float *out_rgb_dev, void *stream)
 {
     if (!ctx) return FLOD_E_INVALID_ARG;
     if (int rc = check_frame_args(ctx, cam, out_rgb_dev)) return rc;
@@ -471,7 +478,31 @@ int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, flo
     p.first_gid = ctx->level_off[i0];
     p.n_scan = (int)(ctx->level_off[i1 + 1] - ctx->level_off[i0]);
     band_params(ctx, i0, i1, cam->fx, gamma, p.level_end, p.lo2, p.hi2);
+    if (ty_end >= 0) {
+        if (ty_begin < 0 || ty_begin > ty_end || ty_end > p.TY)
+            return fail(ctx, FLOD_E_INVALID_ARG, "render_rows: need 0 <= ty_begin <= ty_end <= ceil(height / 16)");
+        p.ty_begin = ty_begin; p.ty_end = ty_end;
+        p.out_row0 = ty_begin * kTile;
+        p.out_rows = std::min(p.H, ty_end * kTile) - p.out_row0;
+        if (p.out_rows < 0) p.out_rows = 0;
+    }
     return enqueue_frame(ctx, ctx->scene, p, out_rgb_dev, (cudaStream_t)stream);
+}
+
+}  // namespace
+
+extern "C" {
+
+int flod_render(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, float *out_rgb_dev, void *stream)
+{
+    return render_impl(ctx, cam, mode, gamma, 0, -1, out_rgb_dev, stream);
+}
+
+int flod_render_rows(flod_ctx *ctx, const flod_camera *cam, flod_level_mode mode, float gamma, int ty_begin, int ty_end,
+                     float *out_strip_dev, void *stream)
+{
+    if (ty_end < 0) return ctx ? fail(ctx, FLOD_E_INVALID_ARG, "render_rows: ty_end < 0") : FLOD_E_INVALID_ARG;
+    return render_impl(ctx, cam, mode, gamma, ty_begin, ty_end, out_strip_dev, stream);
 }
 
 }  // extern "C"

@@ -113,6 +113,9 @@ struct FrameParams {
     int n_pre_blocks;                     // blocks of k_geometry
     int n_tiles;                          // TX * TY
     int pair_rule;                        // FLOD_PAIR_RULE_BOX / FLOD_PAIR_RULE_ELLIPSE
+    int ty_begin, ty_end;                 // the strip of tile rows this frame renders ([0, TY) = the whole image): rects are
+                                          // clipped to it, tiles outside it get no pairs and are not blended
+    int out_row0, out_rows;               // out_rgb holds image rows [out_row0, out_row0 + out_rows) of every colour plane
 };
 
 struct Context {

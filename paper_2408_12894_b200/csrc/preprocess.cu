@@ -140,7 +140,7 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
             const float ax = fmaf(p.fx * px, rz, p.cx), ay = fmaf(p.fy * py, rz, p.cy);
             const float bnd = sqrtf(fmaf(rho2[k] * p.pre_c1, rz * rz, 3.33f)) * 1.01f + 1.0f + 1e-5f * (fabsf(ax) + fabsf(ay));
             const bool off = ax + bnd < 0.0f || ax - bnd > (float)(p.TX * kTile) ||
-                             ay + bnd < 0.0f || ay - bnd > (float)(p.TY * kTile);
+                             ay + bnd < (float)(p.ty_begin * kTile) || ay - bnd > (float)(p.ty_end * kTile);
             if (!off) m_cand |= 1u << k;                       // (a NaN or infinite bound keeps the Gaussian)
         }
     }
@@ -186,7 +186,7 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
         const unsigned int s = s0 + tid;
         bool vis = false;
         float mx2 = 0.f, my2 = 0.f, z = 0.f, cA = 0.f, cB = 0.f, cC = 0.f, l2o = 0.f, wxk = 0.f, wyk = 0.f, wzk = 0.f, kap = 0.f;
-        int tx0 = 0, tx1 = 0, ty0 = 0, ty1 = 0;
+        int tx0 = 0, tx1 = 0, ty0 = 0, ty1 = 0, rty0 = 0, rty1 = 0;
         long long g = 0;
         if (s < n_cand) {
             g = gb + S.cand[s];
@@ -235,7 +235,9 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
                 const float y0 = fminf(fmaxf(floorf(fmul(fsub(my2, hy), 0.0625f)), 0.0f), fTY);
                 const float y1 = fminf(fmaxf(fadd(floorf(fmul(fadd(my2, hy), 0.0625f)), 1.0f), 0.0f), fTY);
                 tx0 = (int)x0; tx1 = (int)x1; ty0 = (int)y0; ty1 = (int)y1;
-                vis = (tx1 - tx0) * (ty1 - ty0) > 0;
+                rty0 = ty0; rty1 = ty1;                    // the canonical rect (debug record)
+                ty0 = max(ty0, p.ty_begin); ty1 = min(ty1, p.ty_end);      // ... clipped to the frame's strip of tile rows
+                vis = (tx1 - tx0) > 0 && (ty1 - ty0) > 0;
             }
         }
         // ---- position of the visible ones: ballot inside the warp, warp totals through shared memory
@@ -274,7 +276,7 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
                 d.gid = g_scene; d.mu2d[0] = mx2; d.mu2d[1] = my2; d.depth = z;
                 d.conic[0] = cA; d.conic[1] = cB; d.conic[2] = cC; d.opacity = __ldg(sc.opacity + g);
                 d.rgb[0] = 0.0f; d.rgb[1] = 0.0f; d.rgb[2] = 0.0f;                                // by k_colour
-                d.rect[0] = tx0; d.rect[1] = ty0; d.rect[2] = tx1; d.rect[3] = ty1;
+                d.rect[0] = tx0; d.rect[1] = rty0; d.rect[2] = tx1; d.rect[3] = rty1;
                 ws.dbg[c] = d;
             }
             // a5, first half: the difference grid of the per-tile pair counts

@@ -201,12 +201,12 @@ __device__ void finish_sort(const u64 *buf, unsigned int n, const BinMap &m, u64
 }
 
 __global__ void __launch_bounds__(kSortThreads, 4)      // 4 CTAs per SM is what the 49 KB of shared memory allow
-k_tile_sort(const WorkspaceDev ws, int n_tiles)
+k_tile_sort(const WorkspaceDev ws, int tile0, int n_tiles)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     SortSmem &S = *reinterpret_cast<SortSmem *>(smem_raw);
 
-    const int tile = blockIdx.x;
+    const int tile = tile0 + blockIdx.x;               // the grid covers the frame's strip of tile rows
     if (tile >= n_tiles) return;
     const int tid = threadIdx.x;
     const uint2 rg = ws.ranges[tile];
@@ -253,7 +253,9 @@ int init_tile_sort()
 int launch_tile_sort(const Context &c, const FrameParams &p, cudaStream_t s)
 {
     if (p.n_pre_blocks <= 0) return 0;
-    k_tile_sort<<<p.n_tiles, kSortThreads, sizeof(SortSmem), s>>>(c.ws, p.n_tiles);
+    const int tile0 = p.ty_begin * p.TX, n_tiles = p.ty_end * p.TX;
+    if (n_tiles <= tile0) return 0;
+    k_tile_sort<<<n_tiles - tile0, kSortThreads, sizeof(SortSmem), s>>>(c.ws, tile0, n_tiles);
     return 1;
 }
 

@@ -121,3 +121,15 @@ def test_config4_materialised_subset_on_the_walk(config4):
         finally:
             r.set_selection_reference(None)
         assert np.array_equal(img, fused)
+
+
+def test_config4_1080p_row_sharded_over_four_ranks(config4):
+    """Screen-space sharding on the config it is meant for: 1920x1080, selective {3,4,5}: the strips four
+    ranks would render, stacked the way the all-gather stacks them, are the single-GPU image bit for bit."""
+    from test_gpu_parity import _assemble_strips
+    scene, osc, r = config4
+    cam = fs.make_poses(4, 1920, 1080)[149]
+    full = r.render(cam, 3, 5, 1.0).cpu().numpy()
+    st = r.get_stats()
+    img, pairs = _assemble_strips(r, cam, 3, 5, 1.0, 4)
+    assert np.array_equal(img, full) and pairs == st["n_pairs"]

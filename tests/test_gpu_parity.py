@@ -552,3 +552,57 @@ def test_random_scenes_every_kernel_path(pkg, seed):
     assert np.array_equal(a, b)
     check_image(a, osc.frame(cam, 1, L, gamma, ref_pos=ref, pair_rule=r.pair_rule))
     r.close()
+
+
+# ------------------------------------------------------------------------------------ tile-row strips
+
+def _assemble_strips(r, cam, ls, le, gamma, world):
+    """What `world` ranks would produce (paper_2408_12894_b200.shard.RowShardedFrame without a process group: the strips
+    are rendered one after the other on this GPU and stacked the way the all-gather stacks them)."""
+    import torch
+    from paper_2408_12894_b200.shard import RowShardedFrame
+    frames = [RowShardedFrame(cam.width, cam.height, rank, world, r.device) for rank in range(world)]
+    pairs = 0
+    for fr in frames:
+        n = fr.strip_rows()
+        if n:
+            fr.piece[:, :n].copy_(r.render_rows(cam, ls, le, gamma, fr.tyb, fr.tye))
+            pairs += r.get_stats()["n_pairs"]
+    gathered = torch.stack([fr.piece for fr in frames])
+    img = gathered.permute(1, 0, 2, 3).reshape(3, world * frames[0].rows_px, cam.width)[:, :cam.height]
+    return img.cpu().numpy(), pairs
+
+
+@pytest.mark.parametrize("rule", [1, 2])
+def test_tile_row_strips_stack_to_the_full_frame_bit_for_bit(pkg, config0, rule):
+    """flod_render_rows: the strips of 2, 3 and 5 ranks, stacked, are the image flod_render writes, bit for bit, and
+    together they hold exactly the frame's pairs (a rect is clipped to the strip, never listed twice)."""
+    sc, cam, osc, r = config0
+    r.set_pair_rule(rule)
+    try:
+        for (ls, le) in ((2, 2), (1, 2)):
+            full = r.render(cam, ls, le, 1.0).cpu().numpy()
+            n_pairs = r.get_stats()["n_pairs"]
+            for world in (2, 3, 5):
+                img, pairs = _assemble_strips(r, cam, ls, le, 1.0, world)
+                assert np.array_equal(img, full) and pairs == n_pairs
+        # a strip against the oracle directly: the oracle's frame of a camera cropped to those rows is the same strip
+        strip = r.render_rows(cam, 1, 2, 1.0, 2, 5).cpu().numpy()
+        assert np.array_equal(strip, full[:, 32:80])
+        with pytest.raises(pkg.FlodError):
+            r.render_rows(cam, 1, 2, 1.0, 3, 9)              # 128 px = 8 tile rows
+        assert r.render_rows(cam, 1, 2, 1.0, 4, 4).shape == (3, 0, cam.width)
+    finally:
+        r.set_pair_rule(pkg.PAIR_RULE_ELLIPSE)
+
+
+def test_tile_row_strips_on_a_ragged_image_with_large_footprints(pkg):
+    rng = np.random.default_rng(303)
+    lv = _rand_levels(rng, (3000, 5000), (0.05, 0.0), sh_degree=1, logs=(-2.5, 0.0))
+    cam = camera(width=211, height=157, f=140.0, bg=(0.3, 0.2, 0.1))
+    r = make_renderer(pkg, lv, 1, 211, 157, max_pairs=1 << 23)
+    full = r.render(cam, 1, 2, 1.5).cpu().numpy()
+    for world in (2, 4, 7, 16):                                  # 10 tile rows: the last ranks of 16 own nothing
+        img, _ = _assemble_strips(r, cam, 1, 2, 1.5, world)
+        assert np.array_equal(img, full)
+    r.close()
