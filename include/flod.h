@@ -35,7 +35,7 @@ extern "C" {
 #define FLOD_API
 #endif
 
-#define FLOD_ABI_VERSION 6
+#define FLOD_ABI_VERSION 7
 #define FLOD_MAX_LEVELS 16
 #define FLOD_TILE 16                 /* tiles are 16x16 pixels */
 #define FLOD_N_STAGES 5              /* 0 geometry (a1-a3), 1 colour (a4) with the tile scan (a5, a8) in one of its blocks,
@@ -234,6 +234,21 @@ FLOD_API int flod_debug_copy(flod_ctx *ctx, int what, void *host_dst, size_t byt
 
 /* Number of kernel launches flod_render enqueues per frame with the current options. */
 FLOD_API int flod_launches_per_frame(const flod_ctx *ctx);
+
+/* ---- Training-side kernels.  They need no context: all arrays are caller-owned device memory. ---- */
+
+/* Overlap pruning (§4.3; Alg. 1 "OverlapPruning()"): remove_dev[i] = 1 iff the average distance from
+ * Gaussian i to its three nearest neighbours (by mean, Euclidean; k = n - 1 when n <= 3, nothing when n <= 1) is below
+ * d_OP = s_min / 2, all decided on the set as given (simultaneous rule).  mean_dev is [n][3] fp32.
+ * mean_dist_dev (may be NULL) receives that average where it is decided exactly -- whenever the third neighbour lies
+ * within 3 d_OP -- and +inf otherwise (then it is >= d_OP, which is all the rule needs).  bbox_lo: any point with
+ * bbox_lo <= mean componentwise (the grid's origin; the minimum of the means, or a bound of the scene).
+ * Arithmetic (both sides of the parity test): d^2 = (dx dx + dy dy) + dz dz, mean = ((sqrt d1 + sqrt d2) + sqrt d3) / 3
+ * with d1 <= d2 <= d3, compared with 0.5f * s_min, every operation one IEEE binary32 operation.
+ * s_min must be > 0 (the rule is for levels below L_max).  Asynchronous on `stream`. */
+FLOD_API size_t flod_overlap_prune_workspace_bytes(int64_t n);
+FLOD_API int flod_overlap_prune(const float *mean_dev, int64_t n, float s_min, const float bbox_lo[3], unsigned char *remove_dev,
+                       float *mean_dist_dev, void *workspace_dev, size_t workspace_bytes, void *stream);
 
 FLOD_API const char *flod_last_error(const flod_ctx *ctx);
 FLOD_API int flod_abi_version(void);

@@ -105,6 +105,9 @@ def load_library():
     L.flod_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.flod_debug_copy.argtypes = [vp, C.c_int, vp, sz]
     L.flod_launches_per_frame.argtypes = [vp]
+    L.flod_overlap_prune_workspace_bytes.restype = sz
+    L.flod_overlap_prune_workspace_bytes.argtypes = [i64]
+    L.flod_overlap_prune.argtypes = [vp, i64, C.c_float, C.POINTER(C.c_float), vp, vp, vp, sz, vp]
     L.flod_last_error.restype = C.c_char_p
     L.flod_last_error.argtypes = [vp]
     L.flod_abi_version.restype = C.c_int
@@ -316,3 +319,29 @@ class Renderer:
 
     def debug_activated(self):
         return self._dbg(FLOD_DBG_ACTIVATED, np.zeros((max(self.n_total, 1), 8), np.float32))[:self.n_total]
+
+
+# ---- flod_overlap_prune (training-side): no context, caller-owned device arrays
+def overlap_prune(mean, s_min: float, with_distances: bool = True):
+    """mean: CUDA float32 tensor [n, 3].  Returns (remove uint8 [n], mean 3-NN distance float32 [n] or None)."""
+    import torch
+    if not (mean.is_cuda and mean.dtype == torch.float32 and mean.dim() == 2 and mean.shape[1] == 3):
+        raise ValueError("overlap_prune wants a CUDA float32 tensor of shape [n, 3]")
+    lib = load_library()
+    mean = mean.contiguous()
+    n = mean.shape[0]
+    remove = torch.zeros(n, dtype=torch.uint8, device=mean.device)
+    dist = torch.full((n,), float("inf"), dtype=torch.float32, device=mean.device) if with_distances else None
+    if n == 0:
+        return remove, dist
+    lo = mean.min(dim=0).values.cpu().numpy().astype(np.float32)
+    ws = torch.empty(lib.flod_overlap_prune_workspace_bytes(n), dtype=torch.uint8, device=mean.device)
+    with torch.cuda.device(mean.device):
+        rc = lib.flod_overlap_prune(C.c_void_p(mean.data_ptr()), n, float(s_min), (C.c_float * 3)(*[float(v) for v in lo]),
+                                    C.c_void_p(remove.data_ptr()), C.c_void_p(dist.data_ptr()) if dist is not None else None,
+                                    C.c_void_p(ws.data_ptr()), ws.numel(),
+                                    C.c_void_p(torch.cuda.current_stream(mean.device).cuda_stream))
+        torch.cuda.current_stream(mean.device).synchronize()      # the workspace is freed on return
+    if rc:
+        raise FlodError(rc, "flod_overlap_prune rejected its arguments")
+    return remove, dist
