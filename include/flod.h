@@ -35,7 +35,7 @@ extern "C" {
 #define FLOD_API
 #endif
 
-#define FLOD_ABI_VERSION 7
+#define FLOD_ABI_VERSION 8
 #define FLOD_MAX_LEVELS 16
 #define FLOD_TILE 16                 /* tiles are 16x16 pixels */
 #define FLOD_N_STAGES 5              /* 0 geometry (a1-a3), 1 colour (a4) with the tile scan (a5, a8) in one of its blocks,
@@ -236,6 +236,21 @@ FLOD_API int flod_debug_copy(flod_ctx *ctx, int what, void *host_dst, size_t byt
 FLOD_API int flod_launches_per_frame(const flod_ctx *ctx);
 
 /* ---- Training-side kernels.  They need no context: all arrays are caller-owned device memory. ---- */
+
+/* Backward pass of the rasterizer (Alg. 1 "Adam(grad L)"): the gradient of <dL_dimage, image> with
+ * respect to every learnable parameter of the LAST frame rendered by flod_render on this context (its lists are still in
+ * the workspace; cam must be that frame's camera, else FLOD_E_INVALID_ARG).  All arrays are device memory indexed by gid
+ * (levels concatenated in upload order) over the whole scene; the call zeroes them and the Gaussians the frame drew add
+ * their gradients: d_mean [n][3], d_log_scale [n][3] (of the stored log of the effective scale; d s / d s_opt =
+ * exp(s_opt) of Eq. 4 is the caller's chain), d_quat [n][4] (of the un-normalised quaternion), d_opacity_logit [n],
+ * d_sh [n][K][3].  The discrete decisions of the forward pass (selection, culls, order, the 1/255 skip, the stop at
+ * T < 1e-4) are constants; min(0.99, .) and max(0, .) have their mathematical derivative.  fp32, sums in the order the
+ * atomics are served (not bit-reproducible); asynchronous on `stream`.  workspace_dev: flod_backward_workspace_bytes,
+ * 256-byte aligned, caller-owned. */
+typedef struct { float *d_mean, *d_log_scale, *d_quat, *d_opacity_logit, *d_sh; } flod_grads;
+FLOD_API size_t flod_backward_workspace_bytes(const flod_ctx *ctx);
+FLOD_API int flod_render_backward(flod_ctx *ctx, const flod_camera *cam, const float *dL_dimage_dev, const flod_grads *grads,
+                         void *workspace_dev, size_t workspace_bytes, void *stream);
 
 /* Overlap pruning (§4.3; Alg. 1 "OverlapPruning()"): remove_dev[i] = 1 iff the average distance from
  * Gaussian i to its three nearest neighbours (by mean, Euclidean; k = n - 1 when n <= 3, nothing when n <= 1) is below

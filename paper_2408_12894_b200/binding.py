@@ -43,6 +43,11 @@ class CameraStruct(C.Structure):
                 ("width", C.c_int), ("height", C.c_int), ("z_near", C.c_float), ("bg", C.c_float * 3)]
 
 
+class Grads(C.Structure):
+    _fields_ = [("d_mean", C.c_void_p), ("d_log_scale", C.c_void_p), ("d_quat", C.c_void_p),
+                ("d_opacity_logit", C.c_void_p), ("d_sh", C.c_void_p)]
+
+
 class LevelMode(C.Structure):
     _fields_ = [("l_start", C.c_int), ("l_end", C.c_int)]
 
@@ -105,6 +110,9 @@ def load_library():
     L.flod_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.flod_debug_copy.argtypes = [vp, C.c_int, vp, sz]
     L.flod_launches_per_frame.argtypes = [vp]
+    L.flod_backward_workspace_bytes.restype = sz
+    L.flod_backward_workspace_bytes.argtypes = [vp]
+    L.flod_render_backward.argtypes = [vp, C.POINTER(CameraStruct), vp, C.POINTER(Grads), vp, sz, vp]
     L.flod_overlap_prune_workspace_bytes.restype = sz
     L.flod_overlap_prune_workspace_bytes.argtypes = [i64]
     L.flod_overlap_prune.argtypes = [vp, i64, C.c_float, C.POINTER(C.c_float), vp, vp, vp, sz, vp]
@@ -285,6 +293,23 @@ class Renderer:
             out = self._torch.empty((3, cs.height, cs.width), dtype=self._torch.float32, device=self.device)
         self._check(self.lib.flod_render_subset(self._h, C.byref(cs), C.c_void_p(out.data_ptr()), self._stream()))
         return out
+
+    # ---- flod_render_backward: gradients of <upstream, image> of the last frame rendered by render()
+    def render_backward(self, cam, upstream, sh_degree: int):
+        """upstream: CUDA float32 [3, H, W].  Returns a dict of CUDA float32 tensors indexed by gid."""
+        t = self._torch
+        cs = cam if isinstance(cam, CameraStruct) else camera_struct(cam)
+        n, K = max(self.n_total, 1), (sh_degree + 1) ** 2
+        z = lambda *shape: t.empty(shape, dtype=t.float32, device=self.device)
+        out = {"mean": z(n, 3), "log_scale": z(n, 3), "quat": z(n, 4), "logit": z(n), "sh": z(n, K, 3)}
+        g = Grads(*[C.c_void_p(out[k].data_ptr()) for k in ("mean", "log_scale", "quat", "logit", "sh")])
+        nbytes = self.lib.flod_backward_workspace_bytes(self._h)
+        if getattr(self, "bwd_workspace", None) is None or self.bwd_workspace.numel() < nbytes:
+            self.bwd_workspace = t.empty(nbytes, dtype=t.uint8, device=self.device)
+        upstream = upstream.contiguous()
+        self._check(self.lib.flod_render_backward(self._h, C.byref(cs), C.c_void_p(upstream.data_ptr()), C.byref(g),
+                                                  C.c_void_p(self.bwd_workspace.data_ptr()), nbytes, self._stream()))
+        return {k: v[:self.n_total] for k, v in out.items()}
 
     def launches_per_frame(self) -> int:
         return self.lib.flod_launches_per_frame(self._h)

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libflod.so")
-SOURCES = ["flod_api.cu", "preprocess.cu", "binning.cu", "tile_sort.cu", "blend.cu", "subset.cu", "knn.cu"]
+SOURCES = ["flod_api.cu", "preprocess.cu", "binning.cu", "tile_sort.cu", "blend.cu", "subset.cu", "knn.cu", "backward.cu"]
 import glob
 HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h")) +
                  glob.glob(os.path.join(HERE, "..", "include", "*.h")))

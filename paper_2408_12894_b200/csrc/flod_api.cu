@@ -41,7 +41,7 @@ const char *overflow_text(unsigned int bits)
 
 int sh_stride_for(int deg) { int k = (deg + 1) * (deg + 1); return (3 * k + 3) / 4 * 4; }
 
-constexpr int kScenePlanes = 3 + 6 + 4;   // mean xyz, cov x6, opacity, kappa, log2 o, rho2
+constexpr int kScenePlanes = 3 + 6 + 4 + 8;   // mean xyz, cov x6, opacity, kappa, log2 o, rho2; raw log_scale xyz, quat wxyz, logit
 
 size_t scene_bytes_for(int64_t n, int sh_degree)
 {
@@ -261,6 +261,9 @@ int flod_upload_levels(flod_ctx *ctx, int n_levels, const flod_level_desc *level
                 activate_one(d.log_scale + 3 * i, d.quat + 4 * i, d.opacity_logit[i], cov, &o, &kap, &l2o, &rho2);
                 for (int k = 0; k < 6; ++k) pl[3 + k][g] = cov[k];
                 pl[9][g] = o; pl[10][g] = kap; pl[11][g] = l2o; pl[12][g] = rho2;
+                for (int k = 0; k < 3; ++k) pl[13 + k][g] = d.log_scale[3 * i + k];
+                for (int k = 0; k < 4; ++k) pl[16 + k][g] = d.quat[4 * i + k];
+                pl[20][g] = d.opacity_logit[i];
                 float *dst = shp + (size_t)g * stride;
                 const float *src = d.sh + (size_t)i * 3 * K;
                 if (sh_degree == 3) {
@@ -290,6 +293,7 @@ int flod_upload_levels(flod_ctx *ctx, int n_levels, const flod_level_desc *level
     ctx->scene.mx = P(0); ctx->scene.my = P(1); ctx->scene.mz = P(2);
     for (int k = 0; k < 6; ++k) ctx->scene.cov[k] = P(3 + k);
     ctx->scene.opacity = P(9); ctx->scene.kappa = P(10); ctx->scene.l2o = P(11); ctx->scene.rho2 = P(12);
+    for (int k = 0; k < 8; ++k) ctx->scene.raw[k] = P(13 + k);
     ctx->scene.sh = P(kScenePlanes);
     ctx->scene.sh_stride = stride; ctx->scene.sh_degree = sh_degree;
     ctx->arena = scene_arena_dev;
@@ -447,6 +451,7 @@ int enqueue_frame(flod_ctx *ctx, const SceneDev &sc, FrameParams &p, float *out_
     CUDA_TRY(ctx, cudaGetLastError());
     ctx->ev_valid = prof;
     ctx->last_stream = s; ctx->rendered = true;
+    ctx->last_params = p; ctx->last_full_scene = sc.src_gid == nullptr;
     ctx->last_n_scan = n_scan; ctx->last_n_segs = p.n_pre_blocks;
     ctx->last_w = p.W; ctx->last_h = p.H; ctx->last_tx = p.TX; ctx->last_ty = p.TY; ctx->last_first_gid = p.first_gid;
     return FLOD_OK;
@@ -708,6 +713,47 @@ int flod_render_subset(flod_ctx *ctx, const flod_camera *cam, float *out_rgb_dev
     if (rc != FLOD_OK) return rc;
     CUDA_TRY(ctx, cudaEventRecord(ctx->ev_sub_read[f], s));
     ctx->sub_read_pending[f] = true;
+    return FLOD_OK;
+}
+
+size_t flod_backward_workspace_bytes(const flod_ctx *ctx)
+{
+    if (!ctx || !ctx->uploaded) return 0;
+    return align_up(((size_t)std::max<int64_t>(ctx->n_total, 1) + 2 * kGeoBlock) * 9 * sizeof(float));
+}
+
+int flod_render_backward(flod_ctx *ctx, const flod_camera *cam, const float *dL_dimage_dev, const flod_grads *grads,
+                         void *workspace_dev, size_t workspace_bytes, void *stream)
+{
+    if (!ctx) return FLOD_E_INVALID_ARG;
+    if (!cam || !dL_dimage_dev || !grads || !workspace_dev) return fail(ctx, FLOD_E_INVALID_ARG, "render_backward: null pointer");
+    if (!grads->d_mean || !grads->d_log_scale || !grads->d_quat || !grads->d_opacity_logit || !grads->d_sh)
+        return fail(ctx, FLOD_E_INVALID_ARG, "render_backward: null gradient array");
+    if (!ctx->rendered || !ctx->last_full_scene)
+        return fail(ctx, FLOD_E_INVALID_ARG, "render_backward: the last frame must come from flod_render");
+    if ((uintptr_t)workspace_dev % 256 || workspace_bytes < flod_backward_workspace_bytes(ctx))
+        return fail(ctx, FLOD_E_ARENA_TOO_SMALL, "render_backward: workspace unaligned or too small");
+    const FrameParams &p = ctx->last_params;
+    // the contract: the inputs of the forward pass that left its lists in the workspace
+    FrameParams q{};
+    camera_params(q, cam);
+    if (memcmp(q.R, p.R, sizeof(q.R)) || memcmp(q.t, p.t, sizeof(q.t)) || memcmp(q.bg, p.bg, sizeof(q.bg)) || q.fx != p.fx ||
+        q.fy != p.fy || q.cx != p.cx || q.cy != p.cy || q.W != p.W || q.H != p.H || q.z_near != p.z_near)
+        return fail(ctx, FLOD_E_INVALID_ARG, "render_backward: the camera is not the one of the last flod_render");
+    if (p.ty_begin != 0 || p.ty_end != p.TY)
+        return fail(ctx, FLOD_E_INVALID_ARG, "render_backward: the last frame was a strip (flod_render_rows)");
+    cudaStream_t s = (cudaStream_t)stream;
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    // gradients are indexed by gid over the whole scene: zero, then the drawn Gaussians add theirs
+    const size_t n = (size_t)std::max<int64_t>(ctx->n_total, 1), K = (size_t)(ctx->sh_degree + 1) * (ctx->sh_degree + 1);
+    CUDA_TRY(ctx, cudaMemsetAsync(grads->d_mean, 0, n * 3 * sizeof(float), s));
+    CUDA_TRY(ctx, cudaMemsetAsync(grads->d_log_scale, 0, n * 3 * sizeof(float), s));
+    CUDA_TRY(ctx, cudaMemsetAsync(grads->d_quat, 0, n * 4 * sizeof(float), s));
+    CUDA_TRY(ctx, cudaMemsetAsync(grads->d_opacity_logit, 0, n * sizeof(float), s));
+    CUDA_TRY(ctx, cudaMemsetAsync(grads->d_sh, 0, n * K * 3 * sizeof(float), s));
+    CUDA_TRY(ctx, cudaMemsetAsync(workspace_dev, 0, flod_backward_workspace_bytes(ctx), s));
+    launch_backward(*ctx, p, dL_dimage_dev, (float *)workspace_dev, *grads, s);
+    CUDA_TRY(ctx, cudaGetLastError());
     return FLOD_OK;
 }
 

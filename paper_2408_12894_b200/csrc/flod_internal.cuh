@@ -30,6 +30,7 @@ struct SceneDev {
     const float *kappa;                   // 2 ln(255 o); -1 when dead
     const float *l2o;                     // log2(o)
     const float *rho2;                    // kappa * largest eigenvalue of Sigma, rounded up (squared bounding radius); -1 when dead
+    const float *raw[8];                  // the uploaded log_scale xyz, quat wxyz, opacity logit (read by the backward pass only)
     const float *sh;                      // [n][sh_stride] floats, row = K*3 coefficients padded to a multiple of 4
     int sh_stride;
     int sh_degree;
@@ -142,6 +143,8 @@ struct Context {
     float ref[3] = {0, 0, 0};
     cudaStream_t last_stream = nullptr;
     bool rendered = false;
+    FrameParams last_params{};            // of the last frame enqueued by flod_render (what flod_render_backward differentiates)
+    bool last_full_scene = false;         // ... and whether it scanned the scene arena itself (not a snapshot)
     int last_w = 0, last_h = 0, last_tx = 0, last_ty = 0;
     int64_t last_first_gid = 0;
     int64_t last_n_scan = 0;
@@ -176,5 +179,7 @@ int init_duplicate();                                                           
 int init_tile_sort();                                                            // once per device: shared-memory opt-in
 int launch_tile_sort(const Context &c, const FrameParams &p, cudaStream_t s);   // a7
 int launch_blend(const Context &c, const FrameParams &p, float *out_rgb, cudaStream_t s);   // a9
+// backward pass of a9 and of a2-a4 (backward.cu); g9 = [positions][9] screen-space gradients (workspace of the backward pass)
+int launch_backward(const Context &c, const FrameParams &p, const float *dL_dimage, float *g9, const flod_grads &out, cudaStream_t s);
 
 }  // namespace flod

@@ -81,3 +81,105 @@ def test_zero_upstream_and_dead_gaussians():
     fr = OracleScene(lv, 0).frame(cam, 1, 1, 1.0)
     g2, _ = ob.backward(lv, 0, cam, fr, np.ones((3, 16, 16)))
     assert np.abs(g2["sh"][3]).max() < 1e-7 and np.abs(g2["mean"][3]).max() == 0.0
+
+
+# ------------------------------------------------------------------------------------ the CUDA kernels (GPU)
+
+def _gpu_vs_oracle(lv, deg, cam, ls, le, gamma, up, tol=1e-4):
+    from paper_2408_12894_b200 import build
+    build.build()
+    import paper_2408_12894_b200 as pkg
+    r = pkg.Renderer(0)
+    r.upload_levels(lv, deg)
+    r.set_workspace(cam.width, cam.height, 1 << 22)
+    img = r.render(cam, ls, le, gamma).cpu().numpy()
+    got = {k: v.cpu().numpy() for k, v in r.render_backward(cam, torch.from_numpy(up.astype(np.float32)).cuda(), deg).items()}
+    fr = OracleScene(lv, deg).frame(cam, ls, le, gamma, pair_rule=r.pair_rule)
+    want, ref_img = ob.backward(lv, deg, cam, fr, up)
+    assert np.abs(img - ref_img).max() < 5e-3
+    worst = {}
+    for k in ("mean", "log_scale", "quat", "logit", "sh"):
+        scale = np.abs(want[k]).max()
+        err = np.abs(got[k] - want[k]).max()
+        worst[k] = err / (scale + 1e-30)
+        assert err <= tol * scale + 1e-7, (k, err, scale)
+    # Gaussians the frame does not draw have zero gradients on both sides
+    drawn = fr.state >= oracle.ST_EMPTY_RECT
+    assert all((got[k][~drawn] == 0).all() for k in got)
+    r.close()
+    return worst, got, want
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("seed,deg", [(0, 0), (1, 1), (2, 2), (3, 3), (4, 3), (5, 1)])
+def test_kernel_gradients_match_the_oracle(seed, deg):
+    """Every parameter's gradient within 1e-4 of the array's largest gradient (fp32 kernels, sums in atomic order, against
+    the fp64 oracle), on scenes that span several tiles, ragged images, off-centre anisotropic cameras, both level modes."""
+    rng = np.random.default_rng(100 + seed)
+    lv = _scene(rng, (60, 90), sh_degree=deg, extent=1.2)
+    cam = camera(width=int(rng.integers(30, 70)), height=int(rng.integers(30, 60)), f=float(rng.uniform(25, 60)), fy=float(rng.uniform(25, 60)),
+                 cx=float(rng.uniform(15, 30)), cy=float(rng.uniform(15, 30)), bg=tuple(rng.uniform(0, 1, 3)))
+    up = rng.normal(size=(3, cam.height, cam.width))
+    worst, _, _ = _gpu_vs_oracle(lv, deg, cam, 1, 2, 1.0, up)
+    print("single frame, levels {1,2}:", {k: f"{v:.1e}" for k, v in worst.items()})
+    _gpu_vs_oracle(lv, deg, cam, 2, 2, 1.0, up)
+
+
+@pytest.mark.gpu
+def test_kernel_saturated_pixels_clamps_and_early_stop():
+    """Opaque, large, overlapping Gaussians: alpha clamped at 0.99 (zero slope there), pixels that stop early (entries
+    behind the stop get nothing), a Gaussian beside the frustum (R8's clamp), a non-zero background."""
+    rng = np.random.default_rng(77)
+    n = 80
+    pos = np.stack([rng.uniform(-1.5, 1.5, n), rng.uniform(-1.0, 1.0, n), rng.uniform(1.0, 5.0, n)], axis=1)
+    pos[0] = [4.5, 0.2, 1.5]                                      # far beside the frustum, large: the Jacobian clamp is active
+    sc = np.exp(rng.uniform(-1.8, -0.3, (n, 3))); sc[0] = 1.2
+    sh = rng.normal(0, 0.2, (n, 4, 3)); sh[:, 0, :] += 0.9
+    lv = [level(1, 0.0, pos, sc, quat=rng.normal(size=(n, 4)), logit=rng.normal(4.0, 2.0, n), sh=sh)]
+    cam = camera(width=48, height=40, f=40.0, bg=(0.7, 0.1, 0.4))
+    up = rng.normal(size=(3, 40, 48))
+    worst, got, want = _gpu_vs_oracle(lv, 1, cam, 1, 1, 1.0, up, tol=5e-4)
+    print('saturated:', {k: f'{v:.1e}' for k, v in worst.items()})
+    fr = OracleScene(lv, 1).frame(cam, 1, 1, 1.0)
+    _, E, B, T = fr.composite(stats=True)
+    assert (T < 1e-4).mean() > 0.3                                 # many pixels stop early
+
+
+@pytest.mark.gpu
+def test_kernel_contract_and_zero_upstream():
+    from paper_2408_12894_b200 import build
+    build.build()
+    import paper_2408_12894_b200 as pkg
+    rng = np.random.default_rng(9)
+    lv = _scene(rng, (30,), sh_degree=2)
+    cam = camera(width=32, height=32, f=30.0)
+    r = pkg.Renderer(0)
+    r.upload_levels(lv, 2)
+    r.set_workspace(32, 32, 1 << 20)
+    z = torch.zeros((3, 32, 32), device="cuda")
+    with pytest.raises(pkg.FlodError):                              # nothing rendered yet
+        r.render_backward(cam, z, 2)
+    r.render(cam, 1, 1, 1.0)
+    g = r.render_backward(cam, z, 2)
+    assert all((v == 0).all().item() for v in g.values())           # S:163
+    with pytest.raises(pkg.FlodError):                              # S:160: not the camera of the forward pass
+        r.render_backward(camera(width=32, height=32, f=31.0), z, 2)
+    r.render_rows(cam, 1, 1, 1.0, 0, 1)
+    with pytest.raises(pkg.FlodError):                              # the last frame was a strip
+        r.render_backward(cam, z, 2)
+    r.close()
+
+
+@pytest.mark.gpu
+def test_kernel_on_long_lists_over_many_tiles():
+    """1000 Gaussians (degree 3, two levels, selective rendering) on a ragged 110 x 70 image: 35 tiles whose lists hold
+    hundreds of entries -- several batches of the backward walk, many entries per pixel behind the early stop."""
+    rng = np.random.default_rng(21)
+    lv = _scene(rng, (400, 600), sh_degree=3, extent=1.6)
+    cam = camera(width=110, height=70, f=62.0, fy=55.0, cx=52.0, cy=37.5, bg=(0.2, 0.4, 0.6))
+    up = rng.normal(size=(3, 70, 110))
+    fr = OracleScene(lv, 3).frame(cam, 2, 2, 1.0)
+    assert fr.tile_counts.max() > 3 * 64 and fr.counts["n_vis"] > 400
+    _gpu_vs_oracle(lv, 3, cam, 1, 2, 1.0, up, tol=2e-4)
+    worst, got, want = _gpu_vs_oracle(lv, 3, cam, 2, 2, 1.0, up, tol=2e-4)
+    print("long lists:", {k: f"{v:.1e}" for k, v in worst.items()}, "longest list", int(fr.tile_counts.max()))
