@@ -47,9 +47,9 @@ def parse_args():
     ap.add_argument("--subset-period", type=int, default=0,
                     help="selective modes only: render from a materialised G_sel (flod_render_subset) that is rebuilt "
                          "every N frames on a second stream and swapped in when ready (P:699-711); 0 = Eq. 6 per frame")
-    ap.add_argument("--pair-rule", type=int, default=2, choices=[1, 2],
-                    help="which tiles a Gaussian is listed in: 1 = every tile of its rect (R13), 2 = the tiles the alpha = 1/255 "
-                         "ellipse reaches (R26, the library's default); same image, fewer pairs")
+    ap.add_argument("--pair-rule", type=int, default=1, choices=[1, 2],
+                    help="which tiles a Gaussian is listed in: 1 = every tile of its rect (R13, the library's default), 2 = the "
+                         "tiles the alpha = 1/255 ellipse reaches (R26); same image, 22-32 %% fewer pairs")
     ap.add_argument("--shard", default="poses", choices=["poses", "rows"],
                     help="N > 1: poses = replicas, every rank renders its own poses, no collective (weak scaling); rows = "
                          "every rank renders its strip of tile rows of the SAME pose and one all-gather per frame assembles "
@@ -167,7 +167,7 @@ class ClockSampler:
 
 # ----------------------------------------------------------------------------------------- reference arm
 
-def oracle_frame_seconds(osc, cam, ls, le, gamma, pair_rule=2):
+def oracle_frame_seconds(osc, cam, ls, le, gamma, pair_rule=1):
     t0 = time.perf_counter()
     fr = osc.frame(cam, ls, le, gamma, pair_rule=pair_rule)
     img = fr.composite()
@@ -436,11 +436,16 @@ def run_ours(args):
     tile_bits = max(0, (T_n - 1).bit_length())
     P, NV = agg["n_pairs"], agg["n_vis"]
     grid_cells = ((cam0.width + 15) // 16 + 1) * ((cam0.height + 15) // 16 + 1)
-    alg = {   # algorithmic bytes / flops per frame, DESIGN §6
-        "geometry": 12 * agg["n_scan"] + 28 * agg["n_front"] + 4 * NV + 56 * NV,
-        "colour": (4 + 16 + 12 * Kc) * NV + 12 * NV + 4 * grid_cells + 12 * T_n,     # + the tile scan of its block 0
-        "duplicate": 16 * NV + 8 * P,
-        "tile_sort": 8 * P + 4 * P,
+    # Algorithmic bytes / flops per frame: SURVEY §8(d)'s per-unit figures (what the METHOD must move -- none of this
+    # build's own intermediates) times the frame's measured counts.  a1-a4 = 12 N_scan + 28 N_front + (4 + 12K) N_vis read
+    # + 52 N_vis written, split here into the geometry kernel (means, covariances; mu', z, conic + o, rect, count written)
+    # and the colour kernel (gid + SH row read, rgb written); a6 = 16 N_vis + 12 P; a7 = 24 P (the floor of any
+    # sort-based pipeline: keys read and written once); a9 = 14 E + 10 B flops.
+    alg = {
+        "geometry": 12 * agg["n_scan"] + 28 * agg["n_front"] + 40 * NV,
+        "colour": (4 + 12 * Kc) * NV + 12 * NV,
+        "duplicate": 16 * NV + 12 * P,
+        "tile_sort": 24 * P,
         "blend_flops": 14 * E + 10 * B,
     }
     stages = {}
@@ -451,15 +456,14 @@ def run_ours(args):
     tfl = alg["blend_flops"] / (stage_ms[-1] * 1e-3) / 1e12 if stage_ms[-1] > 0 else 0.0
     stages["blend"] = {"ns": stage_ms[-1] * 1e6, "bound": "alu", "achieved": tfl, "peak": fp32_peak, "unit": "TFLOP/s",
                        "frac": tfl / fp32_peak, "alg_flops": alg["blend_flops"], "evals": E, "blends": B}
-    # steps a6-a8 (duplication + ordering + ranges) against the single 64-bit-key LSD radix sort model
-    # (12 B written + 152 B sorted + 8 B ranges per pair at 6 passes; the tile scan now hides inside the colour kernel
-    # and is not counted), so that replacing the global sort by binning
-    # + per-tile sorts shows up as > model rather than as hidden work
+    # SURVEY §8(d) also asks for steps a6-a8 against the single 64-bit-key LSD radix sort MODEL (12 B written + 152 B
+    # sorted + 8 B ranges per pair at 6 passes): not a roofline of work done -- it says how long the modelled global sort
+    # would take at HBM peak next to what binning + per-tile sorts take (frac > 1: faster than the model at peak)
     sort_ms = stage_ms[2] + stage_ms[3]
     lsd64 = (12 + 2 * 12 * ((32 + tile_bits + 7) // 8) + 8 + 8) * P
-    sort_vs_model = {"model_bytes": lsd64, "ns": sort_ms * 1e6, "achieved": lsd64 / (sort_ms * 1e-3) / 1e9 if sort_ms > 0 else 0.0,
-                     "peak": hbm, "unit": "GB/s"}
-    sort_vs_model["frac"] = sort_vs_model["achieved"] / hbm
+    sort_vs_model = {"model_bytes": lsd64, "ns": sort_ms * 1e6, "model_ns_at_hbm_peak": lsd64 / hbm,
+                     "frac": (lsd64 / hbm) / (sort_ms * 1e6) if sort_ms > 0 else 0.0,
+                     "note": "time the 172 B/pair LSD-sort model needs at HBM peak / time of duplicate + tile_sort; a model, not a roofline"}
     dominant = max(stages, key=lambda n: stages[n]["ns"])
     roof = {k: stages[dominant][k] for k in ("bound", "achieved", "peak", "unit", "frac")}
     traffic, traffic_src = ncu_traffic(dominant) if (args.config, mode, args.count_scale) == (1, "max", 1.0) else (None, None)
@@ -491,7 +495,8 @@ def run_ours(args):
         osc = oracle.OracleScene(scene.levels, scene.sh_degree)
         dt, fr, _ = oracle_frame_seconds(osc, cams[0], ls, le, args.gamma, args.pair_rule)
         line["cpu_baseline"] = {"value": 1.0 / dt, "unit": "frames/s", "cores": oracle.num_threads(), "kind": "oracle",
-                                "sample": "1 full frame (pose 0): selection + projection + pair sort + tiled compositing"}
+                                "sample": "1 full frame (pose 0): selection + projection + per-tile pair lists and their sorts + tiled compositing, "
+                                          "OpenMP over Gaussians / tiles (two serial passes build the lists)"}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

@@ -35,7 +35,7 @@ extern "C" {
 #define FLOD_API
 #endif
 
-#define FLOD_ABI_VERSION 8
+#define FLOD_ABI_VERSION 9
 #define FLOD_MAX_LEVELS 16
 #define FLOD_TILE 16                 /* tiles are 16x16 pixels */
 #define FLOD_N_STAGES 5              /* 0 geometry (a1-a3), 1 colour (a4) with the tile scan (a5, a8) in one of its blocks,
@@ -99,8 +99,12 @@ enum {                               /* flod_set_options bits */
     FLOD_OPT_DEBUG   = 1,            /* also write the selection mask and per-Gaussian projection records */
     FLOD_OPT_PROFILE = 2,            /* record CUDA events between stages (flod_get_stats reports ms) */
     FLOD_OPT_COUNT   = 4,            /* instrumented blend kernel counting evaluations and blends */
-    FLOD_OPT_SMALL_WINDOWS = 8       /* test knob: the large-rect duplication kernel walks the tiles in windows of 1024 (the
+    FLOD_OPT_SMALL_WINDOWS = 8,      /* test knob: the large-rect duplication kernel walks the tiles in windows of 1024 (the
                                         path an image of more than 48 Ki tiles takes) */
+    FLOD_OPT_FULL_SORT = 16          /* order every tile list completely.  By default a list of more than 4096 pairs is ordered
+                                        only as far as the blend reads it (nearest depth slices first, the rest if pixels of
+                                        the tile are still alive): same image bit for bit.  FLOD_OPT_DEBUG and FLOD_OPT_COUNT
+                                        imply it; flod_render_backward needs it. */
 };
 
 enum {                               /* flod_debug_copy selectors; host_dst sizes in bytes */
@@ -151,10 +155,11 @@ FLOD_API int flod_set_options(flod_ctx *ctx, unsigned flags);
 /* Which tiles a visible Gaussian is listed in (R13, R26).  Both rules are conservative -- every pixel with
  * alpha >= 1/255 lies in a listed tile -- so the image is the same; per-tile pair counts, n_pairs and
  * the sorted pair sequence are those of the chosen rule.
- *   FLOD_PAIR_RULE_BOX      every tile of the rect (the padded box of the alpha = 1/255 contour);
- *   FLOD_PAIR_RULE_ELLIPSE  (default) the tiles of the rect that hold a pixel centre of the padded alpha = 1/255 ellipse
- *                           of Eq. 2: one span of tiles per tile row, computed in fp64 from the rounded
- *                           conic; 20-30 % fewer pairs. */
+ *   FLOD_PAIR_RULE_BOX      (default) every tile of the rect (the padded box of the alpha = 1/255 contour);
+ *   FLOD_PAIR_RULE_ELLIPSE  the tiles of the rect that hold a pixel centre of the padded alpha = 1/255 ellipse of Eq. 2
+ *                           (P:104-108): one span of tiles per tile row, canonical fp32 on the factorised exponent.
+ *                           22-32 % fewer pairs; finding them costs about what they save on fine levels (config 1:
+ *                           -2 % frames/s) and pays on coarse ones (config 3, levels 2-5: +2 .. +10 %). */
 enum { FLOD_PAIR_RULE_BOX = 1, FLOD_PAIR_RULE_ELLIPSE = 2 };
 FLOD_API int flod_set_pair_rule(flod_ctx *ctx, int rule);
 

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libflod.so")
 HEADER = os.path.join(HERE, "..", "include", "flod.h")
 
-FLOD_OPT_DEBUG, FLOD_OPT_PROFILE, FLOD_OPT_COUNT, FLOD_OPT_SMALL_WINDOWS = 1, 2, 4, 8
+FLOD_OPT_DEBUG, FLOD_OPT_PROFILE, FLOD_OPT_COUNT, FLOD_OPT_SMALL_WINDOWS, FLOD_OPT_FULL_SORT = 1, 2, 4, 8, 16
 FLOD_DBG_MASK, FLOD_DBG_TILE_COUNTS, FLOD_DBG_PROJECTED, FLOD_DBG_SORTED_PAIRS, FLOD_DBG_ACTIVATED = range(5)
 PAIR_RULE_BOX, PAIR_RULE_ELLIPSE = 1, 2
 FLOD_N_STAGES = 5
@@ -160,7 +160,7 @@ class Renderer:
         self.workspace = None
         self.n_total = 0
         self.ws_dims = None
-        self.pair_rule = PAIR_RULE_ELLIPSE          # the library's default (include/flod.h)
+        self.pair_rule = PAIR_RULE_BOX              # the library's default (include/flod.h)
 
     def close(self):
         if getattr(self, "_h", None):

@@ -59,10 +59,15 @@ __device__ __forceinline__ float ex2(float x)
 
 constexpr int kBlendUnroll = 4;
 constexpr int kBlendMinBlocks = 8;                   // 64 registers per thread
-template <bool COUNT>
+// RESUME: the second round of blend-driven ordering.  In a lazy frame k_tile_sort orders only the nearest
+// slices of a long list; the first round (RESUME = false) blends that prefix and, if pixels of the tile are still alive at
+// its end, saves (T, r, g, b) of every pixel and asks for the rest; k_tile_sort_rest orders it, and this kernel
+// (RESUME = true) takes the saved state up from where the first round stopped.  The per-pixel sequence of blends is the
+// one of a fully sorted list, so the image is bit-identical.
+template <bool COUNT, bool RESUME>
 __global__ void __launch_bounds__(kBlendThreads, kBlendMinBlocks)
 k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, int n_tiles,
-        float bg0, float bg1, float bg2, int tile0, int out_row0, int out_rows)
+        float bg0, float bg1, float bg2, int tile0, int out_row0, int out_rows, int lazy)
 {
     // staging, 36 bytes per Gaussian of the batch: A = (mu'x, mu'y, k, a2), B = (d2, log2 o, r, g), c = b
     __shared__ float4 s_A[2][kBatch], s_B[2][kBatch];           // double-buffered
@@ -85,7 +90,19 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
     const float row0 = (float)(warp * 4);               // first row of the warp's strip inside the tile
     const float kThr = -7.994353436858858f - 1.0e-3f;   // log2(1/255) minus a safety margin
 
-    const uint2 rg = ws.ranges[tile];
+    uint2 rg = ws.ranges[tile];
+    const unsigned int L_full = rg.y - rg.x;
+    bool partial = false;                               // this round ends before the list does
+    if (RESUME) {
+        if (L_full <= (unsigned int)kSortCap) return;
+        const uint4 lz = ws.lazy[tile];
+        if (!lz.w) return;                              // the first round finished this tile
+        rg.x += lz.x;                                   // go on behind the prefix it consumed
+    } else if (lazy && L_full > (unsigned int)kSortCap) {
+        const unsigned int upto = ws.lazy[tile].x;
+        partial = upto < L_full;
+        rg.y = rg.x + upto;
+    }
     const uint32_t *__restrict__ vals = ws.vals;
     const float4 *__restrict__ gA = ws.gA;
     const float4 *__restrict__ gB = ws.gB;
@@ -94,10 +111,14 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
     // two pixels per thread, packed as float2 (.x = row py0, .y = row py1): the per-pixel arithmetic runs on the
     // packed FP32 instructions of sm_100 (FADD2 / FMUL2 / FFMA2: one issue slot for both pixels)
     float2 T = make_float2(in0 ? 1.0f : 0.0f, in1 ? 1.0f : 0.0f), cr = make_float2(0.0f, 0.0f), cg = cr, cb2 = cr;
+    if (RESUME) {
+        const float4 s0 = ws.tile_state[(size_t)tile * 256 + 2 * tid], s1 = ws.tile_state[(size_t)tile * 256 + 2 * tid + 1];
+        T = make_float2(s0.x, s1.x); cr = make_float2(s0.y, s1.y); cg = make_float2(s0.z, s1.z); cb2 = make_float2(s0.w, s1.w);
+    }
     unsigned int n_eval = 0, n_blend = 0;
     float4 *my_buf = s_buf[warp];
     const float4 *my_half = my_buf + half;
-    bool warp_done = __all_sync(0xffffffffu, !in0 && !in1);         // pixels outside the image start with T = 0
+    bool warp_done = __all_sync(0xffffffffu, T.x < 1e-4f && T.y < 1e-4f);   // (pixels outside the image start with T = 0)
 
     // evaluates my_buf[0, cnt) on the thread's two pixels.  a2 <= 0 and e0 <= log2 o (k_geometry clamps d2), so
     // q >= 0 holds by construction and alpha needs the 0.99 clamp only.  A pixel that is done or below 1/255 blends 0.
@@ -213,6 +234,15 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
             }
         }
     }
+    if (!RESUME && partial) {
+        // the sorted prefix is used up: is any pixel of the tile still alive?  Then the rest of the list is wanted
+        if (__syncthreads_or(!(T.x < 1e-4f && T.y < 1e-4f))) {
+            ws.tile_state[(size_t)tile * 256 + 2 * tid] = make_float4(T.x, cr.x, cg.x, cb2.x);
+            ws.tile_state[(size_t)tile * 256 + 2 * tid + 1] = make_float4(T.y, cr.y, cg.y, cb2.y);
+            if (tid == 0) ws.lazy[tile].w = 1u;
+            return;                                     // k_blend<.., true> writes the pixels
+        }
+    }
     const bool done0 = T.x < 1e-4f, done1 = T.y < 1e-4f;
     const float T0 = T.x, T1 = T.y, r0 = cr.x, r1 = cr.y, g0 = cg.x, g1 = cg.y, b0 = cb2.x, b1 = cb2.y;
     const size_t plane = (size_t)W * out_rows;          // out holds image rows [out_row0, out_row0 + out_rows) of every plane
@@ -245,11 +275,21 @@ int launch_blend(const Context &c, const FrameParams &p, float *out_rgb, cudaStr
     const int tile0 = p.ty_begin * p.TX, n_tiles = p.ty_end * p.TX, grid = n_tiles - tile0;
     if (grid <= 0) return 0;
     if (c.flags & FLOD_OPT_COUNT)
-        k_blend<true><<<grid, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
-                                                     p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows);
+        k_blend<true, false><<<grid, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
+                                                            p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows, 0);
     else
-        k_blend<false><<<grid, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
-                                                      p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows);
+        k_blend<false, false><<<grid, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
+                                                             p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows, p.lazy_sort);
+    return 1;
+}
+
+// second round of a lazy frame: the tiles the first round left unfinished (all other CTAs exit at once)
+int launch_blend_rest(const Context &c, const FrameParams &p, float *out_rgb, cudaStream_t s)
+{
+    const int tile0 = p.ty_begin * p.TX, n_tiles = p.ty_end * p.TX, grid = n_tiles - tile0;
+    if (grid <= 0 || !p.lazy_sort) return 0;
+    k_blend<false, true><<<grid, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
+                                                        p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows, 1);
     return 1;
 }
 

@@ -130,6 +130,9 @@ WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_p
     L.ws.vals = (uint32_t *)take((size_t)max_pairs * 4);
     L.ws.ovf_slots = (unsigned int *)take(4 * sizeof(unsigned int));
     L.ws.ovf_out = L.ws.ovf_slots + 2;
+    L.ws.lazy = (uint4 *)take(tiles * sizeof(uint4));
+    L.ws.slice_ends = (unsigned int *)take(tiles * kCoarseBins * sizeof(unsigned int));
+    L.ws.tile_state = (float4 *)take(tiles * 256 * sizeof(float4));
     L.ws.image[0] = (float *)take((size_t)3 * w * h * sizeof(float));
     L.ws.image[1] = (float *)take((size_t)3 * w * h * sizeof(float));
     L.bytes = off;
@@ -356,7 +359,9 @@ int flod_set_pair_rule(flod_ctx *ctx, int rule)
 int flod_launches_per_frame(const flod_ctx *ctx)
 {
     if (!ctx || !ctx->has_ws) return 0;
-    return 6;   // geometry, colour (+ tile scan in its block 0), duplication (two kernels, one of which exits), tile sort, blend
+    // geometry, colour (+ tile scan in its block 0), duplication (two kernels, one of which exits), tile sort, blend; with
+    // blend-driven ordering also the second round of the last two (their CTAs exit at once unless a tile asked for it)
+    return (ctx->flags & (FLOD_OPT_DEBUG | FLOD_OPT_COUNT | FLOD_OPT_FULL_SORT)) ? 6 : 8;
 }
 
 }  // extern "C"
@@ -430,6 +435,8 @@ int enqueue_frame(flod_ctx *ctx, const SceneDev &sc, FrameParams &p, float *out_
     const int64_t n_scan = p.n_scan;
     p.max_pairs = (unsigned int)ctx->max_pairs;
     p.pair_rule = ctx->pair_rule;
+    // blend-driven ordering of long lists, unless a view of the frame needs every list in its final order
+    p.lazy_sort = (ctx->flags & (FLOD_OPT_DEBUG | FLOD_OPT_COUNT | FLOD_OPT_FULL_SORT)) ? 0 : 1;
     p.quad_gid = p.first_gid & ~3ll;
     p.n_pre_blocks = (int)((p.first_gid - p.quad_gid + n_scan + kGeoBlock - 1) / kGeoBlock);
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
@@ -447,6 +454,7 @@ int enqueue_frame(flod_ctx *ctx, const SceneDev &sc, FrameParams &p, float *out_
     mark(); launch_duplicate(*ctx, p, s);
     mark(); launch_tile_sort(*ctx, p, s);
     mark(); launch_blend(*ctx, p, out_rgb_dev, s);
+    launch_tile_sort_rest(*ctx, p, s); launch_blend_rest(*ctx, p, out_rgb_dev, s);     // (both exit at once unless a tile asked)
     mark();
     CUDA_TRY(ctx, cudaGetLastError());
     ctx->ev_valid = prof;
@@ -742,6 +750,8 @@ int flod_render_backward(flod_ctx *ctx, const flod_camera *cam, const float *dL_
         return fail(ctx, FLOD_E_INVALID_ARG, "render_backward: the camera is not the one of the last flod_render");
     if (p.ty_begin != 0 || p.ty_end != p.TY)
         return fail(ctx, FLOD_E_INVALID_ARG, "render_backward: the last frame was a strip (flod_render_rows)");
+    if (p.lazy_sort)
+        return fail(ctx, FLOD_E_INVALID_ARG, "render_backward: render the frame with FLOD_OPT_FULL_SORT (its lists must be in their final order throughout)");
     cudaStream_t s = (cudaStream_t)stream;
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     // gradients are indexed by gid over the whole scene: zero, then the drawn Gaussians add theirs

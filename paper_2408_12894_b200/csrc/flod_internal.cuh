@@ -19,6 +19,7 @@ constexpr int kGeoPer = 1024 / kGeoThreads;     // a block scans 1024 Gaussians 
 static_assert(kGeoPer % 4 == 0 && kGeoPer * kGeoThreads == 1024, "whole quads per thread, 1024 per block");
 constexpr int kGeoBlock = kGeoThreads * kGeoPer;
 constexpr int kSortCap = 4096;            // per-tile sort: lists up to this many keys are scattered into shared memory
+constexpr int kCoarseBins = 256;          // ... longer ones are first cut into at most this many depth slices
 constexpr int kCtrStride = 64;            // ints between two per-tile atomic counters: one counter per 256 B, so that the
                                           // L2 slices share the atomic traffic (a dense 16 KB grid sits on a few slices)
 
@@ -90,6 +91,10 @@ struct WorkspaceDev {
     uint32_t *vals;                       // [max_pairs] positions, grouped by tile, sorted by (depth, gid)
     unsigned int *ovf_slots;              // [3] overflow word of the frame rendered into image[0], image[1], and of any other frame
     unsigned int *ovf_out;                // where THIS frame's tile scan reports (set on the host before the launches)
+    uint4 *lazy;                          // [T_n] lists longer than kSortCap, blend-driven ordering: (keys in final order so far, next
+                                          // slice to sort, slices, 1 = the blend wants the rest)
+    unsigned int *slice_ends;             // [T_n][kCoarseBins] ends of the depth slices of those lists
+    float4 *tile_state;                   // [T_n][256] (T, r, g, b) of every pixel of a tile the blend left unfinished
     float *image[2];                      // 2 x [3][H][W] for flod_render_to_host(_async): double-buffered so that the copy
                                           // of frame k overlaps the kernels of frame k + 1
 };
@@ -117,6 +122,7 @@ struct FrameParams {
     int ty_begin, ty_end;                 // the strip of tile rows this frame renders ([0, TY) = the whole image): rects are
                                           // clipped to it, tiles outside it get no pairs and are not blended
     int out_row0, out_rows;               // out_rgb holds image rows [out_row0, out_row0 + out_rows) of every colour plane
+    int lazy_sort;                        // blend-driven ordering of long lists (off for the debug / counting / training views)
 };
 
 struct Context {
@@ -138,7 +144,7 @@ struct Context {
     int64_t max_pairs = 0;
     // options / state
     unsigned flags = 0;
-    int pair_rule = FLOD_PAIR_RULE_ELLIPSE;
+    int pair_rule = FLOD_PAIR_RULE_BOX;
     bool has_ref = false;
     float ref[3] = {0, 0, 0};
     cudaStream_t last_stream = nullptr;
@@ -178,6 +184,8 @@ int launch_duplicate(const Context &c, const FrameParams &p, cudaStream_t s);   
 int init_duplicate();                                                            // once per device: shared-memory opt-in
 int init_tile_sort();                                                            // once per device: shared-memory opt-in
 int launch_tile_sort(const Context &c, const FrameParams &p, cudaStream_t s);   // a7
+int launch_tile_sort_rest(const Context &c, const FrameParams &p, cudaStream_t s);   // a7, the lists the blend did not finish
+int launch_blend_rest(const Context &c, const FrameParams &p, float *out_rgb, cudaStream_t s);   // a9, those tiles
 int launch_blend(const Context &c, const FrameParams &p, float *out_rgb, cudaStream_t s);   // a9
 // backward pass of a9 and of a2-a4 (backward.cu); g9 = [positions][9] screen-space gradients (workspace of the backward pass)
 int launch_backward(const Context &c, const FrameParams &p, const float *dL_dimage, float *g9, const flod_grads &out, cudaStream_t s);

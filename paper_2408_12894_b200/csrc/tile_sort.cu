@@ -22,7 +22,8 @@ constexpr int kSortBins = 1 << kSortBinsLog;
 constexpr int kSortKeysPerBinLog = 1;                     // about two keys per bin
 constexpr int kSortSliceLog = 10;                         // depth slices of long lists: 512-1024 keys
 constexpr int kCoarseBinsLog = 8;
-constexpr int kCoarseBins = 1 << kCoarseBinsLog;
+static_assert(kCoarseBins == 1 << kCoarseBinsLog, "slices per long list");
+constexpr unsigned int kLazyFirst = 1024;                 // LAZY: keys of a long list that are sorted before the blend starts
 constexpr unsigned int kRankMax = 64;                     // bins up to this size are finished by per-key rank counting
 
 typedef unsigned long long u64;
@@ -200,6 +201,27 @@ __device__ void finish_sort(const u64 *buf, unsigned int n, const BinMap &m, u64
     }
 }
 
+// Sorts slice b (keys tmp[lo, lo + n2), left there by the coarse pass) into vals[lo, lo + n2); pairs[lo, ...) is scratch.
+__device__ __forceinline__ void sort_slice(u64 *pairs, u64 *tmp, uint32_t *vals, unsigned int lo, unsigned int n2, SortSmem &S, int tid)
+{
+    if (n2 == 0) return;
+    if (n2 == 1) { if (tid == 0) vals[lo] = (uint32_t)tmp[lo]; return; }
+    if (n2 <= (unsigned int)kSortCap) {
+        const BinMap m = bin_pass(tmp + lo, S.keys, n2, S.ends[0], S, tid);
+        finish_sort(S.keys, n2, m, pairs + lo, vals + lo, S, tid);
+    } else {
+        const BinMap m = bin_pass(tmp + lo, pairs + lo, n2, S.ends[0], S, tid);
+        finish_sort(pairs + lo, n2, m, tmp + lo, vals + lo, S, tid);
+    }
+    __syncthreads();
+    if (tid == 0) S.any_big[0] = 0;                      // ordered before its next readers by the barriers of bin_pass
+}
+
+// LAZY (blend-driven ordering): of a list longer than kSortCap only the nearest depth slices -- at least
+// kLazyFirst keys -- are sorted here; the slice ends stay in ws.slice_ends, ws.lazy[tile] says how far the order goes.
+// k_blend consumes that prefix, and only the tiles whose pixels are still alive at its end are finished by
+// k_tile_sort_rest / k_blend<.., true>.  On a coarse level alone the blend reads 5-7 % of every list.
+template <bool LAZY>
 __global__ void __launch_bounds__(kSortThreads, 4)      // 4 CTAs per SM is what the 49 KB of shared memory allow
 k_tile_sort(const WorkspaceDev ws, int tile0, int n_tiles)
 {
@@ -227,19 +249,39 @@ k_tile_sort(const WorkspaceDev ws, int tile0, int n_tiles)
     // equal depths) goes through global memory.
     u64 *tmp = ws.pairs_tmp + rg.x;
     const BinMap mc = bin_pass(pairs, tmp, L, S.cends, S, tid, kSortSliceLog, 1, kCoarseBinsLog);
-    for (unsigned int b = 0; b < mc.nb; ++b) {
-        const unsigned int lo = b ? S.cends[b - 1] : 0u, n2 = S.cends[b] - lo;
-        if (n2 == 0) continue;
-        if (n2 == 1) { if (tid == 0) vals[lo] = (uint32_t)tmp[lo]; continue; }
-        if (n2 <= (unsigned int)kSortCap) {
-            const BinMap m = bin_pass(tmp + lo, S.keys, n2, S.ends[0], S, tid);
-            finish_sort(S.keys, n2, m, pairs + lo, vals + lo, S, tid);
-        } else {
-            const BinMap m = bin_pass(tmp + lo, pairs + lo, n2, S.ends[0], S, tid);
-            finish_sort(pairs + lo, n2, m, tmp + lo, vals + lo, S, tid);
-        }
-        __syncthreads();
-        if (tid == 0) S.any_big[0] = 0;                  // ordered before its next readers by the barriers of bin_pass
+    unsigned int b = 0;
+    for (; b < mc.nb; ++b) {
+        const unsigned int lo = b ? S.cends[b - 1] : 0u;
+        if (LAZY && lo >= kLazyFirst) break;             // enough for most tiles: the rest on demand
+        sort_slice(pairs, tmp, vals, lo, S.cends[b] - lo, S, tid);
+    }
+    if (LAZY) {
+        for (unsigned int i = tid; i < mc.nb; i += kSortThreads) ws.slice_ends[(size_t)tile * kCoarseBins + i] = S.cends[i];
+        if (tid == 0) ws.lazy[tile] = make_uint4(b ? S.cends[b - 1] : 0u, b, mc.nb, 0u);   // sorted up to, next slice, slices, more wanted
+    }
+}
+
+// The rest of the lists whose tiles k_blend left unfinished (ws.lazy[tile].w set): slices next .. n of the coarse pass.
+__global__ void __launch_bounds__(kSortThreads, 4)
+k_tile_sort_rest(const WorkspaceDev ws, int tile0, int n_tiles)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    SortSmem &S = *reinterpret_cast<SortSmem *>(smem_raw);
+    const int tile = tile0 + blockIdx.x;
+    if (tile >= n_tiles) return;
+    const uint2 rg = ws.ranges[tile];
+    if (rg.y - rg.x <= (unsigned int)kSortCap || ws.hdr->overflow) return;
+    const uint4 lz = ws.lazy[tile];
+    if (!lz.w) return;
+    const int tid = threadIdx.x;
+    for (unsigned int i = tid; i < lz.z; i += kSortThreads) S.cends[i] = ws.slice_ends[(size_t)tile * kCoarseBins + i];
+    if (tid == 0) S.any_big[0] = 0;
+    __syncthreads();
+    u64 *pairs = ws.pairs + rg.x, *tmp = ws.pairs_tmp + rg.x;
+    uint32_t *vals = ws.vals + rg.x;
+    for (unsigned int b = lz.y; b < lz.z; ++b) {
+        const unsigned int lo = b ? S.cends[b - 1] : 0u;
+        sort_slice(pairs, tmp, vals, lo, S.cends[b] - lo, S, tid);
     }
 }
 
@@ -247,7 +289,10 @@ k_tile_sort(const WorkspaceDev ws, int tile0, int n_tiles)
 // the opt-in is a per-device attribute of the function.
 int init_tile_sort()
 {
-    return cudaFuncSetAttribute(k_tile_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)) == cudaSuccess ? 0 : -1;
+    const int bytes = (int)sizeof(SortSmem);
+    return cudaFuncSetAttribute(k_tile_sort<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess &&
+           cudaFuncSetAttribute(k_tile_sort<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess &&
+           cudaFuncSetAttribute(k_tile_sort_rest, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess ? 0 : -1;
 }
 
 int launch_tile_sort(const Context &c, const FrameParams &p, cudaStream_t s)
@@ -255,7 +300,16 @@ int launch_tile_sort(const Context &c, const FrameParams &p, cudaStream_t s)
     if (p.n_pre_blocks <= 0) return 0;
     const int tile0 = p.ty_begin * p.TX, n_tiles = p.ty_end * p.TX;
     if (n_tiles <= tile0) return 0;
-    k_tile_sort<<<n_tiles - tile0, kSortThreads, sizeof(SortSmem), s>>>(c.ws, tile0, n_tiles);
+    if (p.lazy_sort) k_tile_sort<true><<<n_tiles - tile0, kSortThreads, sizeof(SortSmem), s>>>(c.ws, tile0, n_tiles);
+    else k_tile_sort<false><<<n_tiles - tile0, kSortThreads, sizeof(SortSmem), s>>>(c.ws, tile0, n_tiles);
+    return 1;
+}
+
+int launch_tile_sort_rest(const Context &c, const FrameParams &p, cudaStream_t s)
+{
+    const int tile0 = p.ty_begin * p.TX, n_tiles = p.ty_end * p.TX;
+    if (p.n_pre_blocks <= 0 || n_tiles <= tile0 || !p.lazy_sort) return 0;
+    k_tile_sort_rest<<<n_tiles - tile0, kSortThreads, sizeof(SortSmem), s>>>(c.ws, tile0, n_tiles);
     return 1;
 }
 

@@ -92,6 +92,7 @@ def _gpu_vs_oracle(lv, deg, cam, ls, le, gamma, up, tol=1e-4):
     r = pkg.Renderer(0)
     r.upload_levels(lv, deg)
     r.set_workspace(cam.width, cam.height, 1 << 22)
+    r.set_options(pkg.FLOD_OPT_FULL_SORT)             # the backward pass walks the lists of the forward pass: all of them in order
     img = r.render(cam, ls, le, gamma).cpu().numpy()
     got = {k: v.cpu().numpy() for k, v in r.render_backward(cam, torch.from_numpy(up.astype(np.float32)).cuda(), deg).items()}
     fr = OracleScene(lv, deg).frame(cam, ls, le, gamma, pair_rule=r.pair_rule)
@@ -157,6 +158,11 @@ def test_kernel_contract_and_zero_upstream():
     r.upload_levels(lv, 2)
     r.set_workspace(32, 32, 1 << 20)
     z = torch.zeros((3, 32, 32), device="cuda")
+    r.render(cam, 1, 1, 1.0)
+    with pytest.raises(pkg.FlodError):                              # the forward pass must have ordered every list (FLOD_OPT_FULL_SORT)
+        r.render_backward(cam, z, 2)
+    r.set_options(pkg.FLOD_OPT_FULL_SORT)
+    r.set_workspace(32, 32, 1 << 20)                                # (forgets the frame)
     with pytest.raises(pkg.FlodError):                              # nothing rendered yet
         r.render_backward(cam, z, 2)
     r.render(cam, 1, 1, 1.0)

@@ -37,6 +37,7 @@ def _setup(config, width, height):
     r.upload_levels(scene.levels, scene.sh_degree)
     r.set_workspace(width, height, MAX_PAIRS)
     r.set_options(pkg.FLOD_OPT_DEBUG)
+    r.set_pair_rule(pkg.PAIR_RULE_ELLIPSE if config == 3 else pkg.PAIR_RULE_BOX)     # the rule that pays on each config
     return scene, osc, r
 
 
@@ -60,8 +61,15 @@ def test_config3_single_level(config3, l):
             print(f"config3 level {l} pose {pose}: P={fr.counts['n_pairs']} n_vis={fr.counts['n_vis']} "
                   f"max list={int(fr.tile_counts.max())} max|gpu-oracle|={res[0]:.2e} marginal={res[1]}")
     assert fr.counts["n_scan"] == scene.levels[l - 1].n
+    # the frame as bench.py renders it (no debug view: blend-driven ordering of the long lists) is the same image, bit for bit
+    import paper_2408_12894_b200 as pkg
+    dbg = r.render(cams[61], l, l, 1.0).cpu().numpy()
+    r.set_options(0)
+    try:
+        assert np.array_equal(r.render(cams[61], l, l, 1.0).cpu().numpy(), dbg)
+    finally:
+        r.set_options(pkg.FLOD_OPT_DEBUG)
     if l == 3:      # the box rule (R13) on the heaviest frame of the config
-        import paper_2408_12894_b200 as pkg
         r.set_pair_rule(pkg.PAIR_RULE_BOX)
         try:
             _, _, fr1 = check_frame(r, osc, cams[61], l, l, 1.0, image=False)

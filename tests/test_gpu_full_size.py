@@ -61,7 +61,7 @@ def test_config1_max_level_pose0_everything(full, rule):
     try:
         _config1_pose0(full)
     finally:
-        r.set_pair_rule(2)
+        r.set_pair_rule(1)
 
 
 def _config1_pose0(full):
@@ -103,8 +103,9 @@ def test_config2_selective_masks_and_counts_exact(full, gamma):
     assert per_level[0] == per_level[1] == 0 and sum(per_level[2:]) == st["n_sel"]
 
 
+@pytest.mark.parametrize("rule", [1, 2])
 @pytest.mark.parametrize("gamma", [1.0, 2.0, 4.0])
-def test_config2_sweep_all_poses_masks_and_counts_exact(full, gamma):
+def test_config2_sweep_all_poses_masks_and_counts_exact(full, gamma, rule):
     """BASELINE.json configs[2]'s contract: "the level-selection masks and per-tile pair counts are checked against the
     oracle exactly" on the 200 poses x gamma in {1,2,4}.  Geometry only on both sides (no image download, no stored
     lists in the oracle): masks, the five frame counters and the per-tile pair counts of every pose.
@@ -112,11 +113,15 @@ def test_config2_sweep_all_poses_masks_and_counts_exact(full, gamma):
     scene, cams, osc, r = full
     stride = int(os.environ.get("FLOD_SWEEP_STRIDE", "1"))
     n_sel = n_pairs = 0
-    for pose in range(0, len(cams), stride):
-        _, fr, st = _geometry_exact(r, osc, cams[pose], 3, 5, gamma, geometry_only=True)
-        n_sel += st["n_sel"]; n_pairs += st["n_pairs"]
+    r.set_pair_rule(rule)
+    try:
+        for pose in range(0, len(cams), stride):
+            _, fr, st = _geometry_exact(r, osc, cams[pose], 3, 5, gamma, geometry_only=True)
+            n_sel += st["n_sel"]; n_pairs += st["n_pairs"]
+    finally:
+        r.set_pair_rule(1)
     n = len(range(0, len(cams), stride))
-    print(f"config2 gamma {gamma}: {n} poses, 0 mismatches; mean N_sel {n_sel / n:.0f}, mean P {n_pairs / n:.0f}")
+    print(f"config2 gamma {gamma} pair rule {rule}: {n} poses, 0 mismatches; mean N_sel {n_sel / n:.0f}, mean P {n_pairs / n:.0f}")
 
 
 def test_single_levels_sweep(full):

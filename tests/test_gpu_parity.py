@@ -124,7 +124,7 @@ def test_config0_both_pair_rules(pkg, config0):
                 imgs[rule, ls] = img
                 pairs[rule, ls] = fr.counts["n_pairs"]
     finally:
-        r.set_pair_rule(pkg.PAIR_RULE_ELLIPSE)
+        r.set_pair_rule(pkg.PAIR_RULE_BOX)
     for ls in (2, 1):
         assert np.array_equal(imgs[1, ls], imgs[2, ls]) and pairs[2, ls] < 0.95 * pairs[1, ls]
     with pytest.raises(pkg.FlodError):
@@ -262,8 +262,41 @@ def test_sort_corner_cases_long_lists_and_depth_plateaus(pkg):
     cam = camera(width=64, height=48, f=100.0)
     r = make_renderer(pkg, [lv], 0, 64, 48, max_pairs=1 << 20)
     osc = OracleScene([lv], 0)
-    _, _, fr = check_frame(r, osc, cam, 1, 1, 1.0)
+    _, img_dbg, fr = check_frame(r, osc, cam, 1, 1, 1.0)
     assert fr.tile_counts.max() > 2 * 4096          # beyond the shared-memory path of the sort
+    # blend-driven ordering (the default without a debug view): long lists are ordered only as far as the blend reads
+    # them, in one or two rounds -- the image is the fully sorted frame's, bit for bit
+    for flags in (0, pkg.FLOD_OPT_FULL_SORT, pkg.FLOD_OPT_PROFILE):
+        r.set_options(flags)
+        assert np.array_equal(r.render(cam, 1, 1, 1.0).cpu().numpy(), img_dbg)
+    r.close()
+
+
+def test_blend_driven_ordering_two_rounds(pkg):
+    """Lists of six thousand faint Gaussians: the sorted prefix of the first round (the nearest slices, >= 1024 keys) is
+    not enough for most tiles, so the second round (k_tile_sort_rest, k_blend resuming from the saved pixel state) runs;
+    other tiles (opaque foreground) finish in the first.  Bit-identical to the fully sorted frame."""
+    rng = np.random.default_rng(88)
+    n_faint, n_front = 60000, 300
+    pos = np.column_stack([rng.uniform(-1.2, 1.2, (n_faint, 2)), rng.uniform(1.0, 40.0, n_faint)])
+    pos[:, :2] *= pos[:, 2:3] * 0.5
+    front = np.column_stack([rng.uniform(-0.25, 0.0, (n_front, 2)), rng.uniform(0.5, 0.9, n_front)])      # covers the upper-left tiles only
+    allpos = np.concatenate([pos, front])
+    scale = np.concatenate([0.03 * pos[:, 2:3] * np.ones((1, 3)), 0.05 * np.ones((n_front, 3))])
+    opac = np.concatenate([rng.uniform(0.01, 0.03, n_faint), np.full(n_front, 0.95)])
+    lv = level(1, 0.0, allpos, scale, opacity=opac, rgb=rng.uniform(0, 1, (len(allpos), 3)))
+    cam = camera(width=96, height=64, f=60.0, bg=(0.1, 0.1, 0.1))
+    r = make_renderer(pkg, [lv], 0, 96, 64, max_pairs=1 << 22)
+    osc = OracleScene([lv], 0)
+    (dmax, _), img_dbg, fr = check_frame(r, osc, cam, 1, 1, 1.0)
+    assert np.median(fr.tile_counts) > 4096 + 1024
+    _, E, B, T = fr.composite(stats=True)
+    assert (T > 1e-4).mean() > 0.3 and (T < 1e-4).mean() > 0.02      # both kinds of tiles exist
+    r.set_options(0)
+    for _ in range(2):
+        assert np.array_equal(r.render(cam, 1, 1, 1.0).cpu().numpy(), img_dbg)
+    # ... and strips of such a frame
+    assert np.array_equal(r.render_rows(cam, 1, 1, 1.0, 1, 3).cpu().numpy(), img_dbg[:, 16:48])
     r.close()
 
 
@@ -278,6 +311,7 @@ def test_needle_gaussians_stay_within_tolerance(pkg):
     cam = camera(width=640, height=400, f=600.0)
     r = make_renderer(pkg, [lv], 0, 640, 400)
     osc = OracleScene([lv], 0)
+    r.set_pair_rule(pkg.PAIR_RULE_ELLIPSE)
     (dmax, nm), img, fr = check_frame(r, osc, cam, 1, 1, 1.0)
     r.set_pair_rule(pkg.PAIR_RULE_BOX)
     _, img1, fr1 = check_frame(r, osc, cam, 1, 1, 1.0)
@@ -593,7 +627,7 @@ def test_tile_row_strips_stack_to_the_full_frame_bit_for_bit(pkg, config0, rule)
             r.render_rows(cam, 1, 2, 1.0, 3, 9)              # 128 px = 8 tile rows
         assert r.render_rows(cam, 1, 2, 1.0, 4, 4).shape == (3, 0, cam.width)
     finally:
-        r.set_pair_rule(pkg.PAIR_RULE_ELLIPSE)
+        r.set_pair_rule(pkg.PAIR_RULE_BOX)
 
 
 def test_tile_row_strips_on_a_ragged_image_with_large_footprints(pkg):
