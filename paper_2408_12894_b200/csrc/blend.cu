@@ -65,9 +65,8 @@ constexpr int kBlendMinBlocks = 8;                   // 64 registers per thread
 // (RESUME = true) takes the saved state up from where the first round stopped.  The per-pixel sequence of blends is the
 // one of a fully sorted list, so the image is bit-identical.
 template <bool COUNT, bool RESUME>
-__global__ void __launch_bounds__(kBlendThreads, kBlendMinBlocks)
-k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, int n_tiles,
-        float bg0, float bg1, float bg2, int tile0, int out_row0, int out_rows, int lazy)
+__device__ __forceinline__ void blend_tile(const WorkspaceDev &ws, float *__restrict__ out, int W, int H, int TX, int n_tiles,
+                                           float bg0, float bg1, float bg2, int tile, int out_row0, int out_rows, int lazy)
 {
     // staging, 36 bytes per Gaussian of the batch: A = (mu'x, mu'y, k, a2), B = (d2, log2 o, r, g), c = b
     __shared__ float4 s_A[2][kBatch], s_B[2][kBatch];           // double-buffered
@@ -76,7 +75,6 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
     __shared__ float4 s_buf[kBlendWarps][kWarpBuf * 3];
     __shared__ unsigned short s_idx[kBlendWarps][kWarpBuf];    // batch index of the survivor (counting variant only)
 
-    const int tile = tile0 + blockIdx.x;                // the grid covers the frame's strip of tile rows
     if (tile >= n_tiles || ws.hdr->overflow) return;   // an overflowed frame is undefined: its lists were not sorted
     const int tx = tile % TX, ty = tile / TX;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -239,8 +237,8 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
         if (__syncthreads_or(!(T.x < 1e-4f && T.y < 1e-4f))) {
             ws.tile_state[(size_t)tile * 256 + 2 * tid] = make_float4(T.x, cr.x, cg.x, cb2.x);
             ws.tile_state[(size_t)tile * 256 + 2 * tid + 1] = make_float4(T.y, cr.y, cg.y, cb2.y);
-            if (tid == 0) ws.lazy[tile].w = 1u;
-            return;                                     // k_blend<.., true> writes the pixels
+            if (tid == 0) { ws.lazy[tile].w = 1u; ws.todo[atomicAdd(&ws.hdr->n_todo, 1u)] = (unsigned int)tile; }
+            return;                                     // k_blend_rest writes the pixels
         }
     }
     const bool done0 = T.x < 1e-4f, done1 = T.y < 1e-4f;
@@ -270,16 +268,38 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
     }
 }
 
+template <bool COUNT>
+__global__ void __launch_bounds__(kBlendThreads, kBlendMinBlocks)
+k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, int n_tiles,
+        float bg0, float bg1, float bg2, int tile0, int out_row0, int out_rows, int lazy)
+{
+    // the grid covers the frame's strip of tile rows
+    blend_tile<COUNT, false>(ws, out, W, H, TX, n_tiles, bg0, bg1, bg2, tile0 + (int)blockIdx.x, out_row0, out_rows, lazy);
+}
+
+// Second round of blend-driven ordering: a small persistent grid walks the tiles that asked for the rest of their list
+// (ws.todo), so that a frame without any costs one short launch.
+__global__ void __launch_bounds__(kBlendThreads, kBlendMinBlocks)
+k_blend_rest(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, int n_tiles,
+             float bg0, float bg1, float bg2, int out_row0, int out_rows)
+{
+    const unsigned int n_todo = ws.hdr->n_todo;
+    for (unsigned int w = blockIdx.x; w < n_todo; w += gridDim.x) {
+        blend_tile<false, true>(ws, out, W, H, TX, n_tiles, bg0, bg1, bg2, (int)ws.todo[w], out_row0, out_rows, 1);
+        __syncthreads();                                // the staging buffers are reused by the next tile
+    }
+}
+
 int launch_blend(const Context &c, const FrameParams &p, float *out_rgb, cudaStream_t s)
 {
     const int tile0 = p.ty_begin * p.TX, n_tiles = p.ty_end * p.TX, grid = n_tiles - tile0;
     if (grid <= 0) return 0;
     if (c.flags & FLOD_OPT_COUNT)
-        k_blend<true, false><<<grid, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
-                                                            p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows, 0);
+        k_blend<true><<<grid, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
+                                                     p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows, 0);
     else
-        k_blend<false, false><<<grid, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
-                                                             p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows, p.lazy_sort);
+        k_blend<false><<<grid, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
+                                                      p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows, p.lazy_sort);
     return 1;
 }
 
@@ -288,8 +308,8 @@ int launch_blend_rest(const Context &c, const FrameParams &p, float *out_rgb, cu
 {
     const int tile0 = p.ty_begin * p.TX, n_tiles = p.ty_end * p.TX, grid = n_tiles - tile0;
     if (grid <= 0 || !p.lazy_sort) return 0;
-    k_blend<false, true><<<grid, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
-                                                        p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows, 1);
+    k_blend_rest<<<min(grid, 4 * c.sm_count), kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
+                                                                      p.bg[0], p.bg[1], p.bg[2], p.out_row0, p.out_rows);
     return 1;
 }
 

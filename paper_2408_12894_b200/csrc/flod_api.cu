@@ -132,6 +132,8 @@ WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_p
     L.ws.ovf_out = L.ws.ovf_slots + 2;
     L.ws.lazy = (uint4 *)take(tiles * sizeof(uint4));
     L.ws.slice_ends = (unsigned int *)take(tiles * kCoarseBins * sizeof(unsigned int));
+    L.ws.hint_state = (unsigned int *)take(sizeof(unsigned int));
+    L.ws.todo = (unsigned int *)take(tiles * sizeof(unsigned int));
     L.ws.tile_state = (float4 *)take(tiles * 256 * sizeof(float4));
     L.ws.image[0] = (float *)take((size_t)3 * w * h * sizeof(float));
     L.ws.image[1] = (float *)take((size_t)3 * w * h * sizeof(float));
@@ -172,7 +174,7 @@ int flod_create(flod_ctx **out, int device)
         ok &= cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming) == cudaSuccess;
     }
     // pinned words the device reports into: [0] N_sel of a rebuild, [1], [2] overflow flag of the frame in image[0], image[1]
-    ok &= cudaHostAlloc((void **)&c->sub_n_host, 64, cudaHostAllocDefault) == cudaSuccess;
+    ok &= cudaHostAlloc((void **)&c->sub_n_host, 64, cudaHostAllocMapped) == cudaSuccess;
     if (!ok) { flod_destroy(c); return FLOD_E_CUDA; }      // releases whatever was created
     memset(c->sub_n_host, 0, 64);
     *out = c;
@@ -326,6 +328,9 @@ int flod_set_workspace(flod_ctx *ctx, void *workspace_dev, size_t bytes, int wid
     for (int i = 0; i < 2; ++i)
         if (ctx->copy_pending[i]) { cudaEventSynchronize(ctx->ev_copied[i]); ctx->copy_pending[i] = false; }
     ctx->img_turn = 0;
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    CUDA_TRY(ctx, cudaMemset(ctx->ws.hint_state, 0, sizeof(unsigned int)));     // no hint yet about this workspace's frames
+    ctx->sub_n_host[3] = 0;
     ctx->has_ws = true; ctx->rendered = false;
     return FLOD_OK;
 }
@@ -360,8 +365,8 @@ int flod_launches_per_frame(const flod_ctx *ctx)
 {
     if (!ctx || !ctx->has_ws) return 0;
     // geometry, colour (+ tile scan in its block 0), duplication (two kernels, one of which exits), tile sort, blend; with
-    // blend-driven ordering also the second round of the last two (their CTAs exit at once unless a tile asked for it)
-    return (ctx->flags & (FLOD_OPT_DEBUG | FLOD_OPT_COUNT | FLOD_OPT_FULL_SORT)) ? 6 : 8;
+    // blend-driven ordering (frames that follow a frame with long lists) also the second round of the last two
+    return ctx->rendered && ctx->last_params.lazy_sort ? 8 : 6;
 }
 
 }  // extern "C"
@@ -435,11 +440,20 @@ int enqueue_frame(flod_ctx *ctx, const SceneDev &sc, FrameParams &p, float *out_
     const int64_t n_scan = p.n_scan;
     p.max_pairs = (unsigned int)ctx->max_pairs;
     p.pair_rule = ctx->pair_rule;
-    // blend-driven ordering of long lists, unless a view of the frame needs every list in its final order
-    p.lazy_sort = (ctx->flags & (FLOD_OPT_DEBUG | FLOD_OPT_COUNT | FLOD_OPT_FULL_SORT)) ? 0 : 1;
     p.quad_gid = p.first_gid & ~3ll;
     p.n_pre_blocks = (int)((p.first_gid - p.quad_gid + n_scan + kGeoBlock - 1) / kGeoBlock);
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    // Blend-driven ordering of long lists (two more launches), unless a view of the frame needs every list in its final
+    // order -- and only when the previous frames had lists longer than kSortCap at all: the tile scan leaves that in a
+    // mapped host word, read here without synchronisation.  It is a hint about cost, never about the result: either way
+    // the frame's image is the same, bit for bit.
+    {
+        unsigned int *hint_dev = nullptr;
+        CUDA_TRY(ctx, cudaHostGetDevicePointer((void **)&hint_dev, (void *)(ctx->sub_n_host + 3), 0));
+        ctx->ws.long_hint = hint_dev;
+    }
+    const bool allowed = !(ctx->flags & (FLOD_OPT_DEBUG | FLOD_OPT_COUNT | FLOD_OPT_FULL_SORT));
+    p.lazy_sort = (allowed && *(volatile unsigned int *)(ctx->sub_n_host + 3) != 0) ? 1 : 0;
     const bool prof = ctx->flags & FLOD_OPT_PROFILE;
     // zero the header and the tile difference grid (contiguous in the workspace)
     const size_t zero_bytes = (size_t)((unsigned char *)ctx->ws.tile_diff - (unsigned char *)ctx->ws.hdr) +

@@ -63,6 +63,8 @@ struct FrameHeader {
     unsigned int pad;
     unsigned long long n_sel, n_front, n_pairs;   // n_pairs = pairs the frame requires (sum of rect areas)
     unsigned long long evals, blends;
+    unsigned int n_todo;                  // blend-driven ordering: tiles whose first blend round asked for the rest of their list
+    unsigned int pad2[3];
 };
 
 // Everything per Gaussian is indexed by the POSITION p = segment * kGeoBlock + j: block `segment` of k_geometry
@@ -94,6 +96,10 @@ struct WorkspaceDev {
     uint4 *lazy;                          // [T_n] lists longer than kSortCap, blend-driven ordering: (keys in final order so far, next
                                           // slice to sort, slices, 1 = the blend wants the rest)
     unsigned int *slice_ends;             // [T_n][kCoarseBins] ends of the depth slices of those lists
+    unsigned int *long_hint;              // mapped pinned host word: 1 when a quarter of the frame's pairs sit in lists longer than kSortCap (tile scan);
+                                          // the host reads it, unsynchronised, as a hint for the NEXT frame (lazy ordering or not)
+    unsigned int *hint_state;             // device copy of what long_hint was last set to (| 0x100), zeroed by flod_set_workspace
+    unsigned int *todo;                   // [T_n] those tiles (hdr->n_todo of them), in the order they asked
     float4 *tile_state;                   // [T_n][256] (T, r, g, b) of every pixel of a tile the blend left unfinished
     float *image[2];                      // 2 x [3][H][W] for flod_render_to_host(_async): double-buffered so that the copy
                                           // of frame k overlaps the kernels of frame k + 1

@@ -15,8 +15,10 @@ namespace flod {
 __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, int TY, unsigned int max_pairs, bool rowwise)
 {
     __shared__ unsigned long long s_wtot[32];
+    __shared__ unsigned int s_long;                            // pairs that sit in lists longer than kSortCap (saturating)
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
     const int gw = TX + 1, gh = TY + 1;
+    if (tid == 0) s_long = 0;
     const int *__restrict__ diff = ws.tile_diff;
     int *cnt = ws.tile_cnt;
 
@@ -73,8 +75,10 @@ __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, 
         total += t;
     }
     unsigned int too_long = 0;
+    unsigned int in_long = 0;
     for (int t = t0; t < t1; ++t) {
         const unsigned int c = (unsigned int)cnt[(t / TX) * gw + (t % TX)];
+        if (c > (unsigned int)kSortCap) in_long += min(c, 1u << 20);
         const unsigned int a = (unsigned int)min(run, (unsigned long long)max_pairs);
         const unsigned int b = (unsigned int)min(run + c, (unsigned long long)max_pairs);
         ws.ranges[t] = make_uint2(a, b);
@@ -86,8 +90,15 @@ __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, 
     const int n_groups = ((TX + 1) / 2) * ((TY + 1) / 2);
     for (int g = tid; g < n_groups; g += nthr)
         *reinterpret_cast<float4 *>(ws.cursor4 + (size_t)g * kCtrStride) = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    in_long = __reduce_add_sync(0xffffffffu, min(in_long, 1u << 26));
+    if (lane == 0 && in_long) atomicAdd(&s_long, in_long);
     too_long = __syncthreads_or((int)too_long);
     if (tid == 0) {
+        // host memory, a hint for the next frame (flod_api.cu): blend-driven ordering pays when a good part of the pairs
+        // sits in long lists (a coarse level alone), not for a few crowded tiles of a fine level
+        // (written only when it changes: a store to host memory holds the kernel's completion back by microseconds)
+        const unsigned int hint = ((unsigned long long)s_long * 4ull >= total && s_long) ? 1u : 0u;
+        if (*ws.hint_state != (hint | 0x100u)) { *ws.hint_state = hint | 0x100u; *ws.long_hint = hint; }
         ws.hdr->n_pairs_clamped = (unsigned int)min(total, (unsigned long long)max_pairs);
         const unsigned int ovf = (total > max_pairs ? 1u : 0u) | (too_long ? 2u : 0u);
         ws.hdr->overflow = ovf;

@@ -261,27 +261,29 @@ k_tile_sort(const WorkspaceDev ws, int tile0, int n_tiles)
     }
 }
 
-// The rest of the lists whose tiles k_blend left unfinished (ws.lazy[tile].w set): slices next .. n of the coarse pass.
+// The rest of the lists whose tiles k_blend left unfinished (ws.todo): slices next .. n of the coarse pass.  A small
+// persistent grid walks the list of those tiles, so that a frame without any costs one short launch.
 __global__ void __launch_bounds__(kSortThreads, 4)
-k_tile_sort_rest(const WorkspaceDev ws, int tile0, int n_tiles)
+k_tile_sort_rest(const WorkspaceDev ws)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     SortSmem &S = *reinterpret_cast<SortSmem *>(smem_raw);
-    const int tile = tile0 + blockIdx.x;
-    if (tile >= n_tiles) return;
-    const uint2 rg = ws.ranges[tile];
-    if (rg.y - rg.x <= (unsigned int)kSortCap || ws.hdr->overflow) return;
-    const uint4 lz = ws.lazy[tile];
-    if (!lz.w) return;
+    const unsigned int n_todo = ws.hdr->n_todo;
     const int tid = threadIdx.x;
-    for (unsigned int i = tid; i < lz.z; i += kSortThreads) S.cends[i] = ws.slice_ends[(size_t)tile * kCoarseBins + i];
-    if (tid == 0) S.any_big[0] = 0;
-    __syncthreads();
-    u64 *pairs = ws.pairs + rg.x, *tmp = ws.pairs_tmp + rg.x;
-    uint32_t *vals = ws.vals + rg.x;
-    for (unsigned int b = lz.y; b < lz.z; ++b) {
-        const unsigned int lo = b ? S.cends[b - 1] : 0u;
-        sort_slice(pairs, tmp, vals, lo, S.cends[b] - lo, S, tid);
+    for (unsigned int w = blockIdx.x; w < n_todo; w += gridDim.x) {
+        const unsigned int tile = ws.todo[w];
+        const uint2 rg = ws.ranges[tile];
+        const uint4 lz = ws.lazy[tile];
+        __syncthreads();                                  // the previous tile's S.cends is no longer read
+        for (unsigned int i = tid; i < lz.z; i += kSortThreads) S.cends[i] = ws.slice_ends[(size_t)tile * kCoarseBins + i];
+        if (tid == 0) S.any_big[0] = 0;
+        __syncthreads();
+        u64 *pairs = ws.pairs + rg.x, *tmp = ws.pairs_tmp + rg.x;
+        uint32_t *vals = ws.vals + rg.x;
+        for (unsigned int b = lz.y; b < lz.z; ++b) {
+            const unsigned int lo = b ? S.cends[b - 1] : 0u;
+            sort_slice(pairs, tmp, vals, lo, S.cends[b] - lo, S, tid);
+        }
     }
 }
 
@@ -309,7 +311,7 @@ int launch_tile_sort_rest(const Context &c, const FrameParams &p, cudaStream_t s
 {
     const int tile0 = p.ty_begin * p.TX, n_tiles = p.ty_end * p.TX;
     if (p.n_pre_blocks <= 0 || n_tiles <= tile0 || !p.lazy_sort) return 0;
-    k_tile_sort_rest<<<n_tiles - tile0, kSortThreads, sizeof(SortSmem), s>>>(c.ws, tile0, n_tiles);
+    k_tile_sort_rest<<<min(n_tiles - tile0, 2 * c.sm_count), kSortThreads, sizeof(SortSmem), s>>>(c.ws);
     return 1;
 }
 
