@@ -42,6 +42,7 @@ k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned int seg = blockIdx.x;
+    cudaGridDependencySynchronize();
     const unsigned int n_here = ws.seg_count[seg];
     if (n_here == 0 || dup_large_rects(ws)) return;       // frames of large rects are served by k_duplicate_shared
     const unsigned int p0 = seg * kGeoBlock;
@@ -287,6 +288,7 @@ k_duplicate_shared(const WorkspaceDev ws, unsigned int TX, unsigned int T_n, uns
     __shared__ unsigned int s_segn[kDupSegRound];
     __shared__ unsigned int s_wtot[kDupSegRound / 32];
     __shared__ unsigned int s_row[kDupSWarps][32][2];   // per warp: (index of the first listed tile, its tile id) of 32 tile rows
+    cudaGridDependencySynchronize();
     if (!dup_large_rects(ws)) return;
     const unsigned int tid = threadIdx.x;
     for (unsigned int win0 = 0; win0 < T_n; win0 += win_cap) {
@@ -316,13 +318,13 @@ int launch_duplicate(const Context &c, const FrameParams &p, cudaStream_t s)
     const unsigned int T_n = (unsigned int)p.n_tiles;
     const unsigned int win_cap = (c.flags & FLOD_OPT_SMALL_WINDOWS) ? 1024u : min(T_n, (unsigned int)kDupWinCap);
     if (p.pair_rule == FLOD_PAIR_RULE_BOX) {
-        k_duplicate<false><<<p.n_pre_blocks, kPreBlock, 0, s>>>(c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs);
-        k_duplicate_shared<false><<<c.sm_count, kDupSThreads, win_cap * sizeof(unsigned int), s>>>(
-            c.ws, (unsigned int)p.TX, T_n, (unsigned int)p.n_pre_blocks, win_cap, p.max_pairs);
+        launch_pdl(k_duplicate<false>, p.n_pre_blocks, kPreBlock, 0, s, c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs);
+        launch_pdl(k_duplicate_shared<false>, c.sm_count, kDupSThreads, win_cap * sizeof(unsigned int), s,
+                   c.ws, (unsigned int)p.TX, T_n, (unsigned int)p.n_pre_blocks, win_cap, p.max_pairs);
     } else {
-        k_duplicate<true><<<p.n_pre_blocks, kPreBlock, 0, s>>>(c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs);
-        k_duplicate_shared<true><<<c.sm_count, kDupSThreads, win_cap * sizeof(unsigned int), s>>>(
-            c.ws, (unsigned int)p.TX, T_n, (unsigned int)p.n_pre_blocks, win_cap, p.max_pairs);
+        launch_pdl(k_duplicate<true>, p.n_pre_blocks, kPreBlock, 0, s, c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs);
+        launch_pdl(k_duplicate_shared<true>, c.sm_count, kDupSThreads, win_cap * sizeof(unsigned int), s,
+                   c.ws, (unsigned int)p.TX, T_n, (unsigned int)p.n_pre_blocks, win_cap, p.max_pairs);
     }
     return 2;
 }

@@ -274,6 +274,9 @@ k_blend(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, in
         float bg0, float bg1, float bg2, int tile0, int out_row0, int out_rows, int lazy)
 {
     // the grid covers the frame's strip of tile rows
+    cudaGridDependencySynchronize();
+    // the NEXT frame's counters start at zero (this frame's header stays for flod_get_stats)
+    if (blockIdx.x == 0 && threadIdx.x < sizeof(FrameHeader) / sizeof(unsigned int)) reinterpret_cast<unsigned int *>(ws.hdr_next)[threadIdx.x] = 0u;
     blend_tile<COUNT, false>(ws, out, W, H, TX, n_tiles, bg0, bg1, bg2, tile0 + (int)blockIdx.x, out_row0, out_rows, lazy);
 }
 
@@ -283,6 +286,7 @@ __global__ void __launch_bounds__(kBlendThreads, kBlendMinBlocks)
 k_blend_rest(const WorkspaceDev ws, float *__restrict__ out, int W, int H, int TX, int n_tiles,
              float bg0, float bg1, float bg2, int out_row0, int out_rows)
 {
+    cudaGridDependencySynchronize();
     const unsigned int n_todo = ws.hdr->n_todo;
     for (unsigned int w = blockIdx.x; w < n_todo; w += gridDim.x) {
         blend_tile<false, true>(ws, out, W, H, TX, n_tiles, bg0, bg1, bg2, (int)ws.todo[w], out_row0, out_rows, 1);
@@ -295,11 +299,11 @@ int launch_blend(const Context &c, const FrameParams &p, float *out_rgb, cudaStr
     const int tile0 = p.ty_begin * p.TX, n_tiles = p.ty_end * p.TX, grid = n_tiles - tile0;
     if (grid <= 0) return 0;
     if (c.flags & FLOD_OPT_COUNT)
-        k_blend<true><<<grid, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
-                                                     p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows, 0);
+        launch_pdl(k_blend<true>, grid, kBlendThreads, 0, s, c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
+                   p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows, 0);
     else
-        k_blend<false><<<grid, kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
-                                                      p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows, p.lazy_sort);
+        launch_pdl(k_blend<false>, grid, kBlendThreads, 0, s, c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
+                   p.bg[0], p.bg[1], p.bg[2], tile0, p.out_row0, p.out_rows, p.lazy_sort);
     return 1;
 }
 
@@ -308,8 +312,8 @@ int launch_blend_rest(const Context &c, const FrameParams &p, float *out_rgb, cu
 {
     const int tile0 = p.ty_begin * p.TX, n_tiles = p.ty_end * p.TX, grid = n_tiles - tile0;
     if (grid <= 0 || !p.lazy_sort) return 0;
-    k_blend_rest<<<min(grid, 4 * c.sm_count), kBlendThreads, 0, s>>>(c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
-                                                                      p.bg[0], p.bg[1], p.bg[2], p.out_row0, p.out_rows);
+    launch_pdl(k_blend_rest, min(grid, 4 * c.sm_count), kBlendThreads, 0, s, c.ws, out_rgb, p.W, p.H, p.TX, n_tiles,
+               p.bg[0], p.bg[1], p.bg[2], p.out_row0, p.out_rows);
     return 1;
 }
 

@@ -110,7 +110,9 @@ WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_p
     const size_t tx = (size_t)(w + kTile - 1) / kTile, ty = (size_t)(h + kTile - 1) / kTile;
     const size_t tiles = tx * ty;
     const size_t nt = (size_t)std::max<int64_t>(n_total, 1) + 2 * kGeoBlock;   // segment positions (see WorkspaceDev)
-    L.ws.hdr = (FrameHeader *)take(sizeof(FrameHeader));
+    L.ws.hdr2[0] = (FrameHeader *)take(sizeof(FrameHeader));
+    L.ws.hdr2[1] = (FrameHeader *)take(sizeof(FrameHeader));
+    L.ws.hdr = L.ws.hdr2[0]; L.ws.hdr_next = L.ws.hdr2[1];
     L.ws.tile_diff = (int *)take((tx + 1) * (ty + 1) * kCtrStride * sizeof(int));
     L.ws.seg_count = (unsigned int *)take((nt / kGeoBlock + 2) * sizeof(unsigned int));
     L.ws.tile_cnt = (int *)take((tx + 1) * (ty + 1) * sizeof(int));
@@ -330,6 +332,14 @@ int flod_set_workspace(flod_ctx *ctx, void *workspace_dev, size_t bytes, int wid
     ctx->img_turn = 0;
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     CUDA_TRY(ctx, cudaMemset(ctx->ws.hint_state, 0, sizeof(unsigned int)));     // no hint yet about this workspace's frames
+    // both frame headers and the difference grid start at zero; from then on the frames keep them so (FrameHeader's comment)
+    CUDA_TRY(ctx, cudaMemset(ctx->ws.hdr2[0], 0, sizeof(FrameHeader)));
+    CUDA_TRY(ctx, cudaMemset(ctx->ws.hdr2[1], 0, sizeof(FrameHeader)));
+    {
+        const size_t tx = (size_t)(width + kTile - 1) / kTile, ty = (size_t)(height + kTile - 1) / kTile;
+        CUDA_TRY(ctx, cudaMemset(ctx->ws.tile_diff, 0, (tx + 1) * (ty + 1) * kCtrStride * sizeof(int)));
+    }
+    ctx->hdr_turn = 1;
     ctx->sub_n_host[3] = 0;
     ctx->has_ws = true; ctx->rendered = false;
     return FLOD_OK;
@@ -455,10 +465,10 @@ int enqueue_frame(flod_ctx *ctx, const SceneDev &sc, FrameParams &p, float *out_
     const bool allowed = !(ctx->flags & (FLOD_OPT_DEBUG | FLOD_OPT_COUNT | FLOD_OPT_FULL_SORT));
     p.lazy_sort = (allowed && *(volatile unsigned int *)(ctx->sub_n_host + 3) != 0) ? 1 : 0;
     const bool prof = ctx->flags & FLOD_OPT_PROFILE;
-    // zero the header and the tile difference grid (contiguous in the workspace)
-    const size_t zero_bytes = (size_t)((unsigned char *)ctx->ws.tile_diff - (unsigned char *)ctx->ws.hdr) +
-                              (size_t)(p.TX + 1) * (p.TY + 1) * kCtrStride * sizeof(int);
-    CUDA_TRY(ctx, cudaMemsetAsync(ctx->ws.hdr, 0, zero_bytes, s));
+    // this frame's header was zeroed by the previous frame's k_blend (or by flod_set_workspace), the difference grid by
+    // the previous tile scan: no memset in the stream
+    ctx->hdr_turn ^= 1;
+    ctx->ws.hdr = ctx->ws.hdr2[ctx->hdr_turn]; ctx->ws.hdr_next = ctx->ws.hdr2[ctx->hdr_turn ^ 1];
     if (ctx->flags & FLOD_OPT_DEBUG)   // the mask is zero outside the scanned levels
         CUDA_TRY(ctx, cudaMemsetAsync(ctx->ws.mask, 0, (size_t)std::max<int64_t>(ctx->n_total, 1), s));
     int stage = 0;
@@ -467,7 +477,9 @@ int enqueue_frame(flod_ctx *ctx, const SceneDev &sc, FrameParams &p, float *out_
     mark(); launch_colour(*ctx, p, s);
     mark(); launch_duplicate(*ctx, p, s);
     mark(); launch_tile_sort(*ctx, p, s);
-    mark(); launch_blend(*ctx, p, out_rgb_dev, s);
+    mark();
+    if (launch_blend(*ctx, p, out_rgb_dev, s) == 0)      // (an empty strip launches no blend kernel: zero the next header here)
+        CUDA_TRY(ctx, cudaMemsetAsync(ctx->ws.hdr_next, 0, sizeof(FrameHeader), s));
     launch_tile_sort_rest(*ctx, p, s); launch_blend_rest(*ctx, p, out_rgb_dev, s);     // (both exit at once unless a tile asked)
     mark();
     CUDA_TRY(ctx, cudaGetLastError());

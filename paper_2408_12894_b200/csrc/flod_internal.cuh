@@ -55,7 +55,9 @@ struct SubsetParams {
     int n_blocks;
 };
 
-// Per-frame counters, zeroed (with the tile difference grid) by one memset at the start of every frame.
+// Per-frame counters.  Two of them alternate from frame to frame: k_blend of frame k zeroes the header of frame k + 1 (its
+// own is still wanted by flod_get_stats), the tile scan zeroes the cells of the difference grid as it reads them -- so a
+// frame starts without a memset in the stream, and k_geometry can be launched programmatically behind the previous frame.
 struct FrameHeader {
     unsigned int n_vis32;                 // visible Gaussians = length of the compact per-frame arrays
     unsigned int overflow;
@@ -73,7 +75,9 @@ struct FrameHeader {
 // sectors, and no inter-block scan is needed.  Blend features (DESIGN R25):
 //   gA = (mu'x, mu'y, k = B/A, -A log2(e)/2)     gB = (min(0, -(C - B^2/A) log2(e)/2), log2 o, r, g)    cB = b
 struct WorkspaceDev {
-    FrameHeader *hdr;
+    FrameHeader *hdr;                     // this frame's header (one of hdr2)
+    FrameHeader *hdr_next;                // the next frame's: zeroed by this frame's k_blend
+    FrameHeader *hdr2[2];
     int *tile_diff;                       // [(TX+1)*(TY+1)][kCtrStride] 2-D difference grid of the tile counts (zeroed per frame)
     unsigned int *seg_count;              // [geometry blocks] visible Gaussians of every segment
     int *tile_cnt;                        // [(TX+1)*(TY+1)] dense copy, used by the tile scan when the grid exceeds shared memory
@@ -166,6 +170,7 @@ struct Context {
     cudaEvent_t ev_copied[2] = {nullptr, nullptr};     // image[i] copied out on the copy stream (free to overwrite)
     bool copy_pending[2] = {false, false};
     int img_turn = 0;
+    int hdr_turn = 0;                     // which of ws.hdr2 the last frame used
     cudaStream_t last_copy_stream = nullptr;
     bool ev_valid = false;
     // materialised G_sel (subset.cu)
@@ -181,6 +186,21 @@ struct Context {
     cudaEvent_t ev_sub_read[2] = {nullptr, nullptr};   // last frame that read snap[i] (on the render stream)
     bool sub_read_pending[2] = {false, false};
 };
+
+// Launch with programmatic stream serialization (PDL): the kernel's CTAs may be scheduled while the previous kernel of the
+// stream is draining its last wave; every such kernel calls cudaGridDependencySynchronize() before it touches memory, so
+// the data dependence is the usual one -- what overlaps is the launch latency and the tail of the previous kernel.
+template <class... KArgs, class... Args>
+inline void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
 
 // kernel launchers (each enqueues on `s` and returns the number of kernels launched)
 int launch_geometry(const Context &c, const SceneDev &sc, const FrameParams &p, cudaStream_t s);   // a1-a3 + tile-count grid + visible list

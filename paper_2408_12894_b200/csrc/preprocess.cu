@@ -80,6 +80,7 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
     __shared__ GeoSmem S;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) { S.cnt[0] = 0; S.cnt[1] = 0; S.pairs = 0; }
+    cudaGridDependencySynchronize();                    // launched programmatically behind the previous frame's last kernel
     const int bid = blockIdx.x;
     const long long gb = p.quad_gid + (long long)bid * kGeoBlock;           // first gid of the block (multiple of 4)
     const long long g0 = gb + tid * kGeoPer;
@@ -339,6 +340,7 @@ __global__ void __launch_bounds__(256)
 k_colour(const SceneDev sc, const WorkspaceDev ws, int TX, int TY, unsigned int max_pairs, int pair_rule)
 {
     constexpr int K = (DEG + 1) * (DEG + 1);
+    cudaGridDependencySynchronize();
     if (blockIdx.x == 0) { tile_scan_block(ws, TX, TY, max_pairs, pair_rule != FLOD_PAIR_RULE_BOX); return; }
     const unsigned int sub = threadIdx.x % LANES;
     const unsigned int per_block = 256 / LANES;
@@ -429,11 +431,11 @@ int launch_geometry(const Context &c, const SceneDev &sc, const FrameParams &p, 
     if (p.n_pre_blocks <= 0) return 0;
     const bool ell = p.pair_rule != FLOD_PAIR_RULE_BOX;
     if (c.flags & FLOD_OPT_DEBUG) {
-        if (ell) k_geometry<true, true><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(sc, c.ws, p);
-        else k_geometry<true, false><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(sc, c.ws, p);
+        if (ell) launch_pdl(k_geometry<true, true>, p.n_pre_blocks, kGeoThreads, 0, s, sc, c.ws, p);
+        else launch_pdl(k_geometry<true, false>, p.n_pre_blocks, kGeoThreads, 0, s, sc, c.ws, p);
     } else {
-        if (ell) k_geometry<false, true><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(sc, c.ws, p);
-        else k_geometry<false, false><<<p.n_pre_blocks, kGeoThreads, 0, s>>>(sc, c.ws, p);
+        if (ell) launch_pdl(k_geometry<false, true>, p.n_pre_blocks, kGeoThreads, 0, s, sc, c.ws, p);
+        else launch_pdl(k_geometry<false, false>, p.n_pre_blocks, kGeoThreads, 0, s, sc, c.ws, p);
     }
     return 1;
 }
@@ -441,8 +443,8 @@ int launch_geometry(const Context &c, const SceneDev &sc, const FrameParams &p, 
 template <int DEG, int LANES>
 static void launch_colour_t(const Context &c, const FrameParams &p, int grid, cudaStream_t s)
 {
-    if (c.flags & FLOD_OPT_DEBUG) k_colour<DEG, LANES, true><<<grid, 256, 0, s>>>(c.scene, c.ws, p.TX, p.TY, p.max_pairs, p.pair_rule);
-    else k_colour<DEG, LANES, false><<<grid, 256, 0, s>>>(c.scene, c.ws, p.TX, p.TY, p.max_pairs, p.pair_rule);
+    if (c.flags & FLOD_OPT_DEBUG) launch_pdl(k_colour<DEG, LANES, true>, grid, 256, 0, s, c.scene, c.ws, p.TX, p.TY, p.max_pairs, p.pair_rule);
+    else launch_pdl(k_colour<DEG, LANES, false>, grid, 256, 0, s, c.scene, c.ws, p.TX, p.TY, p.max_pairs, p.pair_rule);
 }
 
 int launch_colour(const Context &c, const FrameParams &p, cudaStream_t s)

@@ -19,7 +19,7 @@ __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, 
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
     const int gw = TX + 1, gh = TY + 1;
     if (tid == 0) s_long = 0;
-    const int *__restrict__ diff = ws.tile_diff;
+    int *__restrict__ diff = ws.tile_diff;
     int *cnt = ws.tile_cnt;
 
     // ---- prefix along x: a warp owns a row, 32 cells per step, carry in a register
@@ -27,7 +27,8 @@ __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, 
         int carry = 0;
         for (int x0 = 0; x0 < gw; x0 += 32) {
             const int x = x0 + lane;
-            int v = x < gw ? diff[(size_t)(y * gw + x) * kCtrStride] : 0;
+            int v = 0;
+            if (x < gw) { v = diff[(size_t)(y * gw + x) * kCtrStride]; diff[(size_t)(y * gw + x) * kCtrStride] = 0; }   // read once: ready for the next frame
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
                 const int t = __shfl_up_sync(0xffffffffu, v, o);

@@ -231,6 +231,7 @@ k_tile_sort(const WorkspaceDev ws, int tile0, int n_tiles)
     const int tile = tile0 + blockIdx.x;               // the grid covers the frame's strip of tile rows
     if (tile >= n_tiles) return;
     const int tid = threadIdx.x;
+    cudaGridDependencySynchronize();
     const uint2 rg = ws.ranges[tile];
     const unsigned int L = rg.y - rg.x;
     if (L == 0 || ws.hdr->overflow) return;            // an overflowed frame is undefined (and its keys need not be unique)
@@ -268,6 +269,7 @@ k_tile_sort_rest(const WorkspaceDev ws)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     SortSmem &S = *reinterpret_cast<SortSmem *>(smem_raw);
+    cudaGridDependencySynchronize();
     const unsigned int n_todo = ws.hdr->n_todo;
     const int tid = threadIdx.x;
     for (unsigned int w = blockIdx.x; w < n_todo; w += gridDim.x) {
@@ -302,8 +304,8 @@ int launch_tile_sort(const Context &c, const FrameParams &p, cudaStream_t s)
     if (p.n_pre_blocks <= 0) return 0;
     const int tile0 = p.ty_begin * p.TX, n_tiles = p.ty_end * p.TX;
     if (n_tiles <= tile0) return 0;
-    if (p.lazy_sort) k_tile_sort<true><<<n_tiles - tile0, kSortThreads, sizeof(SortSmem), s>>>(c.ws, tile0, n_tiles);
-    else k_tile_sort<false><<<n_tiles - tile0, kSortThreads, sizeof(SortSmem), s>>>(c.ws, tile0, n_tiles);
+    if (p.lazy_sort) launch_pdl(k_tile_sort<true>, n_tiles - tile0, kSortThreads, sizeof(SortSmem), s, c.ws, tile0, n_tiles);
+    else launch_pdl(k_tile_sort<false>, n_tiles - tile0, kSortThreads, sizeof(SortSmem), s, c.ws, tile0, n_tiles);
     return 1;
 }
 
@@ -311,7 +313,7 @@ int launch_tile_sort_rest(const Context &c, const FrameParams &p, cudaStream_t s
 {
     const int tile0 = p.ty_begin * p.TX, n_tiles = p.ty_end * p.TX;
     if (p.n_pre_blocks <= 0 || n_tiles <= tile0 || !p.lazy_sort) return 0;
-    k_tile_sort_rest<<<min(n_tiles - tile0, 2 * c.sm_count), kSortThreads, sizeof(SortSmem), s>>>(c.ws);
+    launch_pdl(k_tile_sort_rest, min(n_tiles - tile0, 2 * c.sm_count), kSortThreads, sizeof(SortSmem), s, c.ws);
     return 1;
 }
 
