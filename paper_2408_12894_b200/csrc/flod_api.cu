@@ -46,7 +46,8 @@ constexpr int kScenePlanes = 3 + 6 + 4 + 8;   // mean xyz, cov x6, opacity, kapp
 size_t scene_bytes_for(int64_t n, int sh_degree)
 {
     size_t per_plane = align_up((size_t)std::max<int64_t>(n, 1) * sizeof(float));
-    return per_plane * kScenePlanes + align_up((size_t)std::max<int64_t>(n, 1) * sh_stride_for(sh_degree) * sizeof(float));
+    return per_plane * kScenePlanes + align_up((size_t)std::max<int64_t>(n, 1) * 8 * sizeof(float)) +
+           align_up((size_t)std::max<int64_t>(n, 1) * sh_stride_for(sh_degree) * sizeof(float));
 }
 
 // Step a0 for one Gaussian (DESIGN §2 "O0"; Eq. 1).  fp64 from the fp32 inputs, rounded once.
@@ -256,7 +257,8 @@ int flod_upload_levels(flod_ctx *ctx, int n_levels, const flod_level_desc *level
     std::vector<unsigned char> stage(total, 0);
     float *pl[kScenePlanes];
     for (int i = 0; i < kScenePlanes; ++i) pl[i] = (float *)(stage.data() + plane * i);
-    float *shp = (float *)(stage.data() + plane * kScenePlanes);
+    float *recp = (float *)(stage.data() + plane * kScenePlanes);
+    float *shp = recp + align_up(nn * 8 * sizeof(float)) / sizeof(float);
     int64_t base = 0;
     for (int l = 0; l < n_levels; ++l) {
         const flod_level_desc d = levels[l];
@@ -268,6 +270,8 @@ int flod_upload_levels(flod_ctx *ctx, int n_levels, const flod_level_desc *level
                 activate_one(d.log_scale + 3 * i, d.quat + 4 * i, d.opacity_logit[i], cov, &o, &kap, &l2o, &rho2);
                 for (int k = 0; k < 6; ++k) pl[3 + k][g] = cov[k];
                 pl[9][g] = o; pl[10][g] = kap; pl[11][g] = l2o; pl[12][g] = rho2;
+                for (int k = 0; k < 6; ++k) recp[8 * g + k] = cov[k];
+                recp[8 * g + 6] = kap; recp[8 * g + 7] = l2o;
                 for (int k = 0; k < 3; ++k) pl[13 + k][g] = d.log_scale[3 * i + k];
                 for (int k = 0; k < 4; ++k) pl[16 + k][g] = d.quat[4 * i + k];
                 pl[20][g] = d.opacity_logit[i];
@@ -301,7 +305,8 @@ int flod_upload_levels(flod_ctx *ctx, int n_levels, const flod_level_desc *level
     for (int k = 0; k < 6; ++k) ctx->scene.cov[k] = P(3 + k);
     ctx->scene.opacity = P(9); ctx->scene.kappa = P(10); ctx->scene.l2o = P(11); ctx->scene.rho2 = P(12);
     for (int k = 0; k < 8; ++k) ctx->scene.raw[k] = P(13 + k);
-    ctx->scene.sh = P(kScenePlanes);
+    ctx->scene.rec = (const float4 *)P(kScenePlanes);
+    ctx->scene.sh = (const float *)((const unsigned char *)P(kScenePlanes) + align_up(nn * 8 * sizeof(float)));
     ctx->scene.sh_stride = stride; ctx->scene.sh_degree = sh_degree;
     ctx->arena = scene_arena_dev;
     ctx->uploaded = true; ctx->has_ws = false; ctx->rendered = false; ctx->has_subset = false;
@@ -625,6 +630,7 @@ SubLayout carve_subset(unsigned char *base, int64_t n_range)
         L.snap[i].n_sel = (unsigned int *)take(sizeof(unsigned int));
         for (int a = 0; a < 13; ++a) L.snap[i].plane[a] = (float *)take(cap * sizeof(float));
         L.snap[i].src_gid = (unsigned int *)take(cap * sizeof(unsigned int));
+        L.snap[i].rec = (float4 *)take(cap * 8 * sizeof(float));
     }
     L.blk = (unsigned int *)take(((size_t)n_range / kGeoBlock + 4) * sizeof(unsigned int));
     L.bytes = off;
@@ -736,7 +742,7 @@ int flod_render_subset(flod_ctx *ctx, const flod_camera *cam, float *out_rgb_dev
     sc.mx = sn.plane[0]; sc.my = sn.plane[1]; sc.mz = sn.plane[2]; sc.rho2 = sn.plane[3]; sc.kappa = sn.plane[4];
     for (int k = 0; k < 6; ++k) sc.cov[k] = sn.plane[5 + k];
     sc.l2o = sn.plane[11]; sc.opacity = sn.plane[12];
-    sc.src_gid = sn.src_gid;
+    sc.src_gid = sn.src_gid; sc.rec = sn.rec;
     FrameParams p{};
     camera_params(p, cam);
     for (int i = 0; i < 3; ++i) p.ref[i] = p.centre[i];      // every entry of a snapshot is selected: one band [0, inf)

@@ -31,6 +31,9 @@ struct SceneDev {
     const float *kappa;                   // 2 ln(255 o); -1 when dead
     const float *l2o;                     // log2(o)
     const float *rho2;                    // kappa * largest eigenvalue of Sigma, rounded up (squared bounding radius); -1 when dead
+    const float4 *rec;                    // [n][2]: (Sxx, Sxy, Sxz, Syy), (Syz, Szz, kappa, log2 o) -- what phase 2 of k_geometry reads
+                                          // of a candidate, as ONE 32-byte sector (the planes above cost nine sectors, most
+                                          // of each unused at the 45 % density of the candidates)
     const float *raw[8];                  // the uploaded log_scale xyz, quat wxyz, opacity logit (read by the backward pass only)
     const float *sh;                      // [n][sh_stride] floats, row = K*3 coefficients padded to a multiple of 4
     int sh_stride;
@@ -42,6 +45,7 @@ struct SceneDev {
 struct SnapshotDev {
     float *plane[13];                     // mx, my, mz, rho2, kappa, cov[0..5], l2o, opacity
     unsigned int *src_gid;
+    float4 *rec;                          // [cap][2] as SceneDev::rec
     unsigned int *n_sel;                  // device copy of the count (written by the rebuild)
 };
 

@@ -192,10 +192,9 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
         if (s < n_cand) {
             g = gb + S.cand[s];
             wxk = __ldg(sc.mx + g); wyk = __ldg(sc.my + g); wzk = __ldg(sc.mz + g);
-            kap = __ldg(sc.kappa + g);
-            const float Sxx = __ldg(sc.cov[0] + g), Sxy = __ldg(sc.cov[1] + g), Sxz = __ldg(sc.cov[2] + g);
-            const float Syy = __ldg(sc.cov[3] + g), Syz = __ldg(sc.cov[4] + g), Szz = __ldg(sc.cov[5] + g);
-            l2o = __ldg(sc.l2o + g);
+            const float4 r0 = __ldg(sc.rec + 2 * g), r1 = __ldg(sc.rec + 2 * g + 1);      // one 32-byte sector
+            const float Sxx = r0.x, Sxy = r0.y, Sxz = r0.z, Syy = r0.w, Syz = r1.x, Szz = r1.y;
+            kap = r1.z; l2o = r1.w;
             const float px = fadd(fadd(fadd(fmul(R[0], wxk), fmul(R[1], wyk)), fmul(R[2], wzk)), p.t[0]);
             const float py = fadd(fadd(fadd(fmul(R[3], wxk), fmul(R[4], wyk)), fmul(R[5], wzk)), p.t[1]);
             z = fadd(fadd(fadd(fmul(R[6], wxk), fmul(R[7], wyk)), fmul(R[8], wzk)), p.t[2]);

@@ -120,6 +120,7 @@ k_subset_scatter(const SceneDev sc, const __grid_constant__ SubsetParams q, cons
 #pragma unroll
         for (int a = 0; a < 13; ++a) dst.plane[a][pos] = __ldg(src[a] + g);
         dst.src_gid[pos] = (unsigned int)g;
+        dst.rec[2 * (size_t)pos] = __ldg(sc.rec + 2 * g); dst.rec[2 * (size_t)pos + 1] = __ldg(sc.rec + 2 * g + 1);
         ++pos;
     }
 }
