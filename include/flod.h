@@ -207,7 +207,7 @@ FLOD_API int flod_wait_host(flod_ctx *ctx);
  * equals flod_render with flod_set_selection_reference(ref_pos) and the same fx and gamma, bit for bit. ---- */
 
 /* Bytes of a subset arena for the level range `mode` (two snapshots, each sized for every Gaussian of the range:
- * 60 B per Gaussian and snapshot; SH rows stay in the scene arena).  0 on invalid input or before upload. */
+ * 92 B per Gaussian and snapshot; SH rows stay in the scene arena).  0 on invalid input or before upload. */
 FLOD_API size_t flod_subset_bytes(const flod_ctx *ctx, flod_level_mode mode);
 
 /* Hand the subset arena (256-byte aligned device pointer, caller-owned) to the context and fix the level range. */
