@@ -16,6 +16,8 @@
 // exponent.  The filter bounds the very values the loop evaluates (same c_r, e0_r; rounding is monotone), so a
 // dropped Gaussian has alpha < 1/255 on every pixel of the strip and the image is bit-identical to the unfiltered
 // loop.  A warp whose 64 pixels have all terminated skips filter and loop; the CTA stops when every warp has.
+#include <type_traits>
+
 #include "flod_internal.cuh"
 
 namespace flod {
@@ -120,14 +122,18 @@ __device__ __forceinline__ void blend_tile(const WorkspaceDev &ws, float *__rest
 
     // evaluates my_buf[0, cnt) on the thread's two pixels.  a2 <= 0 and e0 <= log2 o (k_geometry clamps d2), so
     // q >= 0 holds by construction and alpha needs the 0.99 clamp only.  A pixel that is done or below 1/255 blends 0.
-    auto evaluate = [&](unsigned int cnt, unsigned int base_in_list) {
+    // CLAMP = false: no survivor of the buffer has o > 0.99 - margin (log2 o <= -0.0146), so alpha <= o stays below the
+    // 0.99 clamp and min(0.99, .) would return its argument: the same bits with two instructions less per entry.
+    auto evaluate = [&](unsigned int cnt, unsigned int base_in_list, auto clamp_tag) {
+        constexpr bool CLAMP = decltype(clamp_tag)::value;
 #pragma unroll kBlendUnroll
         for (unsigned int t = 0; t < cnt; ++t) {
             const float4 hrec = my_half[3 * t];
             const float4 c = my_buf[3 * t + 2];
             const float2 w = __fadd2_rn(make_float2(hrec.x, hrec.y), make_float2(nlx, nlx));
             const float2 e = __ffma2_rn(make_float2(c.x, c.x), __fmul2_rn(w, w), make_float2(hrec.z, hrec.w));
-            float al0 = fminf(ex2(e.x), 0.99f), al1 = fminf(ex2(e.y), 0.99f);
+            float al0 = ex2(e.x), al1 = ex2(e.y);
+            if (CLAMP) { al0 = fminf(al0, 0.99f); al1 = fminf(al1, 0.99f); }
             // skip below 1/255 (R11); a pixel that has stopped (T < 1e-4 after an earlier blend, R12) or lies outside
             // the image (T = 0 from the start) blends nothing.  The test reads T directly, so the loop-carried chain is
             // T -> compare -> select -> multiply -> subtract; one predicate per pixel carries both conditions.
@@ -191,11 +197,11 @@ __device__ __forceinline__ void blend_tile(const WorkspaceDev &ws, float *__rest
         const float4 *recA = s_A[b & 1], *recB = s_B[b & 1];
         const float *recC = s_c[b & 1];
 
-        unsigned int cnt = 0;
+        unsigned int cnt = 0, clampy = 0;                       // clampy: a survivor waiting in the buffer may reach the 0.99 clamp
         for (unsigned int j0 = 0; j0 < m; j0 += 32) {
             // ---- filter: can Gaussian j0 + lane reach alpha >= 1/255 somewhere on this warp's strip
             const unsigned int j = j0 + lane;
-            bool hit = false;
+            bool hit = false, near_one = false;
             float4 h0, h1, c;
             if (j < m) {
                 float4 a = recA[j];
@@ -212,6 +218,7 @@ __device__ __forceinline__ void blend_tile(const WorkspaceDev &ws, float *__rest
                 const float best = fmaxf(fmaxf(fmaf(a.w, w0 * w0, h0.z), fmaf(a.w, w1 * w1, h0.w)),
                                          fmaxf(fmaf(a.w, w2 * w2, h1.z), fmaf(a.w, w3 * w3, h1.w)));
                 hit = best >= kThr;
+                near_one = b.y > -0.0146f;                           // log2(0.99) = -0.014500, ex2.approx is good to 2^-22
                 c = make_float4(a.w, b.z, b.w, recC[j]);
             }
             const unsigned int bal = __ballot_sync(0xffffffffu, hit);
@@ -221,11 +228,13 @@ __device__ __forceinline__ void blend_tile(const WorkspaceDev &ws, float *__rest
                 if (COUNT) s_idx[warp][slot] = (unsigned short)j;
             }
             cnt += __popc(bal);
+            clampy |= __ballot_sync(0xffffffffu, hit && near_one);
             // ---- evaluate when the next step might not fit (or at the end of the batch)
             if (cnt > kFlush || j0 + 32 >= m) {
                 __syncwarp();
-                evaluate(cnt, base - rg.x);
-                cnt = 0;
+                if (clampy) evaluate(cnt, base - rg.x, std::true_type{});
+                else evaluate(cnt, base - rg.x, std::false_type{});
+                cnt = 0; clampy = 0;
                 warp_done = __all_sync(0xffffffffu, T.x < 1e-4f && T.y < 1e-4f);
                 if (warp_done) break;
                 __syncwarp();
