@@ -45,6 +45,7 @@ k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs)
     cudaGridDependencySynchronize();
     const unsigned int n_here = ws.seg_count[seg];
     if (n_here == 0 || dup_large_rects(ws)) return;       // frames of large rects are served by k_duplicate_shared
+    const bool absolute = ws.hdr->cursor_abs != 0u;
     const unsigned int p0 = seg * kGeoBlock;
     // thread t owns entries kDupPer t .. kDupPer t + kDupPer - 1 (consecutive, so that the scan is a plain block scan)
     unsigned int ng[kDupPer], mine = 0;
@@ -113,16 +114,17 @@ k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs)
             if (!(h00 || h10 || h01 || h11)) continue;
         }
         const float4 add = make_float4(h00 ? 1.0f : 0.0f, h10 ? 1.0f : 0.0f, h01 ? 1.0f : 0.0f, h11 ? 1.0f : 0.0f);
-        // the four range starts are fetched BEFORE the atomic, so that their L2 round trips overlap its latency
-        const unsigned int t00 = y * (unsigned int)TX + x;
-        const unsigned int s00 = h00 ? ws.ranges[t00].x : 0u, s10 = h10 ? ws.ranges[t00 + 1].x : 0u;
-        const unsigned int s01 = h01 ? ws.ranges[t00 + TX].x : 0u, s11 = h11 ? ws.ranges[t00 + TX + 1].x : 0u;
+        // absolute counters (tile_scan.cuh): the atomic returns the slots themselves; otherwise the four range starts come
+        // from the other half of the counters' sector, fetched BEFORE the atomic so that the round trips overlap
+        float *line = ws.cursor4 + (size_t)(gy * (unsigned int)GX + gx) * kCtrStride;
+        uint4 base = make_uint4(0u, 0u, 0u, 0u);
+        if (!absolute) base = *reinterpret_cast<const uint4 *>(line + 4);
         const unsigned long long key = ((unsigned long long)s_depth[r] << 32) | (p0 + r);
-        const float4 old = atomicAdd(reinterpret_cast<float4 *>(ws.cursor4 + (size_t)(gy * (unsigned int)GX + gx) * kCtrStride), add);
-        if (h00) { const unsigned int pos = s00 + (unsigned int)old.x; if (pos < max_pairs) ws.pairs[pos] = key; }
-        if (h10) { const unsigned int pos = s10 + (unsigned int)old.y; if (pos < max_pairs) ws.pairs[pos] = key; }
-        if (h01) { const unsigned int pos = s01 + (unsigned int)old.z; if (pos < max_pairs) ws.pairs[pos] = key; }
-        if (h11) { const unsigned int pos = s11 + (unsigned int)old.w; if (pos < max_pairs) ws.pairs[pos] = key; }
+        const float4 old = atomicAdd(reinterpret_cast<float4 *>(line), add);
+        if (h00) { const unsigned int pos = base.x + (unsigned int)old.x; if (pos < max_pairs) ws.pairs[pos] = key; }
+        if (h10) { const unsigned int pos = base.y + (unsigned int)old.y; if (pos < max_pairs) ws.pairs[pos] = key; }
+        if (h01) { const unsigned int pos = base.z + (unsigned int)old.z; if (pos < max_pairs) ws.pairs[pos] = key; }
+        if (h11) { const unsigned int pos = base.w + (unsigned int)old.w; if (pos < max_pairs) ws.pairs[pos] = key; }
     }
 }
 

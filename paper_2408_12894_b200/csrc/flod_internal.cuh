@@ -66,7 +66,7 @@ struct FrameHeader {
     unsigned int n_vis32;                 // visible Gaussians = length of the compact per-frame arrays
     unsigned int overflow;
     unsigned int n_pairs_clamped;         // min(n_pairs, max_pairs)
-    unsigned int pad;
+    unsigned int cursor_abs;              // k_duplicate's float counters hold absolute pair positions (the frame has <= 2^24 pairs)
     unsigned long long n_sel, n_front, n_pairs;   // n_pairs = pairs the frame requires (sum of rect areas)
     unsigned long long evals, blends;
     unsigned int n_todo;                  // blend-driven ordering: tiles whose first blend round asked for the rest of their list

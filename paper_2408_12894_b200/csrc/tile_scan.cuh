@@ -1,6 +1,6 @@
 // Steps a5 + a8: the 2-D prefix sum of the difference grid written by k_geometry = pairs per tile; the
 // exclusive scan over the tiles in row-major order = [start, end) of every tile's list (the ranges of step a8, known
-// before any pair exists) (the append counters of k_duplicate are zeroed here too).
+// before any pair exists); the append counters of k_duplicate are initialised here too.
 //
 // Run by ONE block of k_colour (block 0, so that it starts first): 65 KB of traffic and a few microseconds of pure
 // latency, hidden under the HBM-bound colour blocks instead of sitting on the critical path as a kernel of its own.
@@ -87,13 +87,25 @@ __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, 
         if (c > (1u << 24)) too_long = 1u;                     // k_duplicate counts a tile's entries in a float
         run += c;
     }
-    // the append counters of the 2x2 tile groups start at 0
-    const int n_groups = ((TX + 1) / 2) * ((TY + 1) / 2);
-    for (int g = tid; g < n_groups; g += nthr)
-        *reinterpret_cast<float4 *>(ws.cursor4 + (size_t)g * kCtrStride) = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     in_long = __reduce_add_sync(0xffffffffu, min(in_long, 1u << 26));
     if (lane == 0 && in_long) atomicAdd(&s_long, in_long);
     too_long = __syncthreads_or((int)too_long);
+    // The append counters of the 2x2 tile groups (one float4, the target of k_duplicate's one atomic per group).  A frame
+    // of at most 2^24 pairs counts in ABSOLUTE positions: the counters start at the tiles' range starts (exact as floats)
+    // and the atomic returns the slot itself.  A larger frame counts from 0 and k_duplicate adds the four range starts,
+    // kept as integers in the second half of the same 32-byte sector.  (ws.ranges of the whole image are visible here:
+    // the barrier above.)
+    const bool absolute = total <= (1ull << 24);
+    const int GXs = (TX + 1) / 2, n_groups = GXs * ((TY + 1) / 2);
+    for (int g = tid; g < n_groups; g += nthr) {
+        const int x = 2 * (g % GXs), y = 2 * (g / GXs);
+        const bool x1 = x + 1 < TX, y1 = y + 1 < TY;
+        const unsigned int s00 = ws.ranges[y * TX + x].x, s10 = x1 ? ws.ranges[y * TX + x + 1].x : 0u;
+        const unsigned int s01 = y1 ? ws.ranges[(y + 1) * TX + x].x : 0u, s11 = x1 && y1 ? ws.ranges[(y + 1) * TX + x + 1].x : 0u;
+        float4 *line = reinterpret_cast<float4 *>(ws.cursor4 + (size_t)g * kCtrStride);
+        line[0] = absolute ? make_float4((float)s00, (float)s10, (float)s01, (float)s11) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        reinterpret_cast<uint4 *>(line)[1] = absolute ? make_uint4(0u, 0u, 0u, 0u) : make_uint4(s00, s10, s01, s11);
+    }
     if (tid == 0) {
         // host memory, a hint for the next frame (flod_api.cu): blend-driven ordering pays when a good part of the pairs
         // sits in long lists (a coarse level alone), not for a few crowded tiles of a fine level
@@ -103,6 +115,7 @@ __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, 
         ws.hdr->n_pairs_clamped = (unsigned int)min(total, (unsigned long long)max_pairs);
         const unsigned int ovf = (total > max_pairs ? 1u : 0u) | (too_long ? 2u : 0u);
         ws.hdr->overflow = ovf;
+        ws.hdr->cursor_abs = absolute ? 1u : 0u;
         *ws.ovf_out = ovf;                                     // read back with the image by flod_render_to_host*
     }
 }
