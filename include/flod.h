@@ -35,7 +35,7 @@ extern "C" {
 #define FLOD_API
 #endif
 
-#define FLOD_ABI_VERSION 9
+#define FLOD_ABI_VERSION 10
 #define FLOD_MAX_LEVELS 16
 #define FLOD_TILE 16                 /* tiles are 16x16 pixels */
 #define FLOD_N_STAGES 5              /* 0 geometry (a1-a3), 1 colour (a4) with the tile scan (a5, a8) in one of its blocks,
@@ -49,7 +49,8 @@ enum {
     FLOD_E_ARENA_TOO_SMALL = -4,     /* scene arena or workspace smaller than flod_*_bytes() says */
     FLOD_E_CAPACITY = -5,            /* previous frame needed more pairs than max_pairs (reported by flod_get_stats) */
     FLOD_E_CUDA = -6,                /* CUDA runtime error; text in flod_last_error */
-    FLOD_E_NO_WORKSPACE = -7         /* flod_render before flod_set_workspace */
+    FLOD_E_NO_WORKSPACE = -7,        /* flod_render before flod_set_workspace */
+    FLOD_E_STATIC_LIMIT = -8         /* flod_overlap_prune_static: n > flod_overlap_prune_static_max_n() */
 };
 
 typedef struct flod_ctx flod_ctx;    /* opaque, host side */
@@ -269,6 +270,23 @@ FLOD_API int flod_render_backward(flod_ctx *ctx, const flod_camera *cam, const f
 FLOD_API size_t flod_overlap_prune_workspace_bytes(int64_t n);
 FLOD_API int flod_overlap_prune(const float *mean_dev, int64_t n, float s_min, const float bbox_lo[3], unsigned char *remove_dev,
                        float *mean_dist_dev, void *workspace_dev, size_t workspace_bytes, void *stream);
+
+/* The same operation for callers that cannot allocate device memory (code under CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): no workspace argument.  The scratch is a file-scope device array inside the library
+ * (8.0 MiB, held by every GPU that loads libflod.so until the process exits), which bounds the size:
+ * n <= flod_overlap_prune_static_max_n() = 262 144, else FLOD_E_STATIC_LIMIT (use flod_overlap_prune with a workspace).
+ * Same arguments, arithmetic and results as flod_overlap_prune; mean_dev, remove_dev, mean_dist_dev stay the caller's.
+ * The call runs no cudaMalloc / cudaFree and no allocating library routine: one cudaMemsetAsync (the bucket counters must
+ * start at zero; the rest of the array keeps the last call's contents and is overwritten before it is read) and four
+ * kernel launches on `stream`.  EVERY call on a device shares the one array: calls that overlap on the GPU (different
+ * streams without an ordering between them, or two host threads) race; calls on one stream are ordered and safe.
+ * The array's device address is asked from the runtime once per device, on the first call with that device current;
+ * flod_overlap_prune_static_setup() does just that ahead of time (call it, with the device current, before a stream
+ * capture begins).  Devices 0..63. */
+FLOD_API int64_t flod_overlap_prune_static_max_n(void);
+FLOD_API int flod_overlap_prune_static_setup(void);
+FLOD_API int flod_overlap_prune_static(const float *mean_dev, int64_t n, float s_min, const float bbox_lo[3],
+                                       unsigned char *remove_dev, float *mean_dist_dev, void *stream);
 
 FLOD_API const char *flod_last_error(const flod_ctx *ctx);
 FLOD_API int flod_abi_version(void);

@@ -22,7 +22,8 @@ PAIR_RULE_BOX, PAIR_RULE_ELLIPSE = 1, 2
 FLOD_N_STAGES = 5
 STAGE_NAMES = ("geometry", "colour", "duplicate", "tile_sort", "blend")
 ERRORS = {-1: "FLOD_E_INVALID_ARG", -2: "FLOD_E_LEVEL_RANGE", -3: "FLOD_E_NOT_UPLOADED",
-          -4: "FLOD_E_ARENA_TOO_SMALL", -5: "FLOD_E_CAPACITY", -6: "FLOD_E_CUDA", -7: "FLOD_E_NO_WORKSPACE"}
+          -4: "FLOD_E_ARENA_TOO_SMALL", -5: "FLOD_E_CAPACITY", -6: "FLOD_E_CUDA", -7: "FLOD_E_NO_WORKSPACE",
+          -8: "FLOD_E_STATIC_LIMIT"}
 
 
 class FlodError(RuntimeError):
@@ -116,6 +117,10 @@ def load_library():
     L.flod_overlap_prune_workspace_bytes.restype = sz
     L.flod_overlap_prune_workspace_bytes.argtypes = [i64]
     L.flod_overlap_prune.argtypes = [vp, i64, C.c_float, C.POINTER(C.c_float), vp, vp, vp, sz, vp]
+    L.flod_overlap_prune_static_max_n.restype = i64
+    L.flod_overlap_prune_static_max_n.argtypes = []
+    L.flod_overlap_prune_static_setup.argtypes = []
+    L.flod_overlap_prune_static.argtypes = [vp, i64, C.c_float, C.POINTER(C.c_float), vp, vp, vp]
     L.flod_last_error.restype = C.c_char_p
     L.flod_last_error.argtypes = [vp]
     L.flod_abi_version.restype = C.c_int
@@ -370,3 +375,32 @@ def overlap_prune(mean, s_min: float, with_distances: bool = True):
     if rc:
         raise FlodError(rc, "flod_overlap_prune rejected its arguments")
     return remove, dist
+
+
+def overlap_prune_static_max_n() -> int:
+    return int(load_library().flod_overlap_prune_static_max_n())
+
+
+def overlap_prune_static(mean, s_min: float, bbox_lo, remove, dist=None):
+    """flod_overlap_prune_static: overlap_prune without a workspace, for callers that may not allocate device memory.
+    The scratch is a fixed array inside the library, so n <= overlap_prune_static_max_n() (FlodError otherwise), and every
+    call on a device shares it: calls that overlap on the GPU race.  Nothing is allocated here either: the caller passes
+    bbox_lo (three floats <= every mean, componentwise) and the outputs `remove` (uint8 [n]) and `dist` (float32 [n] or
+    None), and the call is asynchronous on torch's current stream."""
+    import torch
+    if not (mean.is_cuda and mean.dtype == torch.float32 and mean.dim() == 2 and mean.shape[1] == 3 and mean.is_contiguous()):
+        raise ValueError("overlap_prune_static wants a contiguous CUDA float32 tensor of shape [n, 3]")
+    n = mean.shape[0]
+    if not (remove.is_cuda and remove.dtype == torch.uint8 and remove.numel() == n and remove.is_contiguous()):
+        raise ValueError("remove must be a contiguous CUDA uint8 tensor of n elements")
+    if dist is not None and not (dist.is_cuda and dist.dtype == torch.float32 and dist.numel() == n and dist.is_contiguous()):
+        raise ValueError("dist must be a contiguous CUDA float32 tensor of n elements")
+    lib = load_library()
+    with torch.cuda.device(mean.device):
+        rc = lib.flod_overlap_prune_static(C.c_void_p(mean.data_ptr()), n, float(s_min), (C.c_float * 3)(*[float(v) for v in bbox_lo]),
+                                           C.c_void_p(remove.data_ptr()), C.c_void_p(dist.data_ptr()) if dist is not None else None,
+                                           C.c_void_p(torch.cuda.current_stream(mean.device).cuda_stream))
+    if rc == -8:
+        raise FlodError(rc, f"n = {n} exceeds the built-in scratch (at most {overlap_prune_static_max_n()} points): use overlap_prune")
+    if rc:
+        raise FlodError(rc, "flod_overlap_prune_static rejected its arguments")

@@ -16,6 +16,8 @@
 // ((sqrt(a) + sqrt(b)) + sqrt(c)) / k with a <= b <= c, fp32; remove iff mean < 0.5f * s_min.
 #include <math.h>
 
+#include <mutex>
+
 #include "flod_internal.cuh"
 
 namespace flod {
@@ -171,6 +173,90 @@ int flod_overlap_prune(const float *mean_dev, int64_t n, float s_min, const floa
     k_knn_scan<<<1, 1024, 0, s>>>(count, start, m);
     k_knn_fill<<<grid, 256, 0, s>>>(n, g, cell, start, count, items);
     const float h2 = (float)(h * h) * 0.99999f;                       // (rounded down: "within h" must not be claimed too early)
+    k_knn_query<<<(unsigned int)((n + 127) / 128), 128, 0, s>>>(mean_dev, n, g, h2, d_op, cell, start, items, mean_dist_dev, remove_dev);
+    return cudaGetLastError() == cudaSuccess ? FLOD_OK : FLOD_E_CUDA;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------ no-allocation variant
+// flod_overlap_prune_static: the same four kernels on a scratch area that lives in the library's own device image, for
+// callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  The array below is
+// held by every GPU that loads libflod.so until the process exits (8.0 MiB: the workspace of kKnnStaticMaxN points).
+// In host code `g_knn_scratch` is a host-side stand-in for the symbol, NOT a device address: the address the kernels get
+// comes from cudaGetSymbolAddress, asked once per device with that device current (knn_static_setup).
+namespace {
+constexpr long long kKnnStaticMaxN = 1ll << 18;                                   // 262 144 points
+constexpr size_t knn_align_c(size_t v) { return (v + 255) / 256 * 256; }
+constexpr size_t kKnnStaticTable = 2 * (size_t)kKnnStaticMaxN;                    // knn_table_size(kKnnStaticMaxN)
+constexpr size_t kKnnStaticBytes = knn_align_c((size_t)kKnnStaticMaxN * sizeof(int3)) + 2 * knn_align_c((kKnnStaticTable + 1) * 4) +
+                                   knn_align_c((size_t)kKnnStaticMaxN * 4);
+static __device__ __align__(256) unsigned char g_knn_scratch[kKnnStaticBytes];
+
+constexpr int kKnnMaxDevices = 64;
+void *g_knn_scratch_ptr[kKnnMaxDevices];            // per device: the array's DEVICE address (null until set up)
+std::mutex g_knn_setup_mutex;
+
+// the device address of the scratch array on the CURRENT device; asked from the runtime once per device
+int knn_static_setup(void **ptr_out)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return FLOD_E_CUDA;
+    if (dev < 0 || dev >= kKnnMaxDevices) return FLOD_E_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_knn_setup_mutex);
+    if (!g_knn_scratch_ptr[dev]) {
+        void *ptr = nullptr;
+        if (cudaGetSymbolAddress(&ptr, g_knn_scratch) != cudaSuccess || !ptr) { cudaGetLastError(); return FLOD_E_CUDA; }
+        g_knn_scratch_ptr[dev] = ptr;
+    }
+    *ptr_out = g_knn_scratch_ptr[dev];
+    return FLOD_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int64_t flod_overlap_prune_static_max_n(void) { return kKnnStaticMaxN; }
+
+int flod_overlap_prune_static_setup(void)
+{
+    void *ptr = nullptr;
+    return knn_static_setup(&ptr);
+}
+
+int flod_overlap_prune_static(const float *mean_dev, int64_t n, float s_min, const float bbox_lo[3], unsigned char *remove_dev,
+                              float *mean_dist_dev, void *stream)
+{
+    if (n < 0 || !(s_min > 0.0f) || !isfinite(s_min) || !bbox_lo) return FLOD_E_INVALID_ARG;
+    if (n > kKnnStaticMaxN) return FLOD_E_STATIC_LIMIT;               // beyond the built-in scratch: use flod_overlap_prune
+    if (n == 0) return FLOD_OK;
+    if (!mean_dev || !remove_dev) return FLOD_E_INVALID_ARG;
+    for (int k = 0; k < 3; ++k) if (!isfinite(bbox_lo[k])) return FLOD_E_INVALID_ARG;
+    void *scratch = nullptr;
+    const int rc = knn_static_setup(&scratch);
+    if (rc != FLOD_OK) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    const float d_op = 0.5f * s_min;                                  // d_OP = s_min / 2
+    const double h = 3.0 * (double)d_op * (1.0 + 9.5367431640625e-7);
+    KnnGrid g;
+    for (int k = 0; k < 3; ++k) g.lo[k] = (double)bbox_lo[k];
+    g.inv_h = 1.0 / h;
+    const unsigned int m = knn_table_size(n);
+    g.mask = m - 1;
+    // the same carving as flod_overlap_prune's, sized by THIS call's n (at most kKnnStaticBytes by construction)
+    unsigned char *base = (unsigned char *)scratch;
+    int3 *cell = (int3 *)base;                  base += knn_align((size_t)n * sizeof(int3));
+    unsigned int *count = (unsigned int *)base; base += knn_align(((size_t)m + 1) * 4);
+    unsigned int *start = (unsigned int *)base; base += knn_align(((size_t)m + 1) * 4);
+    unsigned int *items = (unsigned int *)base;
+    // the array keeps the previous call's contents: the bucket counters are the one part that must start at zero
+    // (cell, start and items are written in full before they are read)
+    if (cudaMemsetAsync(count, 0, ((size_t)m + 1) * 4, s) != cudaSuccess) return FLOD_E_CUDA;
+    const unsigned int grid = (unsigned int)((n + 255) / 256);
+    k_knn_count<<<grid, 256, 0, s>>>(mean_dev, n, g, cell, count);
+    k_knn_scan<<<1, 1024, 0, s>>>(count, start, m);
+    k_knn_fill<<<grid, 256, 0, s>>>(n, g, cell, start, count, items);
+    const float h2 = (float)(h * h) * 0.99999f;
     k_knn_query<<<(unsigned int)((n + 127) / 128), 128, 0, s>>>(mean_dev, n, g, h2, d_op, cell, start, items, mean_dist_dev, remove_dev);
     return cudaGetLastError() == cudaSuccess ? FLOD_OK : FLOD_E_CUDA;
 }

@@ -25,7 +25,7 @@ def test_library_exports_every_declared_symbol(lib):
     assert len(names) >= 15 and "flod_upload_levels" in names and "flod_render" in names
     for n in names:
         assert hasattr(lib, n), f"libflod.so does not export {n}"
-    assert lib.flod_abi_version() == 9
+    assert lib.flod_abi_version() == 10
 
 
 def test_struct_layouts_match_the_c_compiler(lib):
