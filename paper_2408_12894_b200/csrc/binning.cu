@@ -114,11 +114,19 @@ k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs)
             if (!(h00 || h10 || h01 || h11)) continue;
         }
         const float4 add = make_float4(h00 ? 1.0f : 0.0f, h10 ? 1.0f : 0.0f, h01 ? 1.0f : 0.0f, h11 ? 1.0f : 0.0f);
-        // absolute counters (tile_scan.cuh): the atomic returns the slots themselves; otherwise the four range starts come
-        // from the other half of the counters' sector, fetched BEFORE the atomic so that the round trips overlap
+        // absolute counters (tile_scan.cuh): the atomic returns the slots themselves; otherwise the four range starts are
+        // fetched BEFORE the atomic, so that their L2 round trips overlap its latency (from ws.ranges: a copy next to the
+        // counters, in their sector or the neighbouring one, made the load wait for the atomics -- config 3, level 3:
+        // 229 -> 304 / 323 us)
         float *line = ws.cursor4 + (size_t)(gy * (unsigned int)GX + gx) * kCtrStride;
         uint4 base = make_uint4(0u, 0u, 0u, 0u);
-        if (!absolute) base = *reinterpret_cast<const uint4 *>(line + 4);
+        if (!absolute) {
+            const unsigned int t00 = y * (unsigned int)TX + x;
+            if (h00) base.x = ws.ranges[t00].x;
+            if (h10) base.y = ws.ranges[t00 + 1].x;
+            if (h01) base.z = ws.ranges[t00 + TX].x;
+            if (h11) base.w = ws.ranges[t00 + TX + 1].x;
+        }
         const unsigned long long key = ((unsigned long long)s_depth[r] << 32) | (p0 + r);
         const float4 old = atomicAdd(reinterpret_cast<float4 *>(line), add);
         if (h00) { const unsigned int pos = base.x + (unsigned int)old.x; if (pos < max_pairs) ws.pairs[pos] = key; }

@@ -92,9 +92,8 @@ __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, 
     too_long = __syncthreads_or((int)too_long);
     // The append counters of the 2x2 tile groups (one float4, the target of k_duplicate's one atomic per group).  A frame
     // of at most 2^24 pairs counts in ABSOLUTE positions: the counters start at the tiles' range starts (exact as floats)
-    // and the atomic returns the slot itself.  A larger frame counts from 0 and k_duplicate adds the four range starts,
-    // kept as integers in the second half of the same 32-byte sector.  (ws.ranges of the whole image are visible here:
-    // the barrier above.)
+    // and the atomic returns the slot itself.  A larger frame counts from 0 and k_duplicate adds the range starts it reads
+    // from ws.ranges.  (ws.ranges of the whole image are visible here: the barrier above.)
     const bool absolute = total <= (1ull << 24);
     const int GXs = (TX + 1) / 2, n_groups = GXs * ((TY + 1) / 2);
     for (int g = tid; g < n_groups; g += nthr) {
@@ -104,7 +103,6 @@ __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, 
         const unsigned int s01 = y1 ? ws.ranges[(y + 1) * TX + x].x : 0u, s11 = x1 && y1 ? ws.ranges[(y + 1) * TX + x + 1].x : 0u;
         float4 *line = reinterpret_cast<float4 *>(ws.cursor4 + (size_t)g * kCtrStride);
         line[0] = absolute ? make_float4((float)s00, (float)s10, (float)s01, (float)s11) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-        reinterpret_cast<uint4 *>(line)[1] = absolute ? make_uint4(0u, 0u, 0u, 0u) : make_uint4(s00, s10, s01, s11);
     }
     if (tid == 0) {
         // host memory, a hint for the next frame (flod_api.cu): blend-driven ordering pays when a good part of the pairs
