@@ -19,6 +19,7 @@ namespace flod {
 // capacity flag for a longer list).  A block scan of the per-Gaussian group counts lets the block expand its rects
 // cooperatively, one group per thread per step, whatever the individual rect sizes.
 constexpr int kDupPer = kGeoBlock / kPreBlock;
+constexpr int kDupMaxParts = 16;            // CTAs that may share a segment (launch_duplicate)
 
 // Which of the two duplication kernels serves the frame (both are launched, the other one exits at once): the mean
 // rect area, known on the device since k_geometry.  Small rects (config 1: 4.3 tiles per Gaussian): k_duplicate, one
@@ -33,7 +34,7 @@ __device__ __forceinline__ bool dup_large_rects(const WorkspaceDev &ws)
 
 template <bool ELLIPSE>
 __global__ void __launch_bounds__(kPreBlock)
-k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs)
+k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs, unsigned int parts)
 {
     __shared__ unsigned int s_warp_tot[kPreBlock / 32];
     __shared__ unsigned int s_incl[kGeoBlock];      // inclusive group scan of the segment
@@ -41,7 +42,10 @@ k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs)
     __shared__ unsigned int s_depth[kGeoBlock];     // depth bits
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const unsigned int seg = blockIdx.x;
+    // `parts` CTAs share a segment (all of them scan it, each expands every parts-th step of its groups): a frame of few
+    // segments with many tile groups each (config 3, level 3: 293 segments, 22 K groups per segment) would otherwise run
+    // two CTAs per SM with one atomic round trip per thread in flight
+    const unsigned int seg = blockIdx.x / parts, part = blockIdx.x % parts;
     cudaGridDependencySynchronize();
     const unsigned int n_here = ws.seg_count[seg];
     if (n_here == 0 || dup_large_rects(ws)) return;       // frames of large rects are served by k_duplicate_shared
@@ -84,7 +88,7 @@ k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs)
         if (j < n_here) s_incl[j] = run;
     }
     __syncthreads();
-    for (unsigned int q = tid; q < block_groups; q += kPreBlock) {
+    for (unsigned int q = part * kPreBlock + tid; q < block_groups; q += parts * kPreBlock) {
         int lo = 0, hi = (int)n_here - 1;              // first entry with s_incl[entry] > q
         while (lo < hi) {
             const int mid = (lo + hi) >> 1;
@@ -327,12 +331,14 @@ int launch_duplicate(const Context &c, const FrameParams &p, cudaStream_t s)
     if (p.n_pre_blocks <= 0) return 0;
     const unsigned int T_n = (unsigned int)p.n_tiles;
     const unsigned int win_cap = (c.flags & FLOD_OPT_SMALL_WINDOWS) ? 1024u : min(T_n, (unsigned int)kDupWinCap);
+    // CTAs per segment of k_duplicate: about 32 CTAs per SM when the frame has few segments (measured: 16 and 64 per SM are slower)
+    const unsigned int parts = (unsigned int)max(1, min(kDupMaxParts, 32 * c.sm_count / p.n_pre_blocks));
     if (p.pair_rule == FLOD_PAIR_RULE_BOX) {
-        launch_pdl(k_duplicate<false>, p.n_pre_blocks, kPreBlock, 0, s, c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs);
+        launch_pdl(k_duplicate<false>, p.n_pre_blocks * parts, kPreBlock, 0, s, c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs, parts);
         launch_pdl(k_duplicate_shared<false>, c.sm_count, kDupSThreads, win_cap * sizeof(unsigned int), s,
                    c.ws, (unsigned int)p.TX, T_n, (unsigned int)p.n_pre_blocks, win_cap, p.max_pairs);
     } else {
-        launch_pdl(k_duplicate<true>, p.n_pre_blocks, kPreBlock, 0, s, c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs);
+        launch_pdl(k_duplicate<true>, p.n_pre_blocks * parts, kPreBlock, 0, s, c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs, parts);
         launch_pdl(k_duplicate_shared<true>, c.sm_count, kDupSThreads, win_cap * sizeof(unsigned int), s,
                    c.ws, (unsigned int)p.TX, T_n, (unsigned int)p.n_pre_blocks, win_cap, p.max_pairs);
     }
