@@ -200,24 +200,33 @@ __device__ __forceinline__ void blend_tile(const WorkspaceDev &ws, float *__rest
         unsigned int cnt = 0, clampy = 0;                       // clampy: a survivor waiting in the buffer may reach the 0.99 clamp
         for (unsigned int j0 = 0; j0 < m; j0 += 32) {
             // ---- filter: can Gaussian j0 + lane reach alpha >= 1/255 somewhere on this warp's strip
-            const unsigned int j = j0 + lane;
-            bool hit = false, near_one = false;
+            // (a lane beyond the batch's end tests the last entry once more and drops it: no divergent region)
+            const unsigned int j = min(j0 + lane, m - 1u);
+            bool hit, near_one;
             float4 h0, h1, c;
-            if (j < m) {
+            {
                 float4 a = recA[j];
                 const float4 b = recB[j];
                 a.x -= x0c; a.y -= y0c;                              // relative to the tile's first pixel centre
-                const float dy0 = a.y - row0, dy1 = dy0 - 1.0f, dy2 = dy0 - 2.0f, dy3 = dy0 - 3.0f;
-                h0.x = fmaf(a.z, dy0, a.x); h0.y = fmaf(a.z, dy1, a.x);
-                h1.x = fmaf(a.z, dy2, a.x); h1.y = fmaf(a.z, dy3, a.x);
-                h0.z = fmaf(b.x, dy0 * dy0, b.y); h0.w = fmaf(b.x, dy1 * dy1, b.y);
-                h1.z = fmaf(b.x, dy2 * dy2, b.y); h1.w = fmaf(b.x, dy3 * dy3, b.y);
+                // the four rows as two packed pairs (FADD2 / FMUL2 / FFMA2: the kernel is bound by issue slots, and a
+                // packed instruction is the same IEEE operation on both halves -- same bits as the scalar sequence)
+                const float dy0 = a.y - row0;
+                const float2 dyA = make_float2(dy0, dy0 - 1.0f), dyB = __fadd2_rn(make_float2(dy0, dy0), make_float2(-2.0f, -3.0f));
+                const float2 kk = make_float2(a.z, a.z), ax = make_float2(a.x, a.x);
+                const float2 cA = __ffma2_rn(kk, dyA, ax), cB2 = __ffma2_rn(kk, dyB, ax);
+                const float2 dd = make_float2(b.x, b.x), lo = make_float2(b.y, b.y);
+                const float2 eA = __ffma2_rn(dd, __fmul2_rn(dyA, dyA), lo), eB = __ffma2_rn(dd, __fmul2_rn(dyB, dyB), lo);
+                h0 = make_float4(cA.x, cA.y, eA.x, eA.y);
+                h1 = make_float4(cB2.x, cB2.y, eB.x, eB.y);
                 // min over the row's 16 pixel columns x = 0..15 of |c_r - x|
-                const float w0 = fmaxf(fmaxf(h0.x - 15.0f, -h0.x), 0.0f), w1 = fmaxf(fmaxf(h0.y - 15.0f, -h0.y), 0.0f);
-                const float w2 = fmaxf(fmaxf(h1.x - 15.0f, -h1.x), 0.0f), w3 = fmaxf(fmaxf(h1.y - 15.0f, -h1.y), 0.0f);
-                const float best = fmaxf(fmaxf(fmaf(a.w, w0 * w0, h0.z), fmaf(a.w, w1 * w1, h0.w)),
-                                         fmaxf(fmaf(a.w, w2 * w2, h1.z), fmaf(a.w, w3 * w3, h1.w)));
-                hit = best >= kThr;
+                const float2 m15 = make_float2(-15.0f, -15.0f);
+                const float2 tA = __fadd2_rn(cA, m15), tB = __fadd2_rn(cB2, m15);
+                const float2 wA = make_float2(fmaxf(fmaxf(tA.x, -cA.x), 0.0f), fmaxf(fmaxf(tA.y, -cA.y), 0.0f));
+                const float2 wB = make_float2(fmaxf(fmaxf(tB.x, -cB2.x), 0.0f), fmaxf(fmaxf(tB.y, -cB2.y), 0.0f));
+                const float2 aa = make_float2(a.w, a.w);
+                const float2 bA = __ffma2_rn(aa, __fmul2_rn(wA, wA), eA), bB = __ffma2_rn(aa, __fmul2_rn(wB, wB), eB);
+                const float best = fmaxf(fmaxf(bA.x, bA.y), fmaxf(bB.x, bB.y));
+                hit = best >= kThr && j0 + lane < m;
                 near_one = b.y > -0.0146f;                           // log2(0.99) = -0.014500, ex2.approx is good to 2^-22
                 c = make_float4(a.w, b.z, b.w, recC[j]);
             }
