@@ -120,6 +120,7 @@ WsLayout carve(unsigned char *base, int64_t n_total, int w, int h, int64_t max_p
     L.ws.ranges = (uint2 *)take(tiles * sizeof(uint2));
     L.ws.cursor4 = (float *)take(((tx + 1) / 2) * ((ty + 1) / 2) * kCtrStride * sizeof(float));
     L.ws.cursor = (unsigned int *)take(tiles * sizeof(unsigned int));
+    L.ws.cnt4 = (float *)take(((tx + 1) / 2) * ((ty + 1) / 2) * kCtrStride * sizeof(float));
     L.ws.gA = (float4 *)take(nt * sizeof(float4));
     L.ws.gB = (float4 *)take(nt * sizeof(float4));
     L.ws.cB = (float *)take(nt * sizeof(float));
@@ -343,6 +344,7 @@ int flod_set_workspace(flod_ctx *ctx, void *workspace_dev, size_t bytes, int wid
     {
         const size_t tx = (size_t)(width + kTile - 1) / kTile, ty = (size_t)(height + kTile - 1) / kTile;
         CUDA_TRY(ctx, cudaMemset(ctx->ws.tile_diff, 0, (tx + 1) * (ty + 1) * kCtrStride * sizeof(int)));
+        CUDA_TRY(ctx, cudaMemset(ctx->ws.cnt4, 0, ((tx + 1) / 2) * ((ty + 1) / 2) * kCtrStride * sizeof(float)));
     }
     ctx->hdr_turn = 1;
     ctx->sub_n_host[3] = 0;

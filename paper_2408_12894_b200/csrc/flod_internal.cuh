@@ -89,6 +89,8 @@ struct WorkspaceDev {
     float *cursor4;                       // [ceil(TX/2) * ceil(TY/2)][kCtrStride] first 4 floats: entries appended so far to the
                                           // lists of the 2x2 tile group (x, y), (x+1, y), (x, y+1), (x+1, y+1); zeroed by the tile scan
     unsigned int *cursor;                 // [T_n] the same per tile, dense (k_duplicate_shared); zeroed by the tile scan
+    float *cnt4;                          // [ceil(TX/2) * ceil(TY/2)][kCtrStride] first 4 floats: pairs of the group's four tiles that
+                                          // come from rects of at most 2x2 groups (k_geometry, pair rule 1); read and zeroed by the tile scan
     float4 *gA, *gB;                      // [n_total + 2 kGeoBlock]
     float *cB;                            // [n_total + 2 kGeoBlock]
     float4 *dirgid;                       // [n_total + 2 kGeoBlock] (mu - c_cam, gid bits): input of the colour kernel

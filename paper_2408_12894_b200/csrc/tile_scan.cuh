@@ -55,6 +55,21 @@ __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, 
         }
     }
     __syncthreads();
+    // ---- plus the pairs of the small rects, which k_geometry counted per 2x2 tile group (read once: ready for the next frame)
+    {
+        const int GXs = (TX + 1) / 2, n_groups = GXs * ((TY + 1) / 2);
+        for (int g = tid; g < n_groups; g += nthr) {
+            float4 *line = reinterpret_cast<float4 *>(ws.cnt4 + (size_t)g * kCtrStride);
+            const float4 c = *line;
+            *line = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            const int x = 2 * (g % GXs), y = 2 * (g / GXs);
+            cnt[y * gw + x] += (int)c.x;                       // (cells of the grid's last row / column hold 0: a rect ends inside the image)
+            cnt[y * gw + x + 1] += (int)c.y;
+            cnt[(y + 1) * gw + x] += (int)c.z;
+            cnt[(y + 1) * gw + x + 1] += (int)c.w;
+        }
+    }
+    __syncthreads();
     // ---- exclusive scan over the tiles; a thread owns a contiguous chunk
     const int T_n = TX * TY;
     const int per = (T_n + nthr - 1) / nthr;
@@ -84,7 +99,7 @@ __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, 
         const unsigned int b = (unsigned int)min(run + c, (unsigned long long)max_pairs);
         ws.ranges[t] = make_uint2(a, b);
         ws.cursor[t] = 0;                                      // k_duplicate_shared: entries appended so far
-        if (c > (1u << 24)) too_long = 1u;                     // k_duplicate counts a tile's entries in a float
+        if (c >= (1u << 24)) too_long = 1u;                    // k_geometry and k_duplicate count a tile's entries in a float
         run += c;
     }
     in_long = __reduce_add_sync(0xffffffffu, min(in_long, 1u << 26));
