@@ -296,14 +296,18 @@ k_geometry(const SceneDev sc, const WorkspaceDev ws, const __grid_constant__ Fra
                 // grid: four reductions whatever its area.  The tile scan sums the two.
                 const int gx0 = tx0 >> 1, gx1 = (tx1 + 1) >> 1, gy0 = ty0 >> 1, gy1 = (ty1 + 1) >> 1;
                 if (gx1 - gx0 <= 2 && gy1 - gy0 <= 2) {
+                    // straight-line over the (up to) four groups: which of a group's two tile columns / rows the rect covers
                     const int GX = (p.TX + 1) >> 1;
-                    for (int gy = gy0; gy < gy1; ++gy)
-                        for (int gx = gx0; gx < gx1; ++gx) {
-                            const int x = 2 * gx, y = 2 * gy;
-                            const bool cx0 = x >= tx0, cx1 = x + 1 < tx1, cy0 = y >= ty0, cy1 = y + 1 < ty1;
-                            red_add_f32x4(ws.cnt4 + (size_t)(gy * GX + gx) * kCtrStride, cx0 && cy0 ? 1.0f : 0.0f,
-                                          cx1 && cy0 ? 1.0f : 0.0f, cx0 && cy1 ? 1.0f : 0.0f, cx1 && cy1 ? 1.0f : 0.0f);
-                        }
+                    const float xa0 = 2 * gx0 >= tx0 ? 1.0f : 0.0f, xa1 = 2 * gx0 + 1 < tx1 ? 1.0f : 0.0f;      // first group column
+                    const float xb1 = 2 * gx0 + 3 < tx1 ? 1.0f : 0.0f;                                          // second (its first tile is covered)
+                    const float ya0 = 2 * gy0 >= ty0 ? 1.0f : 0.0f, ya1 = 2 * gy0 + 1 < ty1 ? 1.0f : 0.0f;
+                    const float yb1 = 2 * gy0 + 3 < ty1 ? 1.0f : 0.0f;
+                    const bool two_x = gx1 - gx0 == 2, two_y = gy1 - gy0 == 2;
+                    float *g00 = ws.cnt4 + (size_t)(gy0 * GX + gx0) * kCtrStride;
+                    red_add_f32x4(g00, xa0 * ya0, xa1 * ya0, xa0 * ya1, xa1 * ya1);
+                    if (two_x) red_add_f32x4(g00 + kCtrStride, ya0, xb1 * ya0, ya1, xb1 * ya1);
+                    if (two_y) red_add_f32x4(g00 + (size_t)GX * kCtrStride, xa0, xa1, xa0 * yb1, xa1 * yb1);
+                    if (two_x && two_y) red_add_f32x4(g00 + (size_t)(GX + 1) * kCtrStride, 1.0f, xb1, yb1, xb1 * yb1);
                 } else {
                     atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx0) * kCtrStride, 1);
                     atomicAdd(ws.tile_diff + (size_t)(ty0 * gw + tx1) * kCtrStride, -1);
@@ -368,8 +372,10 @@ k_colour(const SceneDev sc, const WorkspaceDev ws, int TX, int TY, unsigned int 
     const unsigned int seg = blockIdx.x - 1;             // one block per segment of k_geometry
     const unsigned int n_here = ws.seg_count[seg];
     // U Gaussians per lane group and step: the U direction records are loaded first, then the U SH rows, then the
-    // arithmetic -- two dependent round trips to memory per step instead of per Gaussian
-    constexpr int U = 2;
+    // arithmetic.  (U = 2 -- two dependent round trips per step instead of per Gaussian -- was worth 2 us in round 1;
+    // with evict-first rows and programmatic launch U = 1 measures 59.5 against 61.0 us on config 1, 97 against 102 on
+    // config 4 at 1920x1080, 48.4 against 47.4 on config 3 level 5)
+    constexpr int U = 1;
     for (unsigned int j0 = 0; j0 < n_here; j0 += U * per_block) {
         bool ok[U];
         unsigned int ci[U];
