@@ -207,6 +207,44 @@ def test_random_scenes(pkg, seed, counts, wh, deg):
     r.close()
 
 
+def test_tile_counts_of_rects_across_tile_group_boundaries(pkg):
+    """Step a5: k_geometry counts the tiles of a rect of at most 2x2 groups of 2x2 tiles in per-group float4 counters
+    and those of a larger rect in the 2-D difference grid (DESIGN 6.1); the tile scan sums the two.  Isotropic Gaussians
+    of graded sizes at controlled screen positions produce every combination of rect origin parity and rect extent
+    1..6 tiles in x and y, on an image whose tile grid is odd in both directions (a group column / row hangs over the
+    edge).  Per-tile counts, the sorted sequence and the image against the oracle, both pair rules, and a strip."""
+    f, z, W, H = 100.0, 10.0, 201, 171                       # 13 x 11 tiles
+    means, scales = [], []
+    for ext in (0.02, 0.35, 0.8, 1.3, 1.9, 2.6):             # alpha = 1/255 radius from about 1 to about 45 pixels
+        for ty in range(0, 11, 1):
+            for tx in range(0, 13, 1):
+                # a centre near a tile corner, near a tile centre, near a group corner -- per size another offset
+                ox, oy = [(1.0, 1.0), (8.0, 8.0), (15.0, 3.0), (4.0, 15.5), (0.2, 9.0), (12.0, 0.3)][int(ext * 10) % 6]
+                u, v = 16.0 * tx + ox, 16.0 * ty + oy
+                means.append(((u - W / 2.0) * z / f, (v - H / 2.0) * z / f, z + 0.001 * len(means)))
+                scales.append(ext)
+    means, scales = np.array(means), np.array(scales)[:, None] * np.ones(3)
+    rng = np.random.default_rng(5)
+    lv = [level(1, 0.0, means, scales, opacity=rng.uniform(0.05, 0.95, len(means)), rgb=rng.uniform(0, 1, (len(means), 3)))]
+    cam = camera(width=W, height=H, f=f, bg=(0.1, 0.2, 0.3))
+    osc = OracleScene(lv, 0)
+    r = make_renderer(pkg, lv, 0, W, H, max_pairs=1 << 21)
+    for rule in (pkg.PAIR_RULE_BOX, pkg.PAIR_RULE_ELLIPSE):
+        r.set_pair_rule(rule)
+        (dmax, nm), img, fr = check_frame(r, osc, cam, 1, 1, 1.0)
+        rc = fr.rect[fr.state == oracle.ST_VISIBLE].astype(np.int64)
+        gw, gh = (rc[:, 2] + 1) // 2 - rc[:, 0] // 2, (rc[:, 3] + 1) // 2 - rc[:, 1] // 2
+        small = (gw <= 2) & (gh <= 2)
+        assert small.sum() > 200 and (~small).sum() > 200            # both counting paths are exercised
+        shapes = {(int(a[0]) & 1, int(a[1]) & 1, int(a[2] - a[0]), int(a[3] - a[1])) for a in rc}
+        assert len(shapes) > 60                                      # origin parities x extents
+    r.set_pair_rule(pkg.PAIR_RULE_BOX)
+    full = r.render(cam, 1, 1, 1.0).cpu().numpy()
+    img, _ = _assemble_strips(r, cam, 1, 1, 1.0, 3)                  # strips that begin on odd tile rows
+    assert np.array_equal(img, full)
+    r.close()
+
+
 def test_empty_scene_and_all_culled(pkg):
     """nothing to draw -> background; also everything behind the camera / dead."""
     lv = level(1, 0.0, np.zeros((0, 3)), 0.1)
