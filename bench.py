@@ -363,6 +363,7 @@ def run_ours(args):
     e1.record()
     barrier()
     ms = e0.elapsed_time(e1)
+    launches = r.launches_per_frame()          # of the timed frames (the diagnostic passes below launch differently)
     # ---- timed region 2: end to end through flod_render_to_host_async (host camera struct in, pinned host image out
     # every frame; kernels on the current stream, copies on a second caller-owned stream so that the copy of frame k
     # overlaps the kernels of frame k + 1; two pinned buffers alternate), closed by flod_wait_host
@@ -420,7 +421,6 @@ def run_ours(args):
         E += st["evals"]; B += st["blends"]
     E /= n_diag; B /= n_diag
     r.set_options(0)
-    launches = r.launches_per_frame()
     peak_mem = torch.cuda.max_memory_allocated(r.device)
 
     if rank != 0:

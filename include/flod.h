@@ -238,7 +238,8 @@ FLOD_API int flod_get_stats(flod_ctx *ctx, flod_stats *out);
  * size implied by the selector; see the FLOD_DBG_* comments. */
 FLOD_API int flod_debug_copy(flod_ctx *ctx, int what, void *host_dst, size_t bytes);
 
-/* Number of kernel launches flod_render enqueues per frame with the current options. */
+/* Number of kernel launches the last flod_render enqueued (5 to 8: one more after frames of large rects, two more after
+ * frames of long lists; 6 before the first frame). */
 FLOD_API int flod_launches_per_frame(const flod_ctx *ctx);
 
 /* ---- Training-side kernels.  They need no context: all arrays are caller-owned device memory. ---- */

@@ -26,7 +26,6 @@ constexpr int kDupMaxParts = 16;            // CTAs that may share a segment (la
 // value-returning global atomic per 2x2 tile group.  Large rects (a coarse level alone: hundreds of tiles per
 // Gaussian on a few hundred counters): those atomics serialise on their addresses (config 3, level 1: 979 us), so
 // k_duplicate_shared counts in shared memory and goes to the global counters once per block and tile.
-constexpr unsigned int kDupLargeArea = 128;
 __device__ __forceinline__ bool dup_large_rects(const WorkspaceDev &ws)
 {
     return ws.hdr->n_pairs > (unsigned long long)kDupLargeArea * ws.hdr->n_vis32;
@@ -34,7 +33,7 @@ __device__ __forceinline__ bool dup_large_rects(const WorkspaceDev &ws)
 
 template <bool ELLIPSE>
 __global__ void __launch_bounds__(kPreBlock)
-k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs, unsigned int parts)
+k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs, unsigned int parts, int alone)
 {
     __shared__ unsigned int s_warp_tot[kPreBlock / 32];
     __shared__ unsigned int s_incl[kGeoBlock];      // inclusive group scan of the segment
@@ -48,7 +47,7 @@ k_duplicate(const WorkspaceDev ws, int TX, int GX, unsigned int max_pairs, unsig
     const unsigned int seg = blockIdx.x / parts, part = blockIdx.x % parts;
     cudaGridDependencySynchronize();
     const unsigned int n_here = ws.seg_count[seg];
-    if (n_here == 0 || dup_large_rects(ws)) return;       // frames of large rects are served by k_duplicate_shared
+    if (n_here == 0 || (!alone && dup_large_rects(ws))) return;   // frames of large rects are served by k_duplicate_shared, if it was launched
     const bool absolute = ws.hdr->cursor_abs != 0u;
     const unsigned int p0 = seg * kGeoBlock;
     // thread t owns entries kDupPer t .. kDupPer t + kDupPer - 1 (consecutive, so that the scan is a plain block scan)
@@ -333,16 +332,22 @@ int launch_duplicate(const Context &c, const FrameParams &p, cudaStream_t s)
     const unsigned int win_cap = (c.flags & FLOD_OPT_SMALL_WINDOWS) ? 1024u : min(T_n, (unsigned int)kDupWinCap);
     // CTAs per segment of k_duplicate: about 32 CTAs per SM when the frame has few segments (measured: 16 and 64 per SM are slower)
     const unsigned int parts = (unsigned int)max(1, min(kDupMaxParts, 32 * c.sm_count / p.n_pre_blocks));
+    // Frames of small rects (the hint of the previous frames' tile scans, flod_api.cu) launch k_duplicate alone, and it serves
+    // the frame whatever its rects are: a kernel that only finds out that it has nothing to do still costs its place in
+    // the chain of dependent launches.  After a frame of large rects both are launched and the device picks.
+    const int alone = p.dup_both ? 0 : 1;
     if (p.pair_rule == FLOD_PAIR_RULE_BOX) {
-        launch_pdl(k_duplicate<false>, p.n_pre_blocks * parts, kPreBlock, 0, s, c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs, parts);
-        launch_pdl(k_duplicate_shared<false>, c.sm_count, kDupSThreads, win_cap * sizeof(unsigned int), s,
-                   c.ws, (unsigned int)p.TX, T_n, (unsigned int)p.n_pre_blocks, win_cap, p.max_pairs);
+        launch_pdl(k_duplicate<false>, p.n_pre_blocks * parts, kPreBlock, 0, s, c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs, parts, alone);
+        if (!alone)
+            launch_pdl(k_duplicate_shared<false>, c.sm_count, kDupSThreads, win_cap * sizeof(unsigned int), s,
+                       c.ws, (unsigned int)p.TX, T_n, (unsigned int)p.n_pre_blocks, win_cap, p.max_pairs);
     } else {
-        launch_pdl(k_duplicate<true>, p.n_pre_blocks * parts, kPreBlock, 0, s, c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs, parts);
-        launch_pdl(k_duplicate_shared<true>, c.sm_count, kDupSThreads, win_cap * sizeof(unsigned int), s,
-                   c.ws, (unsigned int)p.TX, T_n, (unsigned int)p.n_pre_blocks, win_cap, p.max_pairs);
+        launch_pdl(k_duplicate<true>, p.n_pre_blocks * parts, kPreBlock, 0, s, c.ws, p.TX, (p.TX + 1) / 2, p.max_pairs, parts, alone);
+        if (!alone)
+            launch_pdl(k_duplicate_shared<true>, c.sm_count, kDupSThreads, win_cap * sizeof(unsigned int), s,
+                       c.ws, (unsigned int)p.TX, T_n, (unsigned int)p.n_pre_blocks, win_cap, p.max_pairs);
     }
-    return 2;
+    return alone ? 1 : 2;
 }
 
 }  // namespace flod

@@ -381,9 +381,11 @@ int flod_set_pair_rule(flod_ctx *ctx, int rule)
 int flod_launches_per_frame(const flod_ctx *ctx)
 {
     if (!ctx || !ctx->has_ws) return 0;
-    // geometry, colour (+ tile scan in its block 0), duplication (two kernels, one of which exits), tile sort, blend; with
-    // blend-driven ordering (frames that follow a frame with long lists) also the second round of the last two
-    return ctx->rendered && ctx->last_params.lazy_sort ? 8 : 6;
+    // geometry, colour (+ tile scan in its block 0), duplication (one kernel; two, one of which exits, on frames that follow
+    // a frame of large rects), tile sort, blend; with blend-driven ordering (frames that follow a frame with long lists)
+    // also the second round of the last two
+    if (!ctx->rendered) return 6;
+    return 5 + (ctx->last_params.dup_both ? 1 : 0) + (ctx->last_params.lazy_sort ? 2 : 0);
 }
 
 }  // extern "C"
@@ -470,7 +472,9 @@ int enqueue_frame(flod_ctx *ctx, const SceneDev &sc, FrameParams &p, float *out_
         ctx->ws.long_hint = hint_dev;
     }
     const bool allowed = !(ctx->flags & (FLOD_OPT_DEBUG | FLOD_OPT_COUNT | FLOD_OPT_FULL_SORT));
-    p.lazy_sort = (allowed && *(volatile unsigned int *)(ctx->sub_n_host + 3) != 0) ? 1 : 0;
+    const unsigned int hint = *(volatile unsigned int *)(ctx->sub_n_host + 3);
+    p.lazy_sort = (allowed && (hint & 1u)) ? 1 : 0;
+    p.dup_both = (!(hint & 0x100u) || (hint & 2u)) ? 1 : 0;       // (no hint yet about this workspace's frames: both)
     const bool prof = ctx->flags & FLOD_OPT_PROFILE;
     // this frame's header was zeroed by the previous frame's k_blend (or by flod_set_workspace), the difference grid by
     // the previous tile scan: no memset in the stream

@@ -20,6 +20,7 @@ static_assert(kGeoPer % 4 == 0 && kGeoPer * kGeoThreads == 1024, "whole quads pe
 constexpr int kGeoBlock = kGeoThreads * kGeoPer;
 constexpr int kSortCap = 4096;            // per-tile sort: lists up to this many keys are scattered into shared memory
 constexpr int kCoarseBins = 256;          // ... longer ones are first cut into at most this many depth slices
+constexpr unsigned int kDupLargeArea = 128;   // duplication: frames whose mean rect exceeds this many tiles are served by k_duplicate_shared
 constexpr int kCtrStride = 64;            // ints between two per-tile atomic counters: one counter per 256 B, so that the
                                           // L2 slices share the atomic traffic (a dense 16 KB grid sits on a few slices)
 
@@ -106,7 +107,8 @@ struct WorkspaceDev {
     uint4 *lazy;                          // [T_n] lists longer than kSortCap, blend-driven ordering: (keys in final order so far, next
                                           // slice to sort, slices, 1 = the blend wants the rest)
     unsigned int *slice_ends;             // [T_n][kCoarseBins] ends of the depth slices of those lists
-    unsigned int *long_hint;              // mapped pinned host word: 1 when a quarter of the frame's pairs sit in lists longer than kSortCap (tile scan);
+    unsigned int *long_hint;              // mapped pinned host word, written by the tile scan when it changes: bit 0 = a quarter of the frame's pairs sit in
+                                          // lists longer than kSortCap, bit 1 = the frame's rects are large (dup_large_rects): hints about cost for the next frames
                                           // the host reads it, unsynchronised, as a hint for the NEXT frame (lazy ordering or not)
     unsigned int *hint_state;             // device copy of what long_hint was last set to (| 0x100), zeroed by flod_set_workspace
     unsigned int *todo;                   // [T_n] those tiles (hdr->n_todo of them), in the order they asked
@@ -139,6 +141,8 @@ struct FrameParams {
                                           // clipped to it, tiles outside it get no pairs and are not blended
     int out_row0, out_rows;               // out_rgb holds image rows [out_row0, out_row0 + out_rows) of every colour plane
     int lazy_sort;                        // blend-driven ordering of long lists (off for the debug / counting / training views)
+    int dup_both;                         // both duplication kernels are launched and the device picks (the previous frames had
+                                          // large rects); otherwise k_duplicate alone serves the frame, whatever its rects
 };
 
 struct Context {
