@@ -100,8 +100,9 @@ enum {                               /* flod_set_options bits */
     FLOD_OPT_DEBUG   = 1,            /* also write the selection mask and per-Gaussian projection records */
     FLOD_OPT_PROFILE = 2,            /* record CUDA events between stages (flod_get_stats reports ms) */
     FLOD_OPT_COUNT   = 4,            /* instrumented blend kernel counting evaluations and blends */
-    FLOD_OPT_SMALL_WINDOWS = 8,      /* test knob: the large-rect duplication kernel walks the tiles in windows of 1024 (the
-                                        path an image of more than 48 Ki tiles takes) */
+    FLOD_OPT_SMALL_WINDOWS = 8,      /* test knob: the large-rect duplication kernel serves frames from a mean rect of 128 tiles
+                                        (default: 1024) and walks the tiles in windows of 1024 (the path an image of more
+                                        than 48 Ki tiles takes) */
     FLOD_OPT_FULL_SORT = 16          /* order every tile list completely.  By default a list of more than 4096 pairs is ordered
                                         only as far as the blend reads it (nearest depth slices first, the rest if pixels of
                                         the tile are still alive): same image bit for bit.  FLOD_OPT_DEBUG and FLOD_OPT_COUNT

@@ -21,14 +21,15 @@ namespace flod {
 constexpr int kDupPer = kGeoBlock / kPreBlock;
 constexpr int kDupMaxParts = 16;            // CTAs that may share a segment (launch_duplicate)
 
-// Which of the two duplication kernels serves the frame (both are launched, the other one exits at once): the mean
-// rect area, known on the device since k_geometry.  Small rects (config 1: 4.3 tiles per Gaussian): k_duplicate, one
-// value-returning global atomic per 2x2 tile group.  Large rects (a coarse level alone: hundreds of tiles per
-// Gaussian on a few hundred counters): those atomics serialise on their addresses (config 3, level 1: 979 us), so
-// k_duplicate_shared counts in shared memory and goes to the global counters once per block and tile.
+// Which of the two duplication kernels serves the frame (when both are launched, the other one exits at once): the mean
+// rect area, known on the device since k_geometry.  k_duplicate: one value-returning global atomic per 2x2 tile group.
+// With one CTA per segment it was slow on a coarse level alone (hundreds of tiles per Gaussian, few segments: config 3,
+// level 1, 979 us), which is what k_duplicate_shared -- counts in shared memory, one global reservation per block and
+// tile -- was written for (270 us there); since up to 16 CTAs share a segment k_duplicate takes 142 us on that frame, so
+// the shared-counter kernel is left with the frames of VERY large rects (ws.dup_large_area, flod_internal.cuh).
 __device__ __forceinline__ bool dup_large_rects(const WorkspaceDev &ws)
 {
-    return ws.hdr->n_pairs > (unsigned long long)kDupLargeArea * ws.hdr->n_vis32;
+    return ws.hdr->n_pairs > (unsigned long long)ws.dup_large_area * ws.hdr->n_vis32;
 }
 
 template <bool ELLIPSE>

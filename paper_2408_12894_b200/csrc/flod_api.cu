@@ -472,6 +472,7 @@ int enqueue_frame(flod_ctx *ctx, const SceneDev &sc, FrameParams &p, float *out_
         ctx->ws.long_hint = hint_dev;
     }
     const bool allowed = !(ctx->flags & (FLOD_OPT_DEBUG | FLOD_OPT_COUNT | FLOD_OPT_FULL_SORT));
+    ctx->ws.dup_large_area = (ctx->flags & FLOD_OPT_SMALL_WINDOWS) ? kDupLargeAreaTest : kDupLargeArea;
     const unsigned int hint = *(volatile unsigned int *)(ctx->sub_n_host + 3);
     p.lazy_sort = (allowed && (hint & 1u)) ? 1 : 0;
     p.dup_both = (!(hint & 0x100u) || (hint & 2u)) ? 1 : 0;       // (no hint yet about this workspace's frames: both)

@@ -20,7 +20,10 @@ static_assert(kGeoPer % 4 == 0 && kGeoPer * kGeoThreads == 1024, "whole quads pe
 constexpr int kGeoBlock = kGeoThreads * kGeoPer;
 constexpr int kSortCap = 4096;            // per-tile sort: lists up to this many keys are scattered into shared memory
 constexpr int kCoarseBins = 256;          // ... longer ones are first cut into at most this many depth slices
-constexpr unsigned int kDupLargeArea = 128;   // duplication: frames whose mean rect exceeds this many tiles are served by k_duplicate_shared
+// duplication: frames whose mean rect exceeds this many tiles are served by k_duplicate_shared (since several CTAs share a
+// segment in k_duplicate it wins far beyond the 128 of round 1 -- config 3, level 1, mean rect 548 tiles: 240 -> 142 us,
+// level 2, mean 210: 306 -> 198 us); FLOD_OPT_SMALL_WINDOWS keeps the old threshold, for the tests of that kernel
+constexpr unsigned int kDupLargeArea = 1024, kDupLargeAreaTest = 128;
 constexpr int kCtrStride = 64;            // ints between two per-tile atomic counters: one counter per 256 B, so that the
                                           // L2 slices share the atomic traffic (a dense 16 KB grid sits on a few slices)
 
@@ -90,6 +93,7 @@ struct WorkspaceDev {
     float *cursor4;                       // [ceil(TX/2) * ceil(TY/2)][kCtrStride] first 4 floats: entries appended so far to the
                                           // lists of the 2x2 tile group (x, y), (x+1, y), (x, y+1), (x+1, y+1); zeroed by the tile scan
     unsigned int *cursor;                 // [T_n] the same per tile, dense (k_duplicate_shared); zeroed by the tile scan
+    unsigned int dup_large_area;          // kDupLargeArea, or kDupLargeAreaTest under FLOD_OPT_SMALL_WINDOWS (set per frame by the host)
     float *cnt4;                          // [ceil(TX/2) * ceil(TY/2)][kCtrStride] first 4 floats: pairs of the group's four tiles that
                                           // come from rects of at most 2x2 groups (k_geometry, pair rule 1); read and zeroed by the tile scan
     float4 *gA, *gB;                      // [n_total + 2 kGeoBlock]

@@ -123,9 +123,9 @@ __device__ __forceinline__ void tile_scan_block(const WorkspaceDev &ws, int TX, 
         // host memory, a hint for the next frame (flod_api.cu): blend-driven ordering pays when a good part of the pairs
         // sits in long lists (a coarse level alone), not for a few crowded tiles of a fine level
         // (written only when it changes: a store to host memory holds the kernel's completion back by microseconds)
-        // (bit 1: the frame's mean rect exceeds kDupLargeArea tiles -- the next frames launch k_duplicate_shared as well)
+        // (bit 1: the frame's mean rect exceeds ws.dup_large_area tiles -- the next frames launch k_duplicate_shared as well)
         const unsigned int hint = (((unsigned long long)s_long * 4ull >= total && s_long) ? 1u : 0u) |
-                                  (total > (unsigned long long)kDupLargeArea * ws.hdr->n_vis32 ? 2u : 0u);
+                                  (total > (unsigned long long)ws.dup_large_area * ws.hdr->n_vis32 ? 2u : 0u);
         if (*ws.hint_state != (hint | 0x100u)) { *ws.hint_state = hint | 0x100u; *ws.long_hint = hint | 0x100u; }   // 0x100: a hint exists
         ws.hdr->n_pairs_clamped = (unsigned int)min(total, (unsigned long long)max_pairs);
         const unsigned int ovf = (total > max_pairs ? 1u : 0u) | (too_long ? 2u : 0u);

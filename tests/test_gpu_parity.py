@@ -245,6 +245,30 @@ def test_tile_counts_of_rects_across_tile_group_boundaries(pkg):
     r.close()
 
 
+def test_screen_filling_rects_shared_counter_duplication(pkg):
+    """Step a6 on frames of VERY large rects (mean above 1024 tiles per Gaussian): k_duplicate_shared by default, without
+    the test knob.  300 Gaussians that each cover most of a 592 x 560 image (37 x 35 = 1295 tiles) plus a few small
+    ones; counts, sorted sequence and image against the oracle under both pair rules."""
+    rng = np.random.default_rng(77)
+    W, H, f, z = 592, 560, 120.0, 6.0
+    n_big, n_small = 300, 40
+    mean = np.concatenate([np.c_[rng.uniform(-2, 2, n_big), rng.uniform(-2, 2, n_big), z + rng.uniform(0, 3, n_big)],
+                           np.c_[rng.uniform(-10, 10, n_small), rng.uniform(-10, 10, n_small), z + rng.uniform(0, 3, n_small)]])
+    scale = np.concatenate([np.exp(rng.uniform(2.0, 2.6, (n_big, 3))), np.exp(rng.uniform(-3, -2, (n_small, 3)))])
+    q = rng.normal(size=(n_big + n_small, 4)); q /= np.linalg.norm(q, axis=1, keepdims=True)
+    lv = [level(1, 0.0, mean, scale, quat=q, opacity=rng.uniform(0.02, 0.3, n_big + n_small), rgb=rng.uniform(0, 1, (n_big + n_small, 3)))]
+    cam = camera(width=W, height=H, f=f, bg=(0.2, 0.1, 0.0))
+    osc = OracleScene(lv, 0)
+    r = make_renderer(pkg, lv, 0, W, H, max_pairs=1 << 20)
+    for rule in (pkg.PAIR_RULE_BOX, pkg.PAIR_RULE_ELLIPSE):
+        r.set_pair_rule(rule)
+        (dmax, nm), img, fr = check_frame(r, osc, cam, 1, 1, 1.0)
+        if rule == pkg.PAIR_RULE_BOX:
+            assert fr.counts["n_pairs"] > 1024 * fr.counts["n_vis"]        # the default threshold of the shared-counter kernel
+        check_frame(r, osc, cam, 1, 1, 1.0)                                # (a second frame: after the hint reached the host)
+    r.close()
+
+
 def test_empty_scene_and_all_culled(pkg):
     """nothing to draw -> background; also everything behind the camera / dead."""
     lv = level(1, 0.0, np.zeros((0, 3)), 0.1)
@@ -598,7 +622,8 @@ def test_subset_small_scenes_errors_and_empty_selection(pkg):
 @pytest.mark.parametrize("seed", [100, 102, 105, 108, 111, 114, 120, 132])
 def test_random_scenes_every_kernel_path(pkg, seed):
     """Random level counts, SH degrees, image sizes and footprints (every third seed: large footprints, mean rect area
-    up to hundreds of tiles -> k_duplicate_shared; every fourth: its tile windows), every checked intermediate and the
+    up to hundreds of tiles; every fourth: FLOD_OPT_SMALL_WINDOWS -> k_duplicate_shared and its tile windows from a mean
+    rect of 128 tiles; seeds 108, 120, 132 are both), every checked intermediate and the
     image on the fused path, then the materialised-subset path at a random reference: bit-identical to the fused
     predicate and within tolerance of the oracle."""
     rng = np.random.default_rng(seed)
