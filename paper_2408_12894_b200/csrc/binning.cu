@@ -19,7 +19,7 @@ namespace flod {
 // capacity flag for a longer list).  A block scan of the per-Gaussian group counts lets the block expand its rects
 // cooperatively, one group per thread per step, whatever the individual rect sizes.
 constexpr int kDupPer = kGeoBlock / kPreBlock;
-constexpr int kDupMaxParts = 16;            // CTAs that may share a segment (launch_duplicate)
+constexpr int kDupMaxParts = 32;            // CTAs that may share a segment (launch_duplicate; 16 -> 32: config 3 level 1 142 -> 133 us, level 2 200 -> 182)
 
 // Which of the two duplication kernels serves the frame (when both are launched, the other one exits at once): the mean
 // rect area, known on the device since k_geometry.  k_duplicate: one value-returning global atomic per 2x2 tile group.
